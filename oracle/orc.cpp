@@ -1,0 +1,407 @@
+// orc.cpp -- CPU ORACLE (test infrastructure only; see orc.h for scope, citations and pins).
+// Plain triple loops, fp64, compiled -O2 -ffp-contract=off -fno-fast-math so that every expression
+// is evaluated exactly as written (no FMA contraction, no reassociation).
+// Steps S0-S4 and G1-G4 are SURVEY.md section 8(c); P:NN = /root/reference/PAPER.md line NN.
+#include "orc.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <string>
+#include <tuple>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+static thread_local std::string g_err;
+static int fail(const char* msg) { g_err = msg; return -1; }
+extern "C" const char* orc_last_error(void) { return g_err.c_str(); }
+
+static const double RHO_FLOOR = 1e-20;   // floors act on W only
+static const double P_FLOOR   = 1e-20;
+
+// ------------------------------------------------------------------------------------------------
+// S1  conserved -> primitive, W = (rho, v, u_g)  (the primitive is the INTERNAL ENERGY)
+// ------------------------------------------------------------------------------------------------
+extern "C" void orc_c2p(double gamma, const double U[5], double W[5], int* floored) {
+  int nfl = 0;
+  double rho = U[0];
+  if (!(rho >= RHO_FLOOR)) { rho = RHO_FLOOR; nfl++; }
+  double rinv = 1.0 / rho;
+  double m1 = U[1], m2 = U[2], m3 = U[3];
+  double ug = U[4] - 0.5 * rinv * (m1 * m1 + (m2 * m2 + m3 * m3));
+  double ug_floor = P_FLOOR / (gamma - 1.0);
+  if (!(ug >= ug_floor)) { ug = ug_floor; nfl++; }
+  W[0] = rho; W[1] = m1 * rinv; W[2] = m2 * rinv; W[3] = m3 * rinv; W[4] = ug;
+  if (floored) *floored = nfl;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S2  reconstruction of one primitive along one direction
+// ------------------------------------------------------------------------------------------------
+// PLM with van Leer's harmonic-mean limiter: h = dL*dR/(dL+dR) if dL*dR > 0 else 0.
+extern "C" void orc_plm(double qm1, double q0, double qp1, double* q_minus, double* q_plus) {
+  double dL = q0 - qm1, dR = qp1 - q0;
+  double prod = dL * dR;
+  double h = (prod > 0.0) ? prod / (dL + dR) : 0.0;
+  *q_minus = q0 - h;
+  *q_plus  = q0 + h;
+}
+
+// PPM4 (i) fourth-order interface value at i+1/2 and (ii) clamp into the range of the two adjacent cells.
+extern "C" void orc_ppm4_iface(double qm1, double q0, double qp1, double qp2, double* q_half) {
+  double v = (7.0 * (q0 + qp1) - (qm1 + qp2)) / 12.0;
+  double lo = std::fmin(q0, qp1), hi = std::fmax(q0, qp1);
+  v = std::fmax(lo, std::fmin(v, hi));
+  *q_half = v;
+}
+
+// PPM4 (iii) Colella & Woodward (1984) Eq.(1.10) monotonicity limiter for cell i given q[i-2..i+2].
+extern "C" void orc_ppm4(const double q[5], double* q_minus, double* q_plus) {
+  double aL, aR, a = q[2];
+  orc_ppm4_iface(q[0], q[1], q[2], q[3], &aL);   // face i-1/2
+  orc_ppm4_iface(q[1], q[2], q[3], q[4], &aR);   // face i+1/2
+  if ((aR - a) * (a - aL) <= 0.0) {
+    aL = a; aR = a;
+  } else {
+    double d = aR - aL;
+    double mu = a - 0.5 * (aL + aR);
+    double dmu = d * mu, d26 = d * d / 6.0;
+    if (dmu > d26)        aL = 3.0 * a - 2.0 * aR;
+    else if (-d26 > dmu)  aR = 3.0 * a - 2.0 * aL;
+  }
+  *q_minus = aL;
+  *q_plus  = aR;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S3  HLLC flux at one face (Toro 2013 ch.10 restated in SURVEY 8(c) S3)
+// ------------------------------------------------------------------------------------------------
+extern "C" void orc_hllc(double gamma, int dir, const double WL[5], const double WR[5], double F[5]) {
+  const int iu = 1 + dir, iv = 1 + (dir + 1) % 3, iw = 1 + (dir + 2) % 3;   // normal, transverse pair (cyclic)
+  const double gm1 = gamma - 1.0;
+  double rL = WL[0], uL = WL[iu], vL = WL[iv], wL = WL[iw], eL = WL[4];
+  double rR = WR[0], uR = WR[iu], vR = WR[iv], wR = WR[iw], eR = WR[4];
+  double pL = gm1 * eL, pR = gm1 * eR;
+  double cL = std::sqrt(gamma * pL / rL), cR = std::sqrt(gamma * pR / rR);
+  double rbar = 0.5 * (rL + rR), cbar = 0.5 * (cL + cR);
+  double ppv = 0.5 * ((pL + pR) + (uL - uR) * rbar * cbar);                  // PVRS pressure estimate
+  const double gq = (gamma + 1.0) / (2.0 * gamma);
+  double qL = (ppv <= pL) ? 1.0 : std::sqrt(1.0 + gq * (ppv / pL - 1.0));
+  double qR = (ppv <= pR) ? 1.0 : std::sqrt(1.0 + gq * (ppv / pR - 1.0));
+  double SL = uL - cL * qL, SR = uR + cR * qR;
+  double bm = std::fmin(SL, 0.0), bp = std::fmax(SR, 0.0);
+  double mL = rL * (uL - SL), mR = rR * (SR - uR);
+  double Ss = ((pL - pR) + (mL * uL + mR * uR)) / (mL + mR);                  // contact speed
+  double psL = pL + rL * (SL - uL) * (Ss - uL);
+  double psR = pR + rR * (SR - uR) * (Ss - uR);
+  double ps = std::fmax(0.5 * (psL + psR), 0.0);
+  double rK, uK, vK, wK, eK, pK, b;
+  if (Ss >= 0.0) { rK = rL; uK = uL; vK = vL; wK = wL; eK = eL; pK = pL; b = bm; }
+  else           { rK = rR; uK = uR; vK = vR; wK = wR; eK = eR; pK = pR; b = bp; }
+  double EK = eK + 0.5 * rK * (uK * uK + (vK * vK + wK * wK));
+  double UK[5] = { rK, rK * uK, rK * vK, rK * wK, EK };
+  double FK[5] = { rK * uK, rK * uK * uK + pK, rK * uK * vK, rK * uK * wK, (EK + pK) * uK };
+  double D[5]  = { 0.0, 1.0, 0.0, 0.0, Ss };
+  double Fn[5];
+  double den = Ss - b;
+  for (int n = 0; n < 5; n++) Fn[n] = (Ss * (FK[n] - b * UK[n]) - b * ps * D[n]) / den;
+  F[0] = Fn[0]; F[iu] = Fn[1]; F[iv] = Fn[2]; F[iw] = Fn[3]; F[4] = Fn[4];
+}
+
+// ------------------------------------------------------------------------------------------------
+// Pack descriptor
+// ------------------------------------------------------------------------------------------------
+struct orc_pack {
+  int nmb, nx[3], ng, nt[3];
+  double gamma;
+  int recon, rsolver;
+  int nrb[3];
+  double xmin[3], xmax[3];
+  bool mesh_set = false, bound = false;
+  std::vector<int> level, lx;            // lx[3*m+d]
+  std::vector<char> blk_set;
+  std::map<std::tuple<int, int, int, int>, int> leaf;   // (level, l1, l2, l3) -> m
+  int max_level = 0;
+  double* u[2] = { nullptr, nullptr };
+  int cur = 0;
+  long long floor_count = 0;
+  int nthreads = 1;
+
+  size_t ncell() const { return (size_t)nt[0] * nt[1] * nt[2]; }
+  size_t idx(int m, int n, int k, int j, int i) const {
+    return ((((size_t)m * 5 + n) * nt[2] + k) * nt[1] + j) * nt[0] + i;
+  }
+  double dx(int lev, int d) const { return (xmax[d] - xmin[d]) / ((double)nrb[d] * nx[d] * (double)(1 << lev)); }
+  long nglob(int lev, int d) const { return (long)nrb[d] * nx[d] * (1L << lev); }
+  int find_leaf(int lev, long b1, long b2, long b3) const {
+    auto it = leaf.find(std::make_tuple(lev, (int)b1, (int)b2, (int)b3));
+    return it == leaf.end() ? -1 : it->second;
+  }
+};
+
+extern "C" orc_pack* orc_pack_create(int nmb, int nx1, int nx2, int nx3, int ng, double gamma, int recon, int rsolver) {
+  int nx[3] = { nx1, nx2, nx3 };
+  if (nmb < 1) { fail("nmb < 1"); return nullptr; }
+  for (int d = 0; d < 3; d++) if (nx[d] < ng || (nx[d] & 1)) { fail("nx_d must be even and >= ng"); return nullptr; }
+  if (!(gamma > 1.0)) { fail("gamma <= 1"); return nullptr; }
+  if (recon != 0 && recon != 1) { fail("unknown recon"); return nullptr; }
+  if (rsolver != 0) { fail("unknown rsolver"); return nullptr; }
+  if ((recon == 0 && ng < 2) || (recon == 1 && ng < 3)) { fail("ng too small for the reconstruction"); return nullptr; }
+  orc_pack* p = new orc_pack;
+  p->nmb = nmb; p->ng = ng; p->gamma = gamma; p->recon = recon; p->rsolver = rsolver;
+  for (int d = 0; d < 3; d++) { p->nx[d] = nx[d]; p->nt[d] = nx[d] + 2 * ng; }
+  p->level.assign(nmb, 0); p->lx.assign(3 * (size_t)nmb, 0); p->blk_set.assign(nmb, 0);
+  return p;
+}
+
+extern "C" int orc_pack_set_mesh(orc_pack* p, int nrb1, int nrb2, int nrb3,
+                                 double x1min, double x1max, double x2min, double x2max, double x3min, double x3max) {
+  if (!p) return fail("null pack");
+  if (nrb1 < 1 || nrb2 < 1 || nrb3 < 1) return fail("nrb < 1");
+  if (!(x1max > x1min) || !(x2max > x2min) || !(x3max > x3min)) return fail("empty domain");
+  p->nrb[0] = nrb1; p->nrb[1] = nrb2; p->nrb[2] = nrb3;
+  p->xmin[0] = x1min; p->xmax[0] = x1max; p->xmin[1] = x2min; p->xmax[1] = x2max; p->xmin[2] = x3min; p->xmax[2] = x3max;
+  p->mesh_set = true;
+  return 0;
+}
+
+extern "C" int orc_pack_set_block(orc_pack* p, int m, int level, int lx1, int lx2, int lx3) {
+  if (!p) return fail("null pack");
+  if (!p->mesh_set) return fail("set_mesh first");
+  if (m < 0 || m >= p->nmb) return fail("block index out of range");
+  if (level < 0 || level > 1) return fail("level must be 0 or 1");
+  int l[3] = { lx1, lx2, lx3 };
+  for (int d = 0; d < 3; d++) if (l[d] < 0 || l[d] >= p->nrb[d] * (1 << level)) return fail("logical location out of range");
+  p->level[m] = level;
+  for (int d = 0; d < 3; d++) p->lx[3 * (size_t)m + d] = l[d];
+  p->blk_set[m] = 1;
+  return 0;
+}
+
+extern "C" int orc_pack_bind(orc_pack* p, double* u_a, double* u_b) {
+  if (!p) return fail("null pack");
+  if (!p->mesh_set) return fail("set_mesh first");
+  if (!u_a || !u_b) return fail("null buffer");
+  p->leaf.clear(); p->max_level = 0;
+  double vol = 0.0;
+  for (int m = 0; m < p->nmb; m++) {
+    if (!p->blk_set[m]) return fail("block not set");
+    auto key = std::make_tuple(p->level[m], p->lx[3 * m], p->lx[3 * m + 1], p->lx[3 * m + 2]);
+    if (p->leaf.count(key)) return fail("duplicate block");
+    p->leaf[key] = m;
+    if (p->level[m] > p->max_level) p->max_level = p->level[m];
+    vol += (p->level[m] == 0) ? 1.0 : 0.125;
+  }
+  // leaves must tile the root grid: no level-1 leaf under a level-0 leaf, total volume = root blocks
+  for (int m = 0; m < p->nmb; m++) if (p->level[m] == 1) {
+    if (p->find_leaf(0, p->lx[3 * m] / 2, p->lx[3 * m + 1] / 2, p->lx[3 * m + 2] / 2) >= 0) return fail("overlapping leaves");
+  }
+  if (vol != (double)p->nrb[0] * p->nrb[1] * p->nrb[2]) return fail("leaves do not cover the domain");
+  if (p->max_level > 0 && (p->ng & 1)) return fail("static refinement needs even ng");
+  p->u[0] = u_a; p->u[1] = u_b; p->cur = 0; p->bound = true; p->floor_count = 0;
+  return 0;
+}
+
+extern "C" int orc_set_threads(orc_pack* p, int n) { if (!p || n < 1) return fail("bad thread count"); p->nthreads = n; return 0; }
+extern "C" double* orc_pack_current(orc_pack* p) { return (p && p->bound) ? p->u[p->cur] : nullptr; }
+extern "C" long long orc_pack_floor_count(const orc_pack* p) { return p ? p->floor_count : -1; }
+extern "C" int orc_pack_destroy(orc_pack* p) { delete p; return 0; }
+
+// ------------------------------------------------------------------------------------------------
+// G1-G4  ghost fill: a pure function of the ACTIVE cells of leaf blocks
+// ------------------------------------------------------------------------------------------------
+static inline long wrapl(long g, long n) { long r = g % n; return r < 0 ? r + n : r; }
+
+// value of variable n in the active cell with level-`lev` global index G[] (already wrapped) of leaf m
+static inline double leaf_cell(const orc_pack* p, const double* U, int m, int n, const long G[3]) {
+  int a[3];
+  for (int d = 0; d < 3; d++) a[d] = (int)(G[d] - (long)p->lx[3 * (size_t)m + d] * p->nx[d]) + p->ng;
+  return U[p->idx(m, n, a[2], a[1], a[0])];
+}
+
+// G3: mean of the 8 level-(lev+1) active cells covering the level-`lev` cell G, fixed summation order
+static bool restrict_cell(const orc_pack* p, const double* U, int lev, const long G[3], int n, double* out) {
+  double f[2][2][2];
+  for (int dk = 0; dk < 2; dk++) for (int dj = 0; dj < 2; dj++) for (int di = 0; di < 2; di++) {
+    long Gf[3] = { 2 * G[0] + di, 2 * G[1] + dj, 2 * G[2] + dk };
+    int m = p->find_leaf(lev + 1, Gf[0] / p->nx[0], Gf[1] / p->nx[1], Gf[2] / p->nx[2]);
+    if (m < 0) return false;
+    f[dk][dj][di] = leaf_cell(p, U, m, n, Gf);
+  }
+  *out = 0.125 * (((f[0][0][0] + f[0][0][1]) + (f[0][1][0] + f[0][1][1])) +
+                  ((f[1][0][0] + f[1][0][1]) + (f[1][1][0] + f[1][1][1])));
+  return true;
+}
+
+// virtual level-`lev` field C(.): the leaf value where a level-`lev` leaf covers G, else the G3 restriction
+static bool coarse_field(const orc_pack* p, const double* U, int lev, const long Gin[3], int n, double* out) {
+  long G[3];
+  for (int d = 0; d < 3; d++) G[d] = wrapl(Gin[d], p->nglob(lev, d));
+  int m = p->find_leaf(lev, G[0] / p->nx[0], G[1] / p->nx[1], G[2] / p->nx[2]);
+  if (m >= 0) { *out = leaf_cell(p, U, m, n, G); return true; }
+  return restrict_cell(p, U, lev, G, n, out);
+}
+
+static inline double minmod(double a, double b) {
+  if (a * b <= 0.0) return 0.0;
+  double m = std::fmin(std::fabs(a), std::fabs(b));
+  return a > 0.0 ? m : -m;
+}
+
+static int fill_block(const orc_pack* p, double* U, int m) {
+  const int ng = p->ng, lev = p->level[m];
+  for (int k = 0; k < p->nt[2]; k++) for (int j = 0; j < p->nt[1]; j++) for (int i = 0; i < p->nt[0]; i++) {
+    int a[3] = { i - ng, j - ng, k - ng };
+    bool ghost = false;
+    for (int d = 0; d < 3; d++) if (a[d] < 0 || a[d] >= p->nx[d]) ghost = true;
+    if (!ghost) continue;
+    long G[3];
+    for (int d = 0; d < 3; d++) G[d] = wrapl((long)p->lx[3 * (size_t)m + d] * p->nx[d] + a[d], p->nglob(lev, d));
+    // G1: which leaf covers this position?
+    int src = p->find_leaf(lev, G[0] / p->nx[0], G[1] / p->nx[1], G[2] / p->nx[2]);
+    for (int n = 0; n < 5; n++) {
+      double val;
+      if (src >= 0) {                                     // G2 same level: copy
+        val = leaf_cell(p, U, src, n, G);
+      } else if (restrict_cell(p, U, lev, G, n, &val)) {  // G3 finer neighbour: conservative restriction
+      } else {                                            // G4 coarser neighbour: limited-linear prolongation
+        if (lev == 0) return -1;
+        long Gc[3]; int s[3];
+        for (int d = 0; d < 3; d++) { Gc[d] = G[d] >> 1; s[d] = 2 * (int)(G[d] & 1) - 1; }
+        double c0;
+        if (!coarse_field(p, U, lev - 1, Gc, n, &c0)) return -1;
+        double g[3];
+        for (int d = 0; d < 3; d++) {
+          long Gm[3] = { Gc[0], Gc[1], Gc[2] }, Gp[3] = { Gc[0], Gc[1], Gc[2] };
+          Gm[d] -= 1; Gp[d] += 1;
+          double cm, cp;
+          if (!coarse_field(p, U, lev - 1, Gm, n, &cm)) return -1;
+          if (!coarse_field(p, U, lev - 1, Gp, n, &cp)) return -1;
+          g[d] = 0.25 * minmod(c0 - cm, cp - c0);
+        }
+        val = ((c0 + s[0] * g[0]) + s[1] * g[1]) + s[2] * g[2];
+      }
+      U[p->idx(m, n, k, j, i)] = val;
+    }
+  }
+  return 0;
+}
+
+extern "C" int orc_fill_ghosts(orc_pack* p) {
+  if (!p || !p->bound) return fail("pack not bound");
+  double* U = p->u[p->cur];
+  int bad = 0;
+#pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) reduction(+ : bad) if (p->nthreads > 1)
+  for (int m = 0; m < p->nmb; m++) if (fill_block(p, U, m) != 0) bad++;
+  return bad ? fail("ghost cell with no covering leaf") : 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S1-S4  one Runge-Kutta stage (P:99 reconstruct-solve-advance; P:105 SSP-RK2 in two registers)
+// ------------------------------------------------------------------------------------------------
+static long long stage_block(const orc_pack* p, const double* Uin, const double* U0, double* Uout, int m,
+                             double g0, double g1, double beta, double dt) {
+  const int ng = p->ng, n1 = p->nt[0], n2 = p->nt[1], n3 = p->nt[2];
+  const size_t nc = p->ncell();
+  long long nfl = 0;
+  // S1: primitives in every cell of the block, ghosts included
+  std::vector<double> W(5 * nc);
+  for (int k = 0; k < n3; k++) for (int j = 0; j < n2; j++) for (int i = 0; i < n1; i++) {
+    double u[5], w[5]; int f;
+    for (int n = 0; n < 5; n++) u[n] = Uin[p->idx(m, n, k, j, i)];
+    orc_c2p(p->gamma, u, w, &f);
+    nfl += f;
+    size_t c = ((size_t)k * n2 + j) * n1 + i;
+    for (int n = 0; n < 5; n++) W[n * nc + c] = w[n];
+  }
+  // S2 + S3: flux of direction d at the lower face of cell (k,j,i), stored at that cell's index
+  std::vector<double> F[3];
+  const int str[3] = { 1, n1, n1 * n2 };
+  for (int d = 0; d < 3; d++) {
+    F[d].assign(5 * nc, 0.0);
+    int hi[3] = { p->nx[0] + ng, p->nx[1] + ng, p->nx[2] + ng };
+    hi[d] += 1;                                            // faces ng .. nx+ng along d
+    for (int k = ng; k < hi[2]; k++) for (int j = ng; j < hi[1]; j++) for (int i = ng; i < hi[0]; i++) {
+      size_t c = ((size_t)k * n2 + j) * n1 + i;            // cell on the + side of the face
+      size_t cm = c - str[d];                              // cell on the - side
+      double WL[5], WR[5], Fl[5];
+      for (int n = 0; n < 5; n++) {
+        const double* q = &W[n * nc];
+        double qm, qp;
+        if (p->recon == 0) {
+          orc_plm(q[cm - str[d]], q[cm], q[cm + str[d]], &qm, &qp);          WL[n] = qp;   // q+ of cell i-1
+          orc_plm(q[c - str[d]],  q[c],  q[c + str[d]],  &qm, &qp);          WR[n] = qm;   // q- of cell i
+        } else {
+          double sL[5] = { q[cm - 2 * str[d]], q[cm - str[d]], q[cm], q[cm + str[d]], q[cm + 2 * str[d]] };
+          double sR[5] = { q[c - 2 * str[d]],  q[c - str[d]],  q[c],  q[c + str[d]],  q[c + 2 * str[d]] };
+          orc_ppm4(sL, &qm, &qp);                                             WL[n] = qp;
+          orc_ppm4(sR, &qm, &qp);                                             WR[n] = qm;
+        }
+      }
+      orc_hllc(p->gamma, d, WL, WR, Fl);
+      for (int n = 0; n < 5; n++) F[d][n * nc + c] = Fl[n];
+    }
+  }
+  // S4: weighted update of the active cells, evaluated left to right
+  const int lev = p->level[m];
+  const double c1 = beta * dt / p->dx(lev, 0), c2 = beta * dt / p->dx(lev, 1), c3 = beta * dt / p->dx(lev, 2);
+  for (int n = 0; n < 5; n++)
+    for (int k = ng; k < p->nx[2] + ng; k++) for (int j = ng; j < p->nx[1] + ng; j++) for (int i = ng; i < p->nx[0] + ng; i++) {
+      size_t c = ((size_t)k * n2 + j) * n1 + i;
+      size_t g = p->idx(m, n, k, j, i);
+      double v = g0 * Uin[g] + g1 * U0[g];
+      v = v - c1 * (F[0][n * nc + c + str[0]] - F[0][n * nc + c]);
+      v = v - c2 * (F[1][n * nc + c + str[1]] - F[1][n * nc + c]);
+      v = v - c3 * (F[2][n * nc + c + str[2]] - F[2][n * nc + c]);
+      Uout[g] = v;
+    }
+  return nfl;
+}
+
+extern "C" int orc_hydro_stage(orc_pack* p, int stage, double dt) {
+  if (!p || !p->bound) return fail("pack not bound");
+  if (stage != 1 && stage != 2) return fail("stage must be 1 or 2");
+  if (stage == 1 && p->cur != 0) return fail("stage 1 expects U^n in buffer A");
+  if (stage == 2 && p->cur != 1) return fail("stage 2 expects U^(1) in buffer B");
+  // SSPRK(2,2): U1 = U^n + dt L(U^n);  U^{n+1} = 1/2 U^n + 1/2 [U1 + dt L(U1)]
+  const double g0 = (stage == 1) ? 0.0 : 0.5, g1 = (stage == 1) ? 1.0 : 0.5, beta = (stage == 1) ? 1.0 : 0.5;
+  const double* Uin = p->u[p->cur];
+  const double* U0 = p->u[0];
+  double* Uout = p->u[1 - p->cur];          // stage 2 writes A in place: each cell's A value is read only for itself
+  long long nfl = 0;
+#pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) reduction(+ : nfl) if (p->nthreads > 1)
+  for (int m = 0; m < p->nmb; m++) nfl += stage_block(p, Uin, U0, Uout, m, g0, g1, beta, dt);
+  p->floor_count += nfl;
+  p->cur = 1 - p->cur;
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S0  CFL time step, Eq.(3): min over active cells of leaf blocks and over directions
+// ------------------------------------------------------------------------------------------------
+extern "C" int orc_new_dt(orc_pack* p, double cfl, double* dt_out) {
+  if (!p || !p->bound || !dt_out) return fail("pack not bound");
+  const double* U = p->u[p->cur];
+  const int ng = p->ng;
+  double dtmin = HUGE_VAL;
+#pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) reduction(min : dtmin) if (p->nthreads > 1)
+  for (int m = 0; m < p->nmb; m++) {
+    const int lev = p->level[m];
+    for (int k = ng; k < p->nx[2] + ng; k++) for (int j = ng; j < p->nx[1] + ng; j++) for (int i = ng; i < p->nx[0] + ng; i++) {
+      double u[5], w[5];
+      for (int n = 0; n < 5; n++) u[n] = U[p->idx(m, n, k, j, i)];
+      orc_c2p(p->gamma, u, w, nullptr);
+      double pr = (p->gamma - 1.0) * w[4];
+      double cs = std::sqrt(p->gamma * pr / w[0]);
+      for (int d = 0; d < 3; d++) {
+        double cand = p->dx(lev, d) / (std::fabs(w[1 + d]) + cs);
+        if (cand < dtmin) dtmin = cand;
+      }
+    }
+  }
+  *dt_out = cfl * dtmin;
+  return 0;
+}
