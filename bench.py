@@ -1,0 +1,258 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path on the BASELINE.json headline workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference]
+
+One "step" = one full RK2 update of every active cell of the pack: ak_new_dt, then 2 x (ak_fill_ghosts,
+ak_hydro_stage).  Default workload = BASELINE.json configs[3]: 512^3 periodic mesh
+as 64 MeshBlocks of 128^3, PPM4 + HLLC, RK2, fp64, seeded synthetic initial state.  Prints ONE JSON line.
+N > 1 runs N independent replicas (the path does not shard: north_star).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "3D hydro cell-updates/sec (fp64)"
+UNIT = "cell-updates/s"
+BYTES_PER_CELL_UPDATE = 200.0      # 5 streams x 5 vars x 8 B per RK2 cell-update
+BYTES_STAGE = {1: 80.0, 2: 120.0}  # per active cell: stage 1 reads U^n writes U^(1); stage 2 reads U^(1),U^n writes
+
+
+def workloads():
+    from paper_2409_16053_b200 import inputs as I
+    return {
+        "cfg3": lambda: I.config3(),
+        "cfg3_small": lambda: I.config3(nrb=2, nx=64),
+        "cfg1": lambda: I.config1(),
+        "cfg2_16": lambda: I.config2(16), "cfg2_32": lambda: I.config2(32),
+        "cfg2_64": lambda: I.config2(64), "cfg2_128": lambda: I.config2(128),
+        "cfg4": lambda: I.config4(),
+        "table1": lambda: I.table1(),
+    }
+
+
+def measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (profiling guide recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 7 for n, v in zip(names, r[3:7]) if v.lower().startswith("active")})
+        pw = [float(r[2]) for r in self.rows if len(r) > 2 and r[2].replace(".", "").isdigit()]
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+def cpu_baseline(threads=1, target_s=12.0):
+    """The oracle as it stands on a bounded sample of the headline recipe (config 3 at 8 x 32^3 / 8 x 64^3)."""
+    from paper_2409_16053_b200 import inputs as I
+    from oracle import orc
+    w = I.config3(nrb=2, nx=32)
+    U0 = w.state().numpy()
+    p = orc.OrcPack(w.mesh, w.gamma, w.recon, threads=threads)
+    p.load(U0)
+    p.step(w.cfl)                                  # warm the caches / page in
+    t0, n = time.perf_counter(), 0
+    while True:
+        p.step(w.cfl)
+        n += 1
+        el = time.perf_counter() - t0
+        if el >= target_s or n >= 50:
+            break
+    p.close()
+    return {"value": w.mesh.ncells_active * n / el, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"config-3 recipe (PPM4+HLLC, Mach-1 modes + shear) on 8 MeshBlocks of 32^3, {n} RK2 steps, "
+                      f"{el:.1f} s, single-threaded C++ oracle"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cb = cpu_baseline(threads=1, target_s=max(5.0, min(60.0, 2.0 * (args.steps + args.warmup))))
+    from paper_2409_16053_b200 import inputs as I
+    w = I.config3()
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * w.mesh.ncells_active / cb["value"],
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "cfg3: 512^3 periodic, 64 MeshBlocks of 128^3, PPM4+HLLC, RK2 (oracle timed on a bounded "
+                               "sample of this workload; ms_per_step extrapolated to the full mesh)"},
+        "cpu_baseline": cb,
+        "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2409_16053_b200 import ak
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = workloads()[args.workload]()
+    mesh = w.mesh
+    pack = ak.Pack(mesh, w.gamma, w.recon, device=dev, variant=args.variant)
+    U0 = w.state(device=dev)
+    pack.load(U0)
+    ncell = mesh.ncells_active
+    state_bytes = U0.numel() * 8
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing ------------------------------------------------------------------
+    for _ in range(args.warmup):
+        pack.step(w.cfl)
+    stage_ev = []
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    l0 = pack.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(pack.stream)
+    for _ in range(args.steps):
+        dt = pack.new_dt(w.cfl)
+        for stage in (1, 2):
+            pack.fill_ghosts()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(pack.stream)
+            pack.hydro_stage(stage, dt)
+            b.record(pack.stream)
+            stage_ev.append((stage, a, b))
+    e1.record(pack.stream)
+    barrier()
+    clocks = sampler.stop()
+    launches = pack.launch_count() - l0
+    elapsed_ms = e0.elapsed_time(e1)
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    elapsed_ms = float(t.item())
+    floors = pack.floor_count()
+    value = world * ncell * args.steps / (elapsed_ms * 1e-3)
+
+    # dominant kernel = the stage kernel: algorithmic bytes per launch / mean launch duration
+    st_ms = {s: statistics.mean(a.elapsed_time(b) for ss, a, b in stage_ev if ss == s) for s in (1, 2)}
+    stage_ms = 0.5 * (st_ms[1] + st_ms[2])
+    alg_bytes = 0.5 * (BYTES_STAGE[1] + BYTES_STAGE[2]) * ncell
+    peaks, which = measured_peaks()
+    achieved = alg_bytes / (stage_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": achieved / peaks["hbm_gbs"], "traffic": args.traffic, "peak_source": which + " (MEASURED_PEAKS.json hbm_gbs)",
+                "kernel": "ak_hydro_stage", "kernel_ms": stage_ms, "kernel_share_of_step": 2 * stage_ms * args.steps / elapsed_ms,
+                "algorithmic_bytes_per_launch": alg_bytes,
+                "whole_step": {"achieved": BYTES_PER_CELL_UPDATE * value / world / 1e9,
+                               "frac": BYTES_PER_CELL_UPDATE * value / world / 1e9 / peaks["hbm_gbs"]}}
+
+    # ---- end to end through the C-ABI with HOST buffers ------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        host = torch.empty(U0.shape, dtype=torch.float64).pin_memory()
+        host.copy_(U0)
+        nst = max(1, min(args.steps, args.e2e_steps))
+        pack.upload(host); pack.step(w.cfl); pack.download(host)          # warm-up of the copy path
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(nst):
+            pack.upload(host)              # H2D of this step's input state (pinned)
+            pack.step(w.cfl)
+            pack.download(host)            # D2H of the step's result; synchronises
+        torch.cuda.synchronize(dev)
+        el = time.perf_counter() - t0
+        t = torch.tensor([el], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * ncell * nst / float(t.item()), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+               "d2h_bytes_per_step": state_bytes, "steps": nst}
+        del host
+
+    if rank == 0:
+        cb = None if args.no_cpu else cpu_baseline(threads=1)
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.workload}: {w.name}", "nmb": mesh.nmb, "nx": list(mesh.nx), "ng": mesh.ng,
+                       "recon": "PPM4" if w.recon else "PLM", "rsolver": "HLLC", "integrator": "SSPRK2", "cfl": w.cfl,
+                       "cells": ncell, "state_bytes": state_bytes, "l2_policy": "inputs larger than L2 (no flush needed)"
+                       if state_bytes > 4e8 else "state fits L2: numbers are L2-resident", "variant": args.variant,
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "roofline": roofline, "cpu_baseline": cb, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "stage_ms": st_ms, "floor_activations": floors,
+        }))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per stage launch from the committed ncu --set full capture (profiles/)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,131 @@
+/* ak.h -- C-ABI boundary of the B200-native MeshBlockPack hydro stage.
+ *
+ * The library advances Newtonian adiabatic hydrodynamics (paper Eq.(4), /root/reference/PAPER.md
+ * lines 122-126, cited below as P:NN) on a MeshBlockPack -- all MeshBlocks resident on one device
+ * and updated by one kernel launch -- stored as (N+1)-dimensional arrays
+ * U[m][n][k][j][i] that never leave device memory.  The host only sequences calls; every
+ * operation on the dependent variables runs in a CUDA kernel.
+ *
+ * One time step of the paper's method-of-lines RK2 scheme is
+ *
+ *     ak_new_dt(p, cfl, &dt);                        CFL rule, Eq.(3)
+ *     for stage in 1, 2:
+ *         ak_fill_ghosts(p);                         boundary kernels between stages
+ *         ak_hydro_stage(p, stage, dt);              reconstruct - solve - advance
+ *
+ * Memory ownership: the caller (PyTorch in this repo) allocates every device buffer and supplies
+ * the CUDA stream; the pack descriptor is a small host object that owns no device memory.
+ * All functions are host functions.  "device pointer" / "host pointer" is stated per argument.
+ * Threading: a pack is not thread-safe; different packs are independent.
+ * Errors: functions returning int give AK_OK (0) or a negative code; ak_last_error() returns a
+ * thread-local message for the last failing call.  Nothing throws.  Asynchronous CUDA errors
+ * surface at the next synchronising call (ak_new_dt, ak_pack_download, ak_pack_floor_count).
+ * There is no CPU fallback: without a CUDA device every compute call fails with AK_ECUDA.
+ */
+#ifndef AK_H
+#define AK_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define AK_OK            0
+#define AK_EINVAL      (-1)   /* bad argument                                   */
+#define AK_ESTATE      (-2)   /* call order violated (e.g. stage before fill)   */
+#define AK_EUNSUPPORTED (-3)  /* valid request outside the implemented scope    */
+#define AK_ECUDA       (-4)   /* CUDA runtime error, message in ak_last_error() */
+
+#define AK_RECON_PLM   0      /* piecewise linear, van Leer limiter     */
+#define AK_RECON_PPM4  1      /* piecewise parabolic, Colella-Woodward limiters */
+#define AK_RSOLVER_HLLC 0
+
+typedef struct ak_pack ak_pack;          /* opaque host-side descriptor */
+
+const char* ak_last_error(void);
+
+/* Create the descriptor of a pack of `nmb` MeshBlocks of nx1*nx2*nx3 active cells with `ng` ghost
+ * layers, gamma-law EOS p=(gamma-1)u_g, reconstruction and Riemann solver
+ * chosen at run time and instantiated as templates inside.
+ * Returns NULL on error.  Rejects: nmb<1, nx_d<ng, odd nx_d, ng<2 (PLM) or ng<3 (PPM4), ng>4,
+ * gamma<=1, unknown enums. */
+ak_pack* ak_pack_create(int nmb, int nx1, int nx2, int nx3, int ng,
+                        double gamma, int recon, int rsolver);
+
+/* Periodic root grid of nrb1*nrb2*nrb3 blocks on [x_min,x_max]^3, uniform Cartesian. */
+int ak_pack_set_mesh(ak_pack*, int nrb1, int nrb2, int nrb3,
+                     double x1min, double x1max, double x2min, double x2max,
+                     double x3min, double x3max);
+
+/* Logical location of block m in the block tree: level 0 (root) or 1 (refined once),
+ * 0 <= lx_d < nrb_d * 2^level.  Cell size of a block: (x_max-x_min)/(nrb_d*nx_d*2^level). */
+int ak_pack_set_block(ak_pack*, int m, int level, int lx1, int lx2, int lx3);
+
+/* Size in bytes of ONE state buffer, nmb*5*(nx1+2ng)*(nx2+2ng)*(nx3+2ng)*8, layout
+ * U[m][n][k][j][i], n = (rho, rho v1, rho v2, rho v3, E), i fastest, ghosts included. */
+size_t ak_pack_state_bytes(const ak_pack*);
+/* Size in bytes of the scratch buffer (block table, leaf lookup maps, reduction cells). */
+size_t ak_pack_scratch_bytes(const ak_pack*);
+
+/* Attach caller-owned DEVICE memory and a CUDA stream (cudaStream_t passed as void*; NULL = the
+ * legacy default stream).  u_a holds U^n and is the "current" buffer; u_b is the second RK
+ * register; scratch is ak_pack_scratch_bytes() long.  All three must be 256-byte aligned and
+ * must not overlap.  Validates that the blocks tile the domain (each root block is either a leaf
+ * or fully covered by its 8 children), that refinement uses even ng, builds the block table and
+ * leaf maps and uploads them into scratch (synchronises the stream once). */
+int ak_pack_bind(ak_pack*, void* u_a, void* u_b, void* scratch, void* cuda_stream);
+
+/* Fill every ghost cell (faces, edges, corners, depth ng) of the current buffer from the active
+ * cells of the leaf block that covers its periodic image: same level -> copy; finer
+ * neighbour -> conservative restriction (mean of 8, fixed order); coarser neighbour ->
+ * limited-linear (minmod) prolongation of the conserved variables.  Reads active cells only,
+ * writes ghost cells only; bit-exact against the oracle.  Asynchronous on the stream. */
+int ak_fill_ghosts(ak_pack*);
+
+/* One Runge-Kutta stage of SSP-RK2 in two registers:
+ *   stage 1:  B = A - dt L(A)-terms            (reads A, writes B, B becomes current)
+ *   stage 2:  A = 1/2 A + 1/2 (B + dt L(B))    (reads B and A, writes A, A becomes current)
+ * with L = -sum_d (F_d(i+1/2) - F_d(i-1/2))/dx_d, F from conserved->primitive, PLM/PPM4
+ * reconstruction of the primitives and the HLLC flux in x1, x2, x3, fused in one
+ * launch; face fluxes never reach device memory.  Requires ak_fill_ghosts on the current buffer
+ * since the last change (else AK_ESTATE).  Asynchronous on the stream. */
+int ak_hydro_stage(ak_pack*, int stage, double dt);
+
+/* CFL time step, Eq.(3): cfl * min over active cells of all blocks and over d of
+ * dx_d(level) / (|v_d| + c_s), one dt for all levels.  dt_out is a HOST pointer.
+ * Synchronises the stream. */
+int ak_new_dt(ak_pack*, double cfl, double* dt_out);
+
+/* Convenience: ak_new_dt, then 2 x (ak_fill_ghosts, ak_hydro_stage).  dt_out (HOST, may be NULL)
+ * receives the step taken.  If dt_fixed > 0 it is used instead of the CFL value (lock-step parity
+ * runs) and no reduction is launched. */
+int ak_step(ak_pack*, double cfl, double dt_fixed, double* dt_out);
+
+/* DEVICE pointer of the buffer holding the newest U (u_a or u_b). */
+void* ak_pack_current(const ak_pack*);
+
+/* Host <-> device transfer of one whole state buffer through the pack's stream.
+ * upload: HOST -> buffer A, which becomes current, ghosts marked unfilled (asynchronous; the host
+ * buffer must stay valid until the stream reaches the copy -- pinned memory makes it truly async).
+ * download: current buffer -> HOST, synchronises the stream. */
+int ak_pack_upload(ak_pack*, const void* host_u);
+int ak_pack_download(ak_pack*, void* host_u);
+
+/* Number of density / internal-energy floor activations in conserved->primitive since bind
+ * (diagnostic; 0 on all BASELINE configs).  Synchronises the stream.  Negative on error. */
+long long ak_pack_floor_count(ak_pack*);
+
+/* Selects the implementation of ak_hydro_stage: 0 = tiled plane-marching kernel (default),
+ * 1 = straightforward one-thread-per-cell kernel kept as a cross-check.  Both give the same
+ * results to rounding. */
+int ak_pack_set_variant(ak_pack*, int variant);
+
+/* Number of kernel launches issued through this pack since bind (for bench.py's gpu_launches). */
+long long ak_pack_launch_count(const ak_pack*);
+
+/* Frees the host descriptor only; device buffers belong to the caller. */
+int ak_pack_destroy(ak_pack*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

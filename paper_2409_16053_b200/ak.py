@@ -1,0 +1,165 @@
+"""Thin binding over libak.so (include/ak.h): argument marshalling only.
+
+Every step of the path runs inside the library's CUDA kernels; PyTorch is used here to allocate device
+memory and to supply the stream (P:63 device-resident arrays, P:65 host drives / device computes).
+There is no CPU fallback: if the library is missing or cannot be loaded, importing the symbols raises.
+The function names mirror the C-ABI one to one.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libak.so")
+_lib = None
+
+AK_OK = 0
+RECON_PLM, RECON_PPM4 = 0, 1
+RSOLVER_HLLC = 0
+
+SYMBOLS = [
+    "ak_last_error", "ak_pack_create", "ak_pack_set_mesh", "ak_pack_set_block", "ak_pack_state_bytes",
+    "ak_pack_scratch_bytes", "ak_pack_bind", "ak_fill_ghosts", "ak_hydro_stage", "ak_new_dt", "ak_step",
+    "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_floor_count", "ak_pack_set_variant",
+    "ak_pack_launch_count", "ak_pack_destroy",
+]
+
+
+class AkError(RuntimeError):
+    pass
+
+
+def lib():
+    """Load libak.so (built in-tree by paper_2409_16053_b200.build).  Raises if it is absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_SO):
+        raise AkError(f"{_SO} not found: run `python -m paper_2409_16053_b200.build` (no CPU fallback exists)")
+    L = C.CDLL(_SO)
+    vp, i, d, sz, ll = C.c_void_p, C.c_int, C.c_double, C.c_size_t, C.c_longlong
+    sig = {
+        "ak_last_error": (C.c_char_p, []),
+        "ak_pack_create": (vp, [i, i, i, i, i, d, i, i]),
+        "ak_pack_set_mesh": (i, [vp, i, i, i, d, d, d, d, d, d]),
+        "ak_pack_set_block": (i, [vp, i, i, i, i, i]),
+        "ak_pack_state_bytes": (sz, [vp]),
+        "ak_pack_scratch_bytes": (sz, [vp]),
+        "ak_pack_bind": (i, [vp, vp, vp, vp, vp]),
+        "ak_fill_ghosts": (i, [vp]),
+        "ak_hydro_stage": (i, [vp, i, d]),
+        "ak_new_dt": (i, [vp, d, C.POINTER(d)]),
+        "ak_step": (i, [vp, d, d, C.POINTER(d)]),
+        "ak_pack_current": (vp, [vp]),
+        "ak_pack_upload": (i, [vp, vp]),
+        "ak_pack_download": (i, [vp, vp]),
+        "ak_pack_floor_count": (ll, [vp]),
+        "ak_pack_set_variant": (i, [vp, i]),
+        "ak_pack_launch_count": (ll, [vp]),
+        "ak_pack_destroy": (i, [vp]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = L
+    return L
+
+
+def _chk(rc):
+    if rc != AK_OK:
+        raise AkError(f"ak error {rc}: {lib().ak_last_error().decode()}")
+
+
+class Pack:
+    """A MeshBlockPack bound to torch-owned device buffers.  Methods map 1:1 to the ak_* calls."""
+
+    def __init__(self, mesh, gamma, recon, rsolver=RSOLVER_HLLC, device="cuda:0", stream=None, variant=0):
+        L = lib()
+        if not torch.cuda.is_available():
+            raise AkError("no CUDA device: the hydro path has no CPU fallback")
+        self.mesh = mesh
+        self.device = torch.device(device)
+        self._h = L.ak_pack_create(mesh.nmb, *mesh.nx, mesh.ng, gamma, recon, rsolver)
+        if not self._h:
+            raise AkError(L.ak_last_error().decode())
+        _chk(L.ak_pack_set_mesh(self._h, *mesh.nrb, mesh.xmin[0], mesh.xmax[0], mesh.xmin[1], mesh.xmax[1],
+                                mesh.xmin[2], mesh.xmax[2]))
+        for m, (lev, l1, l2, l3) in enumerate(mesh.blocks):
+            _chk(L.ak_pack_set_block(self._h, m, lev, l1, l2, l3))
+        nbytes = L.ak_pack_state_bytes(self._h)
+        assert nbytes == 8 * int(torch.tensor(mesh.state_shape()).prod())
+        with torch.cuda.device(self.device):
+            self.ua = torch.zeros(mesh.state_shape(), dtype=torch.float64, device=self.device)
+            self.ub = torch.zeros(mesh.state_shape(), dtype=torch.float64, device=self.device)
+            self.scratch = torch.zeros(L.ak_pack_scratch_bytes(self._h), dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            torch.cuda.synchronize(self.device)
+            _chk(L.ak_pack_bind(self._h, self.ua.data_ptr(), self.ub.data_ptr(), self.scratch.data_ptr(),
+                                self.stream.cuda_stream))
+        if variant:
+            _chk(L.ak_pack_set_variant(self._h, variant))
+
+    # ---- state -----------------------------------------------------------------------------------
+    def load(self, U):
+        """Device-side load of U^n (tensor of mesh.state_shape()) into buffer A; A becomes current."""
+        with torch.cuda.stream(self.stream):
+            self.ua.copy_(U.to(self.device, non_blocking=True))
+        self.stream.synchronize()
+        _chk(lib().ak_pack_bind(self._h, self.ua.data_ptr(), self.ub.data_ptr(), self.scratch.data_ptr(),
+                                self.stream.cuda_stream))
+
+    def current(self) -> torch.Tensor:
+        p = lib().ak_pack_current(self._h)
+        return self.ua if p == self.ua.data_ptr() else self.ub
+
+    def upload(self, host_tensor):
+        """ak_pack_upload: HOST (ideally pinned) tensor -> buffer A through the C-ABI."""
+        assert host_tensor.device.type == "cpu" and host_tensor.is_contiguous() and host_tensor.dtype == torch.float64
+        _chk(lib().ak_pack_upload(self._h, host_tensor.data_ptr()))
+
+    def download(self, host_tensor):
+        assert host_tensor.device.type == "cpu" and host_tensor.is_contiguous() and host_tensor.dtype == torch.float64
+        _chk(lib().ak_pack_download(self._h, host_tensor.data_ptr()))
+
+    # ---- the hot path ----------------------------------------------------------------------------
+    def fill_ghosts(self):
+        _chk(lib().ak_fill_ghosts(self._h))
+
+    def hydro_stage(self, stage, dt):
+        _chk(lib().ak_hydro_stage(self._h, stage, dt))
+
+    def new_dt(self, cfl):
+        dt = C.c_double()
+        _chk(lib().ak_new_dt(self._h, cfl, C.byref(dt)))
+        return dt.value
+
+    def step(self, cfl, dt=None):
+        out = C.c_double()
+        _chk(lib().ak_step(self._h, cfl, 0.0 if dt is None else dt, C.byref(out)))
+        return out.value
+
+    def floor_count(self):
+        n = lib().ak_pack_floor_count(self._h)
+        if n < 0:
+            raise AkError(lib().ak_last_error().decode())
+        return n
+
+    def launch_count(self):
+        return lib().ak_pack_launch_count(self._h)
+
+    def set_variant(self, v):
+        _chk(lib().ak_pack_set_variant(self._h, v))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().ak_pack_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,247 @@
+// ak_api.cu -- the C-ABI of include/ak.h: pack descriptor, mesh validation, table upload and the
+// host-side sequencing of kernel launches (the host drives, the device computes).
+#include "../../include/ak.h"
+#include "ak_pack.h"
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+static thread_local std::string g_err;
+static int fail(int code, const std::string& msg) { g_err = msg; return code; }
+static int cuda_fail(cudaError_t e, const char* where) {
+  return fail(AK_ECUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define AK_CUDA(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, where); } while (0)
+
+extern "C" const char* ak_last_error(void) { return g_err.c_str(); }
+
+static size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
+
+// scratch layout: [0,256) reduction cells | block table int4[nmb] | leaf0 | leaf1
+struct ScratchLayout { size_t blk, leaf0, leaf1, total; };
+static ScratchLayout scratch_layout(const ak_pack* p) {
+  ScratchLayout s;
+  const ak::PackDev& d = p->d;
+  size_t n0 = (size_t)d.nrb[0] * d.nrb[1] * d.nrb[2];
+  s.blk = 256;
+  s.leaf0 = s.blk + align256(sizeof(int4) * (size_t)d.nmb);
+  s.leaf1 = s.leaf0 + align256(sizeof(int) * n0);
+  s.total = s.leaf1 + align256(sizeof(int) * 8 * n0);
+  return s;
+}
+
+extern "C" ak_pack* ak_pack_create(int nmb, int nx1, int nx2, int nx3, int ng, double gamma, int recon, int rsolver) {
+  int nx[3] = {nx1, nx2, nx3};
+  if (nmb < 1) { fail(AK_EINVAL, "nmb < 1"); return nullptr; }
+  if (ng > 4) { fail(AK_EINVAL, "ng > 4"); return nullptr; }
+  for (int d = 0; d < 3; d++)
+    if (nx[d] < ng || (nx[d] & 1) || nx[d] < 2) { fail(AK_EINVAL, "nx_d must be even and >= ng"); return nullptr; }
+  if (!(gamma > 1.0)) { fail(AK_EINVAL, "gamma <= 1"); return nullptr; }
+  if (recon != AK_RECON_PLM && recon != AK_RECON_PPM4) { fail(AK_EINVAL, "unknown recon"); return nullptr; }
+  if (rsolver != AK_RSOLVER_HLLC) { fail(AK_EINVAL, "unknown rsolver"); return nullptr; }
+  if ((recon == AK_RECON_PLM && ng < 2) || (recon == AK_RECON_PPM4 && ng < 3)) {
+    fail(AK_EINVAL, "ng too small for the reconstruction stencil"); return nullptr;
+  }
+  long long ncell = (long long)(nx1 + 2 * ng) * (nx2 + 2 * ng) * (nx3 + 2 * ng);
+  if (ncell * 5 * nmb >= (1ll << 40)) { fail(AK_EUNSUPPORTED, "pack too large"); return nullptr; }
+  if ((long long)nx2 * nx3 > 65535 || nmb > 65535) { fail(AK_EUNSUPPORTED, "grid dimension limit"); return nullptr; }
+  ak_pack* p = new ak_pack;
+  p->d.nmb = nmb; p->d.ng = ng; p->d.gamma = gamma; p->d.ncell = ncell;
+  for (int d = 0; d < 3; d++) { p->d.nx[d] = nx[d]; p->d.nt[d] = nx[d] + 2 * ng; p->d.nrb[d] = 0; }
+  p->recon = recon; p->rsolver = rsolver;
+  p->level.assign(nmb, 0); p->lx.assign(3 * (size_t)nmb, 0); p->blk_set.assign(nmb, 0);
+  return p;
+}
+
+extern "C" int ak_pack_set_mesh(ak_pack* p, int nrb1, int nrb2, int nrb3, double x1min, double x1max,
+                                double x2min, double x2max, double x3min, double x3max) {
+  if (!p) return fail(AK_EINVAL, "null pack");
+  if (nrb1 < 1 || nrb2 < 1 || nrb3 < 1) return fail(AK_EINVAL, "nrb < 1");
+  if (!(x1max > x1min) || !(x2max > x2min) || !(x3max > x3min)) return fail(AK_EINVAL, "empty domain");
+  int nrb[3] = {nrb1, nrb2, nrb3};
+  for (int d = 0; d < 3; d++) if ((long long)nrb[d] * p->d.nx[d] * 2 > (1ll << 30)) return fail(AK_EUNSUPPORTED, "mesh too large");
+  p->d.nrb[0] = nrb1; p->d.nrb[1] = nrb2; p->d.nrb[2] = nrb3;
+  p->xmin[0] = x1min; p->xmax[0] = x1max; p->xmin[1] = x2min; p->xmax[1] = x2max; p->xmin[2] = x3min; p->xmax[2] = x3max;
+  for (int d = 0; d < 3; d++) p->d.dx0[d] = (p->xmax[d] - p->xmin[d]) / ((double)nrb[d] * p->d.nx[d] * 1.0);
+  p->mesh_set = true; p->bound = false;
+  return AK_OK;
+}
+
+extern "C" int ak_pack_set_block(ak_pack* p, int m, int level, int lx1, int lx2, int lx3) {
+  if (!p) return fail(AK_EINVAL, "null pack");
+  if (!p->mesh_set) return fail(AK_ESTATE, "ak_pack_set_mesh first");
+  if (m < 0 || m >= p->d.nmb) return fail(AK_EINVAL, "block index out of range");
+  if (level < 0) return fail(AK_EINVAL, "negative level");
+  if (level > 1) return fail(AK_EUNSUPPORTED, "only levels 0 and 1 are supported");
+  int l[3] = {lx1, lx2, lx3};
+  for (int d = 0; d < 3; d++) if (l[d] < 0 || l[d] >= (p->d.nrb[d] << level)) return fail(AK_EINVAL, "logical location out of range");
+  p->level[m] = level;
+  for (int d = 0; d < 3; d++) p->lx[3 * (size_t)m + d] = l[d];
+  p->blk_set[m] = 1; p->bound = false;
+  return AK_OK;
+}
+
+extern "C" size_t ak_pack_state_bytes(const ak_pack* p) { return p ? (size_t)p->d.nmb * 5 * (size_t)p->d.ncell * 8 : 0; }
+extern "C" size_t ak_pack_scratch_bytes(const ak_pack* p) { return (p && p->mesh_set) ? scratch_layout(p).total : 0; }
+
+extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, void* cuda_stream) {
+  if (!p) return fail(AK_EINVAL, "null pack");
+  if (!p->mesh_set) return fail(AK_ESTATE, "ak_pack_set_mesh first");
+  if (!u_a || !u_b || !scratch) return fail(AK_EINVAL, "null device buffer");
+  if (((uintptr_t)u_a | (uintptr_t)u_b | (uintptr_t)scratch) & 255) return fail(AK_EINVAL, "buffers must be 256-byte aligned");
+  const size_t sb = ak_pack_state_bytes(p);
+  auto overlap = [](const void* a, size_t na, const void* b, size_t nb) {
+    return (uintptr_t)a < (uintptr_t)b + nb && (uintptr_t)b < (uintptr_t)a + na;
+  };
+  const ScratchLayout sl = scratch_layout(p);
+  if (overlap(u_a, sb, u_b, sb) || overlap(u_a, sb, scratch, sl.total) || overlap(u_b, sb, scratch, sl.total))
+    return fail(AK_EINVAL, "device buffers overlap");
+  ak::PackDev& d = p->d;
+  // ---- validate the block list: leaves must tile the root grid (P:59 block tree, two levels) ----
+  const size_t n0 = (size_t)d.nrb[0] * d.nrb[1] * d.nrb[2];
+  std::vector<int> leaf0(n0, -1), leaf1(8 * n0, -1);
+  d.max_level = 0;
+  for (int m = 0; m < d.nmb; m++) {
+    if (!p->blk_set[m]) return fail(AK_ESTATE, "ak_pack_set_block missing for a block");
+    const int* l = &p->lx[3 * (size_t)m];
+    if (p->level[m] == 0) {
+      size_t k = ((size_t)l[2] * d.nrb[1] + l[1]) * d.nrb[0] + l[0];
+      if (leaf0[k] >= 0) return fail(AK_EINVAL, "duplicate block");
+      leaf0[k] = m;
+    } else {
+      size_t k = ((size_t)l[2] * 2 * d.nrb[1] + l[1]) * 2 * d.nrb[0] + l[0];
+      if (leaf1[k] >= 0) return fail(AK_EINVAL, "duplicate block");
+      leaf1[k] = m;
+      d.max_level = 1;
+    }
+  }
+  for (int b3 = 0; b3 < d.nrb[2]; b3++) for (int b2 = 0; b2 < d.nrb[1]; b2++) for (int b1 = 0; b1 < d.nrb[0]; b1++) {
+    int nchild = 0;
+    for (int c = 0; c < 8; c++) {
+      size_t k = ((size_t)(2 * b3 + (c >> 2)) * 2 * d.nrb[1] + (2 * b2 + ((c >> 1) & 1))) * 2 * d.nrb[0] + (2 * b1 + (c & 1));
+      if (leaf1[k] >= 0) nchild++;
+    }
+    bool root_leaf = leaf0[((size_t)b3 * d.nrb[1] + b2) * d.nrb[0] + b1] >= 0;
+    if (root_leaf && nchild) return fail(AK_EINVAL, "overlapping leaves");
+    if (!root_leaf && nchild != 8) return fail(AK_EINVAL, "leaves do not cover the domain");
+  }
+  if (d.max_level > 0 && (d.ng & 1)) return fail(AK_EUNSUPPORTED, "static refinement needs even ng");
+  // ---- upload tables ----
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::vector<int4> blk(d.nmb);
+  for (int m = 0; m < d.nmb; m++) blk[m] = make_int4(p->level[m], p->lx[3 * m], p->lx[3 * m + 1], p->lx[3 * m + 2]);
+  char* s = (char*)scratch;
+  AK_CUDA(cudaMemsetAsync(s, 0, 256, st), "memset scratch");
+  AK_CUDA(cudaMemcpyAsync(s + sl.blk, blk.data(), sizeof(int4) * d.nmb, cudaMemcpyHostToDevice, st), "upload block table");
+  AK_CUDA(cudaMemcpyAsync(s + sl.leaf0, leaf0.data(), sizeof(int) * n0, cudaMemcpyHostToDevice, st), "upload leaf map 0");
+  AK_CUDA(cudaMemcpyAsync(s + sl.leaf1, leaf1.data(), sizeof(int) * 8 * n0, cudaMemcpyHostToDevice, st), "upload leaf map 1");
+  AK_CUDA(cudaStreamSynchronize(st), "bind sync");
+  d.dtmin_bits = (unsigned long long*)s;
+  d.floor_cnt = (unsigned long long*)(s + 8);
+  d.blk = (const int4*)(s + sl.blk);
+  d.leaf0 = (const int*)(s + sl.leaf0);
+  d.leaf1 = (const int*)(s + sl.leaf1);
+  int dev = 0;
+  AK_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
+  AK_CUDA(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev), "query SM count");
+  p->u[0] = (double*)u_a; p->u[1] = (double*)u_b; p->scratch = scratch; p->stream = st;
+  p->cur = 0; p->ghosts_ok = false; p->bound = true; p->launches = 0;
+  return AK_OK;
+}
+
+extern "C" int ak_pack_set_variant(ak_pack* p, int variant) {
+  if (!p) return fail(AK_EINVAL, "null pack");
+  if (variant != 0 && variant != 1) return fail(AK_EINVAL, "unknown variant");
+  p->variant = variant;
+  return AK_OK;
+}
+
+extern "C" int ak_fill_ghosts(ak_pack* p) {
+  if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  AK_CUDA(ak::launch_fill_ghosts(*p, p->u[p->cur]), "ak_fill_ghosts launch");
+  p->launches += 1;
+  p->ghosts_ok = true;
+  return AK_OK;
+}
+
+extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
+  if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  if (stage != 1 && stage != 2) return fail(AK_EINVAL, "stage must be 1 or 2");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(AK_EINVAL, "dt must be positive and finite");
+  if (stage == 1 && p->cur != 0) return fail(AK_ESTATE, "stage 1 expects U^n in buffer A (call stage 2 first)");
+  if (stage == 2 && p->cur != 1) return fail(AK_ESTATE, "stage 2 expects U^(1) in buffer B (call stage 1 first)");
+  if (!p->ghosts_ok) return fail(AK_ESTATE, "ak_fill_ghosts must precede ak_hydro_stage");
+  // SSPRK(2,2) in two registers (Q1): (g0, g1, beta) = (0,1,1) then (1/2,1/2,1/2)
+  ak::StageCoef sc;
+  const double beta = (stage == 1) ? 1.0 : 0.5;
+  sc.g0 = (stage == 1) ? 0.0 : 0.5;
+  sc.g1 = (stage == 1) ? 1.0 : 0.5;
+  for (int lev = 0; lev < 2; lev++)
+    for (int d = 0; d < 3; d++) {
+      double dx = (p->xmax[d] - p->xmin[d]) / ((double)p->d.nrb[d] * p->d.nx[d] * (double)(1 << lev));
+      sc.c[lev][d] = beta * dt / dx;
+    }
+  AK_CUDA(ak::launch_stage(*p, p->u[p->cur], p->u[0], p->u[1 - p->cur], sc), "ak_hydro_stage launch");
+  p->launches += ak::stage_launches_per_call(*p);
+  p->cur = 1 - p->cur;
+  p->ghosts_ok = false;
+  return AK_OK;
+}
+
+extern "C" int ak_new_dt(ak_pack* p, double cfl, double* dt_out) {
+  if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  if (!dt_out) return fail(AK_EINVAL, "null dt_out");
+  if (!(cfl > 0.0)) return fail(AK_EINVAL, "cfl must be positive");
+  AK_CUDA(ak::launch_new_dt(*p, p->u[p->cur]), "ak_new_dt launch");
+  p->launches += 2;
+  double dtmin = 0.0;
+  AK_CUDA(cudaMemcpyAsync(&dtmin, p->d.dtmin_bits, 8, cudaMemcpyDeviceToHost, p->stream), "ak_new_dt copy");
+  AK_CUDA(cudaStreamSynchronize(p->stream), "ak_new_dt sync");
+  if (!(dtmin > 0.0) || !std::isfinite(dtmin)) return fail(AK_ECUDA, "non-finite time step (state corrupted?)");
+  *dt_out = cfl * dtmin;
+  return AK_OK;
+}
+
+extern "C" int ak_step(ak_pack* p, double cfl, double dt_fixed, double* dt_out) {
+  double dt = dt_fixed;
+  if (!(dt_fixed > 0.0)) { int rc = ak_new_dt(p, cfl, &dt); if (rc) return rc; }
+  for (int stage = 1; stage <= 2; stage++) {
+    int rc = ak_fill_ghosts(p); if (rc) return rc;
+    rc = ak_hydro_stage(p, stage, dt); if (rc) return rc;
+  }
+  if (dt_out) *dt_out = dt;
+  return AK_OK;
+}
+
+extern "C" void* ak_pack_current(const ak_pack* p) { return (p && p->bound) ? (void*)p->u[p->cur] : nullptr; }
+
+extern "C" int ak_pack_upload(ak_pack* p, const void* host_u) {
+  if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  if (!host_u) return fail(AK_EINVAL, "null host buffer");
+  AK_CUDA(cudaMemcpyAsync(p->u[0], host_u, ak_pack_state_bytes(p), cudaMemcpyHostToDevice, p->stream), "ak_pack_upload");
+  p->cur = 0; p->ghosts_ok = false;
+  return AK_OK;
+}
+
+extern "C" int ak_pack_download(ak_pack* p, void* host_u) {
+  if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  if (!host_u) return fail(AK_EINVAL, "null host buffer");
+  AK_CUDA(cudaMemcpyAsync(host_u, p->u[p->cur], ak_pack_state_bytes(p), cudaMemcpyDeviceToHost, p->stream), "ak_pack_download");
+  AK_CUDA(cudaStreamSynchronize(p->stream), "ak_pack_download sync");
+  return AK_OK;
+}
+
+extern "C" long long ak_pack_floor_count(ak_pack* p) {
+  if (!p || !p->bound) { fail(AK_ESTATE, "pack not bound"); return -1; }
+  unsigned long long n = 0;
+  if (cudaMemcpyAsync(&n, p->d.floor_cnt, 8, cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
+      cudaStreamSynchronize(p->stream) != cudaSuccess) { fail(AK_ECUDA, "ak_pack_floor_count copy failed"); return -1; }
+  return (long long)n;
+}
+
+extern "C" long long ak_pack_launch_count(const ak_pack* p) { return p ? p->launches : -1; }
+
+extern "C" int ak_pack_destroy(ak_pack* p) { delete p; return AK_OK; }

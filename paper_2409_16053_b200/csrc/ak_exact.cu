@@ -1,0 +1,178 @@
+// ak_exact.cu -- kernels whose results must match the oracle BIT-EXACTLY: ghost fill (same-level
+// copy, restriction, prolongation) and the CFL reduction (Eq.(3)).
+// Compiled with -fmad=false and IEEE division / sqrt, so every expression rounds once per
+// operation in the order written.
+#define AK_EXACT_MATH 1
+#include "ak_pack.h"
+#include "ak_physics.cuh"
+
+namespace ak {
+
+__device__ __forceinline__ int nglob(const PackDev& P, int lev, int d) { return (P.nrb[d] * P.nx[d]) << lev; }
+
+__device__ __forceinline__ int find_leaf(const PackDev& P, int lev, int b1, int b2, int b3) {
+  if (lev == 0) return P.leaf0[(b3 * P.nrb[1] + b2) * P.nrb[0] + b1];
+  if (P.max_level < 1) return -1;
+  return P.leaf1[(b3 * (2 * P.nrb[1]) + b2) * (2 * P.nrb[0]) + b1];
+}
+
+// address of variable 0 of the active cell with level-`lev` global index G (wrapped) in leaf m
+__device__ __forceinline__ long long leaf_cell(const PackDev& P, int m, int4 b, int G1, int G2, int G3) {
+  int i = G1 - b.y * P.nx[0] + P.ng, j = G2 - b.z * P.nx[1] + P.ng, k = G3 - b.w * P.nx[2] + P.ng;
+  return (long long)m * 5 * P.ncell + ((long long)k * P.nt[1] + j) * P.nt[0] + i;
+}
+
+// G3: conservative restriction of the 8 level-(lev+1) cells under level-`lev` cell G (fixed order).
+// Returns false if no finer leaf covers the cell.
+__device__ bool restrict5(const PackDev& P, const double* __restrict__ U, int lev, int G1, int G2, int G3, double out[5]) {
+  // the 8 children live in one fine block because nx_d is even
+  int F1 = 2 * G1, F2 = 2 * G2, F3 = 2 * G3;
+  int m = find_leaf(P, lev + 1, F1 / P.nx[0], F2 / P.nx[1], F3 / P.nx[2]);
+  if (m < 0) return false;
+  long long a = leaf_cell(P, m, P.blk[m], F1, F2, F3);
+  const long long sj = P.nt[0], sk = (long long)P.nt[0] * P.nt[1];
+  for (int n = 0; n < 5; n++) {
+    const double* q = U + a + n * P.ncell;
+    double f000 = q[0], f100 = q[1], f010 = q[sj], f110 = q[sj + 1];
+    double f001 = q[sk], f101 = q[sk + 1], f011 = q[sk + sj], f111 = q[sk + sj + 1];
+    out[n] = 0.125 * (((f000 + f100) + (f010 + f110)) + ((f001 + f101) + (f011 + f111)));
+  }
+  return true;
+}
+
+__device__ __forceinline__ int wrap1(int g, int n) { return g < 0 ? g + n : (g >= n ? g - n : g); }
+
+// virtual level-`lev` field C(.) of G4: leaf value where a level-`lev` leaf covers G, else restriction
+__device__ bool coarse5(const PackDev& P, const double* __restrict__ U, int lev, int G1, int G2, int G3, double out[5]) {
+  G1 = wrap1(G1, nglob(P, lev, 0)); G2 = wrap1(G2, nglob(P, lev, 1)); G3 = wrap1(G3, nglob(P, lev, 2));
+  int m = find_leaf(P, lev, G1 / P.nx[0], G2 / P.nx[1], G3 / P.nx[2]);
+  if (m >= 0) {
+    long long a = leaf_cell(P, m, P.blk[m], G1, G2, G3);
+    for (int n = 0; n < 5; n++) out[n] = U[a + n * P.ncell];
+    return true;
+  }
+  return restrict5(P, U, lev, G1, G2, G3, out);
+}
+
+__device__ __forceinline__ double minmod(double a, double b) {
+  if (a * b <= 0.0) return 0.0;
+  double m = fmin(fabs(a), fabs(b));
+  return a > 0.0 ? m : -m;
+}
+
+// One thread per ghost cell (all 5 variables).  The ghost shell of a block is enumerated as
+// k-slabs, then j-slabs, then i-slabs so that consecutive threads touch consecutive i.
+__global__ void __launch_bounds__(256) fill_ghosts_kernel(PackDev P, double* __restrict__ U, int nghost) {
+  const int m = blockIdx.y;
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= nghost) return;
+  const int ng = P.ng, n1 = P.nt[0], n2 = P.nt[1];
+  const int A = 2 * ng * n2 * n1, B = P.nx[2] * 2 * ng * n1;
+  int i, j, k;
+  if (g < A) {
+    int kk = g / (n2 * n1), r = g - kk * (n2 * n1);
+    k = kk < ng ? kk : kk + P.nx[2];
+    j = r / n1; i = r - j * n1;
+  } else if (g < A + B) {
+    g -= A;
+    int kk = g / (2 * ng * n1), r = g - kk * (2 * ng * n1);
+    k = ng + kk;
+    int jj = r / n1; i = r - jj * n1;
+    j = jj < ng ? jj : jj + P.nx[1];
+  } else {
+    g -= A + B;
+    int kk = g / (P.nx[1] * 2 * ng), r = g - kk * (P.nx[1] * 2 * ng);
+    k = ng + kk;
+    int jj = r / (2 * ng), ii = r - jj * (2 * ng);
+    j = ng + jj;
+    i = ii < ng ? ii : ii + P.nx[0];
+  }
+  const int4 b = P.blk[m];
+  const int lev = b.x;
+  // G1: which leaf covers the periodic image of this ghost cell?
+  const int G1 = wrap1(b.y * P.nx[0] + i - ng, nglob(P, lev, 0));
+  const int G2 = wrap1(b.z * P.nx[1] + j - ng, nglob(P, lev, 1));
+  const int G3 = wrap1(b.w * P.nx[2] + k - ng, nglob(P, lev, 2));
+  double val[5];
+  const int src = find_leaf(P, lev, G1 / P.nx[0], G2 / P.nx[1], G3 / P.nx[2]);
+  if (src >= 0) {                                           // G2: same level, copy
+    long long a = leaf_cell(P, src, P.blk[src], G1, G2, G3);
+    for (int n = 0; n < 5; n++) val[n] = U[a + n * P.ncell];
+  } else if (lev == 0) {                                    // G3: finer neighbour
+    restrict5(P, U, 0, G1, G2, G3, val);
+  } else {                                                  // G4: coarser neighbour
+    const int C1 = G1 >> 1, C2 = G2 >> 1, C3 = G3 >> 1;
+    const double s1 = (double)(2 * (G1 & 1) - 1), s2 = (double)(2 * (G2 & 1) - 1), s3 = (double)(2 * (G3 & 1) - 1);
+    double c0[5], cm[5], cp[5], g1[5], g2[5], g3[5];
+    coarse5(P, U, lev - 1, C1, C2, C3, c0);
+    coarse5(P, U, lev - 1, C1 - 1, C2, C3, cm); coarse5(P, U, lev - 1, C1 + 1, C2, C3, cp);
+    for (int n = 0; n < 5; n++) g1[n] = 0.25 * minmod(c0[n] - cm[n], cp[n] - c0[n]);
+    coarse5(P, U, lev - 1, C1, C2 - 1, C3, cm); coarse5(P, U, lev - 1, C1, C2 + 1, C3, cp);
+    for (int n = 0; n < 5; n++) g2[n] = 0.25 * minmod(c0[n] - cm[n], cp[n] - c0[n]);
+    coarse5(P, U, lev - 1, C1, C2, C3 - 1, cm); coarse5(P, U, lev - 1, C1, C2, C3 + 1, cp);
+    for (int n = 0; n < 5; n++) g3[n] = 0.25 * minmod(c0[n] - cm[n], cp[n] - c0[n]);
+    for (int n = 0; n < 5; n++) val[n] = ((c0[n] + s1 * g1[n]) + s2 * g2[n]) + s3 * g3[n];
+  }
+  const long long o = (long long)m * 5 * P.ncell + ((long long)k * n2 + j) * n1 + i;
+  for (int n = 0; n < 5; n++) U[o + n * P.ncell] = val[n];
+}
+
+cudaError_t launch_fill_ghosts(const ak_pack& p, double* U) {
+  const PackDev& P = p.d;
+  long long nghost = P.ncell - (long long)P.nx[0] * P.nx[1] * P.nx[2];
+  dim3 grid((unsigned)((nghost + 255) / 256), (unsigned)P.nmb);
+  fill_ghosts_kernel<<<grid, 256, 0, p.stream>>>(P, U, (int)nghost);
+  return cudaGetLastError();
+}
+
+// ---- S0: CFL time step ---------------------------------------------------------------------------
+// Every candidate dx_d/(|v_d|+c_s) is positive, so its IEEE bit pattern orders like an unsigned
+// integer and the global min is one atomicMin per CTA after a shuffle + shared-memory reduction.
+__global__ void dt_init_kernel(PackDev P) { *P.dtmin_bits = 0x7FF0000000000000ull; }
+
+__global__ void __launch_bounds__(256) new_dt_kernel(PackDev P, const double* __restrict__ U, long long nrows) {
+  const double ug_floor = P_FLOOR / (P.gamma - 1.0);
+  double best = __longlong_as_double(0x7FF0000000000000ll);
+  // one warp per row of nx1 active cells; rows enumerated over (m, k, j)
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+  for (long long row = (long long)blockIdx.x * wpb + wib; row < nrows; row += (long long)gridDim.x * wpb) {
+    long long r = row;
+    int j = (int)(r % P.nx[1]); r /= P.nx[1];
+    int k = (int)(r % P.nx[2]); r /= P.nx[2];
+    int m = (int)r;
+    const int lev = P.blk[m].x;
+    const double sc = lev ? 0.5 : 1.0;
+    const double dx1 = sc * P.dx0[0], dx2 = sc * P.dx0[1], dx3 = sc * P.dx0[2];
+    const double* q = U + (long long)m * 5 * P.ncell + ((long long)(k + P.ng) * P.nt[1] + (j + P.ng)) * P.nt[0] + P.ng;
+    for (int i = lane; i < P.nx[0]; i += 32) {
+      double u[5], w[5];
+      for (int n = 0; n < 5; n++) u[n] = q[i + n * P.ncell];
+      c2p(u, w, ug_floor);
+      double pr = (P.gamma - 1.0) * w[4];
+      double cs = sqrt(P.gamma * pr / w[0]);
+      best = fmin(best, dx1 / (fabs(w[1]) + cs));
+      best = fmin(best, dx2 / (fabs(w[2]) + cs));
+      best = fmin(best, dx3 / (fabs(w[3]) + cs));
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
+  __shared__ double sm[8];
+  if (lane == 0) sm[wib] = best;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < wpb; w++) best = fmin(best, sm[w]);
+    atomicMin(P.dtmin_bits, (unsigned long long)__double_as_longlong(best));
+  }
+}
+
+cudaError_t launch_new_dt(const ak_pack& p, const double* U) {
+  const PackDev& P = p.d;
+  dt_init_kernel<<<1, 1, 0, p.stream>>>(P);
+  long long nrows = (long long)P.nmb * P.nx[1] * P.nx[2];
+  long long want = (nrows + 7) / 8;
+  int grid = (int)(want < (long long)p.sm_count * 8 ? want : (long long)p.sm_count * 8);
+  new_dt_kernel<<<grid, 256, 0, p.stream>>>(P, U, nrows);
+  return cudaGetLastError();
+}
+
+}  // namespace ak

@@ -1,0 +1,61 @@
+// ak_pack.h -- host descriptor and the plain-data view of a pack that kernels receive by value.
+// Internal to the library (the public boundary is include/ak.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <string>
+#include <vector>
+
+namespace ak {
+
+struct GasConst;
+
+// Device-side view: everything a kernel needs to address U[m][n][k][j][i] and to find the
+// leaf that covers a position (block tree of P:59 flattened into dense per-level maps).
+struct PackDev {
+  int nmb;
+  int nx[3];        // active cells per block
+  int ng;
+  int nt[3];        // nx + 2 ng
+  int nrb[3];       // root blocks per direction
+  int max_level;    // 0 or 1
+  long long ncell;  // nt0*nt1*nt2, stride between variables
+  const int4* blk;  // (level, lx1, lx2, lx3) per block
+  const int* leaf0; // [nrb3][nrb2][nrb1]       -> block index or -1
+  const int* leaf1; // [2nrb3][2nrb2][2nrb1]    -> block index or -1
+  double dx0[3];    // level-0 cell size; level 1 is exactly half
+  double gamma;
+  unsigned long long* dtmin_bits;   // scratch cell: min candidate dt as ordered bits
+  unsigned long long* floor_cnt;    // scratch cell: floor activations
+};
+
+struct StageCoef {
+  double g0, g1;            // weights of U_in and U0
+  double c[2][3];           // beta*dt/dx_d for level 0 and 1
+};
+
+}  // namespace ak
+
+struct ak_pack {
+  ak::PackDev d{};
+  int recon = 0, rsolver = 0;
+  double xmin[3]{}, xmax[3]{};
+  bool mesh_set = false, bound = false, ghosts_ok = false;
+  std::vector<int> level, lx;     // lx[3m+d]
+  std::vector<char> blk_set;
+  double* u[2] = {nullptr, nullptr};
+  void* scratch = nullptr;
+  cudaStream_t stream = nullptr;
+  int cur = 0;
+  int variant = 0;
+  long long launches = 0;
+  int sm_count = 148;
+};
+
+namespace ak {
+// launchers implemented in the .cu translation units; return cudaGetLastError()
+cudaError_t launch_fill_ghosts(const ak_pack& p, double* U);
+cudaError_t launch_new_dt(const ak_pack& p, const double* U);       // leaves the min in dtmin_bits
+cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, double* Uout,
+                         const StageCoef& sc);
+int stage_launches_per_call(const ak_pack& p);
+}  // namespace ak

@@ -1,0 +1,16 @@
+// ak_stage.cu -- ak_hydro_stage kernels: fused c2p + reconstruction + HLLC in x1/x2/x3 +
+// flux divergence + RK2 weighted update.  FMA contraction is allowed here (parity is to 1e-12, not
+// bit-exact).
+#include "ak_pack.h"
+#include "ak_physics.cuh"
+#include "ak_stage_simple.cuh"
+
+namespace ak {
+
+cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, double* Uout, const StageCoef& sc) {
+  return launch_stage_simple(p, Uin, U0, Uout, sc);
+}
+
+int stage_launches_per_call(const ak_pack&) { return 1; }
+
+}  // namespace ak

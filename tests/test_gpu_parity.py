@@ -1,0 +1,244 @@
+"""GPU parity tests proper (-m gpu): the CUDA path, called through the C-ABI binding, against the
+oracle on the same seeded inputs.  Tolerances are BASELINE.json's: Q14 metric <= 1e-12 after one
+stage, <= 1e-9 after the config's steps, conserved totals within 1e-12, ghost fill bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2409_16053_b200 import inputs as I
+from tests import parity as P
+
+pytestmark = pytest.mark.gpu
+
+TOL_STAGE, TOL_RUN, TOL_TOTALS = 1e-12, 1e-9, 1e-12
+
+
+@pytest.fixture(scope="module")
+def ak():
+    from paper_2409_16053_b200 import ak as _ak
+    _ak.lib()
+    assert torch.cuda.is_available()
+    return _ak
+
+
+def run_lockstep(orc, ak, w, nsteps, variant=0, check_ghosts=True):
+    """Oracle computes dt; both sides take it.  Returns per-step Q14 and the two final states."""
+    U0 = w.state()
+    po, pg = P.make_pair(orc, ak, w, U0, variant)
+    a = P.active(w.mesh)
+    errs = []
+    for step in range(nsteps):
+        dt = po.new_dt(w.cfl)
+        dt_g = pg.new_dt(w.cfl)
+        assert abs(dt_g - dt) <= 4 * np.spacing(dt), (step, dt, dt_g)
+        for stage in (1, 2):
+            po.fill_ghosts()
+            pg.fill_ghosts()
+            if check_ghosts and step == 0:
+                # ghosts of identical active data must be bit-identical; after the first stage the active
+                # data differ by rounding, so compare the oracle's fill of the GPU's active cells instead
+                ug = P.gpu_state(pg)
+                chk = orc.OrcPack(w.mesh, w.gamma, w.recon, threads=P.NTHREADS)
+                chk.load(ug)
+                chk.fill_ghosts()
+                assert np.array_equal(chk.current(), ug), f"ghost fill differs at step {step} stage {stage}"
+                chk.close()
+            po.hydro_stage(stage, dt)
+            pg.hydro_stage(stage, dt)
+            if step == 0:
+                e = P.q14(P.gpu_state(pg)[a], po.current()[a], w.gamma)
+                assert e <= TOL_STAGE * stage, f"stage {stage}: Q14 = {e:.3e}"
+        errs.append(P.q14(P.gpu_state(pg)[a], po.current()[a], w.gamma))
+    assert po.floor_count() == 0 and pg.floor_count() == 0
+    return errs, po, pg, U0
+
+
+def check_totals(w, U0, po, pg):
+    t0 = P.totals(w.mesh, U0.numpy())
+    tg = P.totals(w.mesh, P.gpu_state(pg))
+    to = P.totals(w.mesh, po.current())
+    norm = P.momentum_norm(w.mesh, U0.numpy(), w.gamma)
+    scale = np.array([t0[0], norm, norm, norm, t0[4]])
+    assert (np.abs(tg - to) / scale).max() <= TOL_TOTALS
+    return np.abs(tg - t0) / scale
+
+
+# ------------------------------------------------------------------------------- config 0 --------
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config0_sound_wave_every_cell(orc, ak, variant):
+    w = I.config0()
+    errs, po, pg, U0 = run_lockstep(orc, ak, w, w.nsteps, variant)
+    assert max(errs) <= TOL_RUN, errs
+    po.fill_ghosts()
+    pg.fill_ghosts()
+    full = (slice(None),) * 5
+    assert P.q14(P.gpu_state(pg)[full], po.current()[full], w.gamma) <= TOL_RUN      # every cell, ghosts included
+    drift = check_totals(w, U0, po, pg)
+    assert drift.max() <= 1e-13
+
+
+def test_config0_literal_reading_constant_pressure(orc, ak):
+    w = I.config0(literal=True)
+    errs, *_ = run_lockstep(orc, ak, w, 3)
+    assert max(errs) <= TOL_RUN
+
+
+# ------------------------------------------------------------------------------- config 1 --------
+def test_config1_random_modes_20_steps(orc, ak):
+    w = I.config1()
+    errs, po, pg, U0 = run_lockstep(orc, ak, w, w.nsteps)
+    assert max(errs) <= TOL_RUN, errs
+    drift = check_totals(w, U0, po, pg)
+    assert drift.max() <= 1e-12           # periodic single-level mesh: conservation to round-off
+
+
+def test_config1_free_running_dt(orc, ak):
+    w = I.config1(nrb=2)                  # 8 x 32^3
+    U0 = w.state()
+    po, pg = P.make_pair(orc, ak, w, U0)
+    for _ in range(10):
+        po.step(w.cfl)
+        pg.step(w.cfl)
+    a = P.active(w.mesh)
+    assert P.q14(P.gpu_state(pg)[a], po.current()[a], w.gamma) <= TOL_RUN
+
+
+# ------------------------------------------------------------------------------- config 2 --------
+def test_config2_sedov_32cubed_blocks(orc, ak):
+    w = I.config2(nx=32, n=128)           # 64 x 32^3 crop of the 256^3 mesh, same dx-independent recipe
+    errs, po, pg, U0 = run_lockstep(orc, ak, w, w.nsteps)
+    assert max(errs) <= TOL_RUN, errs
+    check_totals(w, U0, po, pg)
+
+
+def test_config2_block_size_sweep_is_decomposition_invariant_on_gpu(ak):
+    """Same 64^3 Sedov field cut into 16^3 / 32^3 / 64^3 blocks: active cells agree to rounding on the GPU
+    (bit-identical in the oracle; the GPU's tile edges may contract FMAs differently)."""
+    res = []
+    for nx in (16, 32, 64):
+        w = I.config2(nx=nx, n=64)
+        w.prim_fn = I.sedov_prim(r0=0.2)
+        pg = ak.Pack(w.mesh, w.gamma, w.recon)
+        pg.load(w.state())
+        for _ in range(5):
+            pg.step(w.cfl)
+        U = P.gpu_state(pg)
+        ng = w.mesh.ng
+        glob = np.zeros((5, 64, 64, 64))
+        for m, (_, l1, l2, l3) in enumerate(w.mesh.blocks):
+            glob[:, l3 * nx:(l3 + 1) * nx, l2 * nx:(l2 + 1) * nx, l1 * nx:(l1 + 1) * nx] = U[m][:, ng:-ng, ng:-ng, ng:-ng]
+        res.append(glob)
+    for r in res[1:]:
+        assert P.q14(r[None], res[0][None], I.GAMMA) <= 1e-13
+
+
+# ------------------------------------------------------------------------------- config 3 --------
+def test_config3_ppm_reduced_size(orc, ak):
+    w = I.config3(nrb=2, nx=32)           # 8 x 32^3, PPM4, ng=3, Mach-1 modes + double shear layer
+    errs, po, pg, U0 = run_lockstep(orc, ak, w, w.nsteps)
+    assert max(errs) <= TOL_RUN, errs
+    check_totals(w, U0, po, pg)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config3_ppm_noncubic_blocks(orc, ak, variant):
+    w = I.config3(nrb=2, nx=32)
+    w.mesh = I.uniform_mesh((2, 1, 3), (24, 40, 6), 3)
+    errs, *_ = run_lockstep(orc, ak, w, 3, variant)
+    assert max(errs) <= TOL_RUN, errs
+
+
+# ------------------------------------------------------------------------------- config 4 --------
+def test_config4_smr_sedov_20_steps(orc, ak):
+    w = I.config4()
+    errs, po, pg, U0 = run_lockstep(orc, ak, w, w.nsteps)
+    assert max(errs) <= TOL_RUN, errs
+    check_totals(w, U0, po, pg)
+
+
+def test_smr_with_structure_on_level_boundaries(orc, ak):
+    """SURVEY finding 3: config 4 never puts non-uniform data on a level boundary; this input does."""
+    w = I.smr_parity()
+    U0 = w.state()
+    po, pg = P.make_pair(orc, ak, w, U0)
+    a = P.active(w.mesh)
+    for step in range(w.nsteps):
+        dt = po.new_dt(w.cfl)
+        for stage in (1, 2):
+            po.fill_ghosts()
+            pg.fill_ghosts()
+            ug = P.gpu_state(pg)
+            chk = orc.OrcPack(w.mesh, w.gamma, w.recon, threads=P.NTHREADS)
+            chk.load(ug)
+            chk.fill_ghosts()
+            assert np.array_equal(chk.current(), ug)          # restriction + prolongation bit-exact
+            chk.close()
+            po.hydro_stage(stage, dt)
+            pg.hydro_stage(stage, dt)
+        assert P.q14(P.gpu_state(pg)[a], po.current()[a], w.gamma) <= TOL_RUN
+
+
+# ------------------------------------------------------------------------------- edge cases ------
+@pytest.mark.parametrize("nrb,nx,ng,recon", [
+    ((1, 1, 1), (2, 2, 2), 2, I.RECON_PLM),        # smallest legal block, self-periodic
+    ((1, 1, 1), (4, 4, 4), 3, I.RECON_PPM4),
+    ((1, 2, 1), (6, 2, 4), 2, I.RECON_PLM),
+    ((3, 1, 2), (34, 10, 6), 2, I.RECON_PLM),      # ragged: not a multiple of any tile size
+    ((1, 1, 1), (130, 18, 10), 3, I.RECON_PPM4),   # longer than one 128-wide tile row
+    ((1, 1, 1), (16, 16, 16), 4, I.RECON_PPM4),    # more ghosts than the stencil needs
+])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_ragged_and_degenerate_blocks(orc, ak, nrb, nx, ng, recon, variant):
+    mesh = I.uniform_mesh(nrb, nx, ng)
+    w = I.Workload("edge", mesh, recon, 2, I.modes_prim(0.5, shear=False, rho_pert=True))
+    errs, *_ = run_lockstep(orc, ak, w, 2, variant)
+    assert max(errs) <= TOL_RUN, errs
+
+
+def test_uniform_state_preserved_bit_exactly_on_gpu(ak):
+    mesh = I.uniform_mesh((2, 2, 1), (16, 8, 8), 2)
+    prim = lambda X1, X2, X3: (1.3 + 0 * X1, 0.4 + 0 * X1, -0.7 + 0 * X1, 0.2 + 0 * X1, 0.9 + 0 * X1)
+    for recon, mesh_ in ((I.RECON_PLM, mesh), (I.RECON_PPM4, I.uniform_mesh((2, 2, 1), (16, 8, 8), 3))):
+        U0 = I.make_state(mesh_, prim)
+        pg = ak.Pack(mesh_, I.GAMMA, recon)
+        pg.load(U0)
+        pg.step(0.3)
+        a = P.active(mesh_)
+        assert np.array_equal(P.gpu_state(pg)[a], U0.numpy()[a])
+
+
+def test_dt_reduction_bit_exact(orc, ak):
+    for w in (I.config1(nrb=2), I.smr_parity(nx=8), I.config3(nrb=1, nx=32)):
+        U0 = w.state()
+        po, pg = P.make_pair(orc, ak, w, U0)
+        assert pg.new_dt(w.cfl) == po.new_dt(w.cfl)
+
+
+def test_call_order_and_argument_errors(ak):
+    w = I.config0()
+    pg = ak.Pack(w.mesh, w.gamma, w.recon)
+    pg.load(w.state())
+    with pytest.raises(ak.AkError):
+        pg.hydro_stage(1, 1e-3)                      # ghosts not filled
+    pg.fill_ghosts()
+    with pytest.raises(ak.AkError):
+        pg.hydro_stage(2, 1e-3)                      # stage 2 before stage 1
+    with pytest.raises(ak.AkError):
+        pg.hydro_stage(1, -1.0)
+    pg.hydro_stage(1, 1e-3)
+    with pytest.raises(ak.AkError):
+        pg.hydro_stage(2, 1e-3)                      # ghosts stale again
+    pg.fill_ghosts()
+    pg.hydro_stage(2, 1e-3)
+    assert pg.launch_count() >= 4
+
+
+def test_upload_download_round_trip_through_c_abi(ak):
+    w = I.config1(nrb=1)
+    U0 = w.state()
+    pg = ak.Pack(w.mesh, w.gamma, w.recon)
+    host = U0.clone().pin_memory()
+    pg.upload(host)
+    out = torch.empty_like(host).pin_memory()
+    pg.download(out)
+    assert torch.equal(out, U0)
