@@ -4,11 +4,13 @@
 #include "ak_pack.h"
 #include "ak_physics.cuh"
 #include "ak_stage_simple.cuh"
+#include "ak_stage_tiled.cuh"
 
 namespace ak {
 
 cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, double* Uout, const StageCoef& sc) {
-  return launch_stage_simple(p, Uin, U0, Uout, sc);
+  if (p.variant == 1) return launch_stage_simple(p, Uin, U0, Uout, sc);
+  return launch_stage_tiled(p, Uin, U0, Uout, sc);
 }
 
 int stage_launches_per_call(const ak_pack&) { return 1; }
