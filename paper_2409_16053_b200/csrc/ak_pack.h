@@ -1,6 +1,7 @@
 // ak_pack.h -- host descriptor and the plain-data view of a pack that kernels receive by value.
 // Internal to the library (the public boundary is include/ak.h).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <string>
 #include <vector>
@@ -49,6 +50,9 @@ struct ak_pack {
   int variant = 0;
   long long launches = 0;
   int sm_count = 148;
+  // tensor maps over u[0], u[1] for the TMA stage kernel, rebuilt when the staging box changes
+  mutable CUtensorMap tmap[2];
+  mutable int tmap_box[2] = {0, 0};
 };
 
 namespace ak {
