@@ -20,7 +20,7 @@ COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INCLUDE
 UNITS = {                      # translation unit -> extra flags
     "ak_api.cu": [],
     "ak_exact.cu": ["-fmad=false"],
-    "ak_stage.cu": ["-Xptxas", "-v"],
+    "ak_stage.cu": ["-fmad=false", "-Xptxas", "-v"],
 }
 
 

@@ -1,0 +1,149 @@
+// ak_lean.cuh -- branch-free, instruction-lean forms of the per-cell / per-face arithmetic for the
+// production stage kernel (ak_stage_v2.cuh).  Same formulas as ak_physics.cuh (DESIGN.md section 2
+// readings Q1-Q7; paper P:101 reconstruction on primitives, P:103 HLLC, P:122-126 gamma-law gas); they
+// differ from it by rounding only (a few ulp) and are written against what profiles/r01_v1_stage_cfg3.md
+// showed to be expensive on sm_100a:
+//   * fmin/fmax on doubles lower to DSETP + SEL/FSEL + several moves (NaN handling): replaced by one
+//     compare + select, or by a sign test of the high word on the integer pipe where the other operand is 0;
+//   * data-dependent branches (shock branch of the wave speeds, CW84 limiter cases) diverge inside a warp
+//     on turbulent data and cost BSSY/BSYNC: everything here is straight-line code with selects;
+//   * IEEE division / sqrt: MUFU.RCP64H / RSQ64H seed + Newton, as in ak_physics.cuh.
+#pragma once
+#include "ak_physics.cuh"
+
+namespace ak {
+
+// sign tests on the integer pipe.  neg(): true for x < 0 and -0.  pos(): true for x > 0 except positive
+// denormals below 2^-1042 (treated as zero; they only ever gate a slope of that size).
+__device__ __forceinline__ bool neg(double x) { return __double2hiint(x) < 0; }
+__device__ __forceinline__ bool pos(double x) { return __double2hiint(x) > 0; }
+__device__ __forceinline__ double max0(double x) { return neg(x) ? 0.0 : x; }
+__device__ __forceinline__ double min0(double x) { return neg(x) ? x : 0.0; }
+
+// 1/x to <= 1 ulp: MUFU seed (~20 bits) + two Newton steps                       4 FP64 + 1 MUFU
+__device__ __forceinline__ double rcp2(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
+}
+
+// ---- S1  conserved -> primitive ------------------------------------------------------------------
+__device__ __forceinline__ int c2p_lean(const double U[5], double W[5], double ug_floor) {
+  int nfl = 0;
+  double rho = U[0];
+  if (!(rho >= RHO_FLOOR)) { rho = RHO_FLOOR; nfl++; }
+  const double rinv = rcp2(rho);
+  const double ke2 = fma(U[1], U[1], fma(U[2], U[2], U[3] * U[3]));
+  double ug = fma(-0.5 * rinv, ke2, U[4]);
+  if (!(ug >= ug_floor)) { ug = ug_floor; nfl++; }
+  W[0] = rho; W[1] = U[1] * rinv; W[2] = U[2] * rinv; W[3] = U[3] * rinv; W[4] = ug;
+  return nfl;
+}
+
+// ---- S2  reconstruction --------------------------------------------------------------------------
+// PLM, van Leer: q-/q+ of the cell with neighbours (m1, c, p1)
+__device__ __forceinline__ void plm_lean(double m1, double c, double p1, double& qm, double& qp) {
+  const double dL = c - m1, dR = p1 - c, prod = dL * dR;
+  const double q = div_lean(prod, dL + dR);          // discarded by the select where prod <= 0 (may be NaN)
+  const double h = pos(prod) ? q : 0.0;
+  qm = c - h; qp = c + h;
+}
+
+// PPM4 (i)+(ii): 4th-order interface value between q0 and q1 clamped into [min,max](q0,q1)   7 FP64
+__device__ __forceinline__ double iface_lean(double qm1, double q0, double q1, double q2) {
+  double v = fma(7.0, q0 + q1, -(qm1 + q2)) * (1.0 / 12.0);
+  const bool up = q0 < q1;
+  const double lo = up ? q0 : q1, hi = up ? q1 : q0;
+  v = (v < lo) ? lo : v;
+  v = (v > hi) ? hi : v;
+  return v;
+}
+// PPM4 (iii): CW84 Eq.(1.10), straight-line                                                  ~15 FP64
+__device__ __forceinline__ void limit_lean(double a, double& aL, double& aR) {
+  const bool flat = !pos((aR - a) * (a - aL));
+  const double d = aR - aL;
+  const double mu = fma(-0.5, aL + aR, a);
+  const double dmu = d * mu, d26 = (d * d) * (1.0 / 6.0);
+  const double a3 = 3.0 * a;
+  const double nL = fma(-2.0, aR, a3), nR = fma(-2.0, aL, a3);
+  const bool cL = dmu > d26, cR = (-d26 > dmu);
+  aL = flat ? a : (cL ? nL : aL);
+  aR = flat ? a : (cR ? nR : aR);
+}
+
+// sqrt(a / b) for a, b > 0 without a division: r ~ (a b)^(-1/2), s = a r, one residual step on s^2 b = a
+__device__ __forceinline__ double sqrt_ratio(double a, double b) {                // 10 FP64 + 1 MUFU
+  const double t = a * b;
+  double r;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(t));
+  const double e = fma(-(0.5 * t) * r, r, 0.5);
+  r = fma(r, e, r);
+  const double s = a * r;
+  const double res = fma(-(s * b), s, a);
+  return fma(res, 0.5 * r, s);
+}
+
+// ---- S3  HLLC, rotated states (rho, u_normal, v, w, u_g) -------------------------------------------
+// Straight-line: the shock branch of the pressure-based wave speeds is folded into
+//   c_K q_K = sqrt(gamma (p_K + gq max(p_pvrs - p_K, 0)) / rho_K)
+// (equal to c_K where p_pvrs <= p_K), u_K - S_K is taken as c_K q_K, and the upwind side is chosen by the
+// sign of S*.  ~100 FP64-pipe instructions + 6 MUFU.
+__device__ __forceinline__ void hllc2(const GasConst& g, const double WL[5], const double WR[5], double F[5]) {
+  const double rL = WL[0], uL = WL[1], eL = WL[4];
+  const double rR = WR[0], uR = WR[1], eR = WR[4];
+  const double pL = g.gm1 * eL, pR = g.gm1 * eR;
+  const double gpL = g.gamma * pL, gpR = g.gamma * pR;
+  const double cL = sqrt_ratio(gpL, rL), cR = sqrt_ratio(gpR, rR);
+  const double ppv = fma(0.125, ((uL - uR) * (rL + rR)) * (cL + cR), 0.5 * (pL + pR));
+  const double ggq = g.gamma * g.gq;
+  const double cqL = sqrt_ratio(fma(ggq, max0(ppv - pL), gpL), rL);
+  const double cqR = sqrt_ratio(fma(ggq, max0(ppv - pR), gpR), rR);
+  const double SL = uL - cqL, SR = uR + cqR;
+  const double mL = rL * cqL, mR = rR * cqR;
+  const double Ss = div_lean((pL - pR) + fma(mL, uL, mR * uR), mL + mR);
+  const double psL = fma(-mL, Ss - uL, pL);
+  const double psR = fma(mR, Ss - uR, pR);
+  const double ps = max0(0.5 * (psL + psR));
+  const bool left = !neg(Ss);
+  const double rK = left ? rL : rR, uK = left ? uL : uR, vK = left ? WL[2] : WR[2], wK = left ? WL[3] : WR[3];
+  const double eK = left ? eL : eR, pK = left ? pL : pR, b = left ? min0(SL) : max0(SR);
+  const double EK = fma(0.5 * rK, fma(uK, uK, fma(vK, vK, wK * wK)), eK);
+  const double mom = rK * uK;
+  const double inv = rcp2(Ss - b);
+  const double w = Ss * inv;                       // S*/(S* - b)
+  const double bps = b * ps;
+  const double f0 = fma(-b, rK, mom) * w;
+  F[0] = f0;
+  F[1] = fma(Ss, fma(-b, mom, fma(mom, uK, pK)), -bps) * inv;
+  F[2] = f0 * vK;
+  F[3] = f0 * wK;
+  F[4] = (fma(-b, EK, (EK + pK) * uK) - bps) * w;
+}
+
+// direction D known at compile time: pick the normal / cyclic transverse components, un-rotate the flux
+template <int D>
+__device__ __forceinline__ void flux2(const GasConst& g, const double L[5], const double Rr[5], double F[5]) {
+  const double l[5] = {L[0], L[1 + D], L[1 + (D + 1) % 3], L[1 + (D + 2) % 3], L[4]};
+  const double r[5] = {Rr[0], Rr[1 + D], Rr[1 + (D + 1) % 3], Rr[1 + (D + 2) % 3], Rr[4]};
+  double f[5];
+  hllc2(g, l, r, f);
+  F[0] = f[0]; F[1 + D] = f[1]; F[1 + (D + 1) % 3] = f[2]; F[1 + (D + 2) % 3] = f[3]; F[4] = f[4];
+}
+// direction x1 (d2 = false) or x2 (d2 = true) chosen at run time: used by the tile-edge threads so that the
+// x1-edge and x2-edge faces of a tile run through ONE instruction stream instead of two divergent ones
+__device__ __forceinline__ void flux2_12(const GasConst& g, bool d2, const double L[5], const double Rr[5], double F[5]) {
+  const double l[5] = {L[0], d2 ? L[2] : L[1], d2 ? L[3] : L[2], d2 ? L[1] : L[3], L[4]};
+  const double r[5] = {Rr[0], d2 ? Rr[2] : Rr[1], d2 ? Rr[3] : Rr[2], d2 ? Rr[1] : Rr[3], Rr[4]};
+  double f[5];
+  hllc2(g, l, r, f);
+  F[0] = f[0];
+  F[1] = d2 ? f[3] : f[1];
+  F[2] = d2 ? f[1] : f[2];
+  F[3] = d2 ? f[2] : f[3];
+  F[4] = f[4];
+}
+
+}  // namespace ak

@@ -1,13 +1,36 @@
 // ak_stage.cu -- ak_hydro_stage kernels: fused c2p + reconstruction + HLLC in x1/x2/x3 +
-// flux divergence + RK2 weighted update.  FMA contraction is allowed here (parity is to 1e-12, not
-// bit-exact).
+// flux divergence + RK2 weighted update.  Compiled with -fmad=false: every fused multiply-add of the
+// production kernel is written out, so the same face solved by two tiles gives the same bits
+// (DESIGN.md section 6.2).
 #include "ak_pack.h"
 #include "ak_physics.cuh"
 #include "ak_stage_simple.cuh"
 #include "ak_stage_tiled.cuh"
 #include "ak_stage_tma.cuh"
+#include "ak_stage_v2.cuh"
+
+#include <cstdlib>
 
 namespace ak {
+
+// tile shape of the production kernel: 0 = 16x12 (2 CTAs/SM), 1 = 16x8 (3 CTAs/SM), 2 = 32x6 (2 CTAs/SM)
+static int pick_tile(const ak_pack& p) {
+  static int forced = -2;
+  if (forced == -2) { const char* e = std::getenv("AK_TILE"); forced = e ? std::atoi(e) : -1; }
+  if (forced >= 0) return forced;
+  return (p.d.nx[1] % 12 == 0 || p.d.nx[1] >= 48) ? 0 : 1;
+}
+
+template <int RECON>
+static cudaError_t launch_stage_v2(const ak_pack& p, const double* Uin, const double* U0, double* Uout,
+                                   const StageCoef& sc) {
+  const bool stage2 = (Uin != U0);
+  switch (pick_tile(p)) {
+    case 1:  return launch_v2<RECON, 16, 8, 3>(p, Uin, U0, Uout, sc, stage2);
+    case 2:  return launch_v2<RECON, 32, 6, 2>(p, Uin, U0, Uout, sc, stage2);
+    default: return launch_v2<RECON, 16, 12, 2>(p, Uin, U0, Uout, sc, stage2);
+  }
+}
 
 cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, double* Uout, const StageCoef& sc) {
   if (p.variant == 1) return launch_stage_simple(p, Uin, U0, Uout, sc);
@@ -15,7 +38,8 @@ cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, 
   // an odd surplus of ghost layers (ng = 4 with PPM4, ng = 3 with PLM) takes the LDG-staged tiled kernel.
   const int R = (p.recon == 0) ? 2 : 3;
   if (p.variant == 2 || ((p.d.ng - R) & 1)) return launch_stage_tiled(p, Uin, U0, Uout, sc);
-  return launch_stage_tma(p, Uin, U0, Uout, sc);
+  if (p.variant == 3) return launch_stage_tma(p, Uin, U0, Uout, sc);
+  return p.recon == 0 ? launch_stage_v2<0>(p, Uin, U0, Uout, sc) : launch_stage_v2<1>(p, Uin, U0, Uout, sc);
 }
 
 int stage_launches_per_call(const ak_pack&) { return 1; }
