@@ -20,15 +20,16 @@ __device__ __forceinline__ bool pos(double x) { return __double2hiint(x) > 0; }
 __device__ __forceinline__ double max0(double x) { return neg(x) ? 0.0 : x; }
 __device__ __forceinline__ double min0(double x) { return neg(x) ? x : 0.0; }
 
-// 1/x to <= 1 ulp: MUFU seed (~20 bits) + two Newton steps                       4 FP64 + 1 MUFU
+// 1/x to ~1 ulp: MUFU seed (>= 20 bits, error e) + ONE cubically convergent step r (1 + e + e^2), whose
+// truncation error e^3 < 2^-60 is below the rounding error                      3 FP64 + 1 MUFU
 __device__ __forceinline__ double rcp2(double x) {
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
-  e = fma(-x, r, 1.0);
-  return fma(r, e, r);
+  const double e = fma(-x, r, 1.0);
+  return fma(r, fma(e, e, e), r);
 }
+// a / b to ~1.5 ulp                                                              4 FP64 + 1 MUFU
+__device__ __forceinline__ double div2(double a, double b) { return a * rcp2(b); }
 
 // ---- S1  conserved -> primitive ------------------------------------------------------------------
 __device__ __forceinline__ int c2p_lean(const double U[5], double W[5], double ug_floor) {
@@ -47,7 +48,7 @@ __device__ __forceinline__ int c2p_lean(const double U[5], double W[5], double u
 // PLM, van Leer: q-/q+ of the cell with neighbours (m1, c, p1)
 __device__ __forceinline__ void plm_lean(double m1, double c, double p1, double& qm, double& qp) {
   const double dL = c - m1, dR = p1 - c, prod = dL * dR;
-  const double q = div_lean(prod, dL + dR);          // discarded by the select where prod <= 0 (may be NaN)
+  const double q = div2(prod, dL + dR);          // discarded by the select where prod <= 0 (may be NaN)
   const double h = pos(prod) ? q : 0.0;
   qm = c - h; qp = c + h;
 }
@@ -61,29 +62,32 @@ __device__ __forceinline__ double iface_lean(double qm1, double q0, double q1, d
   v = (v > hi) ? hi : v;
   return v;
 }
-// PPM4 (iii): CW84 Eq.(1.10), straight-line                                                  ~15 FP64
+// PPM4 (iii): CW84 Eq.(1.10), straight-line, in difference form.  With x = aR - a, y = a - aL (same sign
+// unless the cell is an extremum) one has d = aR - aL = x + y, 6 mu = 3 (y - x), hence
+//   d mu >  d^2/6  <=>  d (y - 2x) > 0  <=>  y - 2x has the sign of y,   and then aL <- 3a - 2aR = a - 2x
+//   -d^2/6 > d mu  <=>  d (2y - x) < 0  <=>  2y - x has the sign of -y,  and then aR <- 3a - 2aL = a + 2y
+// The sign tests run on the integer pipe.  At a tie the replaced value equals the old one (the limiter is
+// continuous), so a decision that flips through rounding moves the result by rounding error only.   7 FP64
 __device__ __forceinline__ void limit_lean(double a, double& aL, double& aR) {
-  const bool flat = !pos((aR - a) * (a - aL));
-  const double d = aR - aL;
-  const double mu = fma(-0.5, aL + aR, a);
-  const double dmu = d * mu, d26 = (d * d) * (1.0 / 6.0);
-  const double a3 = 3.0 * a;
-  const double nL = fma(-2.0, aR, a3), nR = fma(-2.0, aL, a3);
-  const bool cL = dmu > d26, cR = (-d26 > dmu);
+  const double x = aR - a, y = a - aL;
+  const bool flat = !pos(x * y);
+  const double tL = fma(-2.0, x, y), tR = fma(2.0, y, -x);
+  const double nL = fma(-2.0, x, a), nR = fma(2.0, y, a);
+  const int hy = __double2hiint(y);
+  const bool cL = (__double2hiint(tL) ^ hy) >= 0, cR = (__double2hiint(tR) ^ hy) < 0;
   aL = flat ? a : (cL ? nL : aL);
   aR = flat ? a : (cR ? nR : aR);
 }
 
-// sqrt(a / b) for a, b > 0 without a division: r ~ (a b)^(-1/2), s = a r, one residual step on s^2 b = a
-__device__ __forceinline__ double sqrt_ratio(double a, double b) {                // 10 FP64 + 1 MUFU
+// sqrt(a / b) = a (a b)^(-1/2) for a, b > 0 without a division: MUFU seed r of t^(-1/2) (error e = 1 - t r^2
+// <= 2^-19) + ONE cubic (Halley) step r (1 + e/2 + 3 e^2/8), truncation 5/16 e^3 < 2^-58    7 FP64 + 1 MUFU
+__device__ __forceinline__ double sqrt_ratio(double a, double b) {
   const double t = a * b;
   double r;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(t));
-  const double e = fma(-(0.5 * t) * r, r, 0.5);
-  r = fma(r, e, r);
-  const double s = a * r;
-  const double res = fma(-(s * b), s, a);
-  return fma(res, 0.5 * r, s);
+  const double e = fma(-(t * r), r, 1.0);
+  r = fma(r, e * fma(0.375, e, 0.5), r);
+  return a * r;
 }
 
 // ---- S3  HLLC, rotated states (rho, u_normal, v, w, u_g) -------------------------------------------
@@ -95,7 +99,8 @@ __device__ __forceinline__ void hllc2(const GasConst& g, const double WL[5], con
   const double rL = WL[0], uL = WL[1], eL = WL[4];
   const double rR = WR[0], uR = WR[1], eR = WR[4];
   const double pL = g.gm1 * eL, pR = g.gm1 * eR;
-  const double gpL = g.gamma * pL, gpR = g.gamma * pR;
+  const double ggm1 = g.gamma * g.gm1;
+  const double gpL = ggm1 * eL, gpR = ggm1 * eR;
   const double cL = sqrt_ratio(gpL, rL), cR = sqrt_ratio(gpR, rR);
   const double ppv = fma(0.125, ((uL - uR) * (rL + rR)) * (cL + cR), 0.5 * (pL + pR));
   const double ggq = g.gamma * g.gq;
@@ -103,7 +108,7 @@ __device__ __forceinline__ void hllc2(const GasConst& g, const double WL[5], con
   const double cqR = sqrt_ratio(fma(ggq, max0(ppv - pR), gpR), rR);
   const double SL = uL - cqL, SR = uR + cqR;
   const double mL = rL * cqL, mR = rR * cqR;
-  const double Ss = div_lean((pL - pR) + fma(mL, uL, mR * uR), mL + mR);
+  const double Ss = div2((pL - pR) + fma(mL, uL, mR * uR), mL + mR);
   const double psL = fma(-mL, Ss - uL, pL);
   const double psR = fma(mR, Ss - uR, pR);
   const double ps = max0(0.5 * (psL + psR));
