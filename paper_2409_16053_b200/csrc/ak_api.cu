@@ -150,12 +150,13 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
   p->u[0] = (double*)u_a; p->u[1] = (double*)u_b; p->scratch = scratch; p->stream = st;
   p->cur = 0; p->ghosts_ok = false; p->bound = true; p->launches = 0;
   p->tmap_box[0] = p->tmap_box[1] = 0;
+  p->tmap0_box[0] = p->tmap0_box[1] = 0;
   return AK_OK;
 }
 
 extern "C" int ak_pack_set_variant(ak_pack* p, int variant) {
   if (!p) return fail(AK_EINVAL, "null pack");
-  if (variant < 0 || variant > 3) return fail(AK_EINVAL, "unknown variant");
+  if (variant < 0 || variant > 4) return fail(AK_EINVAL, "unknown variant");
   p->variant = variant;
   return AK_OK;
 }

@@ -55,12 +55,13 @@ __device__ __forceinline__ void plm_lean(double m1, double c, double p1, double&
 
 // PPM4 (i)+(ii): 4th-order interface value between q0 and q1 clamped into [min,max](q0,q1)   7 FP64
 __device__ __forceinline__ double iface_lean(double qm1, double q0, double q1, double q2) {
-  double v = fma(7.0, q0 + q1, -(qm1 + q2)) * (1.0 / 12.0);
-  const bool up = q0 < q1;
-  const double lo = up ? q0 : q1, hi = up ? q1 : q0;
-  v = (v < lo) ? lo : v;
-  v = (v > hi) ? hi : v;
-  return v;
+  const double v = fma(7.0, q0 + q1, -(qm1 + q2)) * (1.0 / 12.0);
+  // median(v, q0, q1) with three compares whose XORs fold into the DSETPs, and two selects
+  const bool c0 = v < q0;
+  const bool inside = (v < q1) != c0;          // v strictly between q0 and q1
+  const bool far = (q0 < q1) != c0;            // otherwise: the bound on v's side is q1 (else q0)
+  const double bound = far ? q1 : q0;
+  return inside ? v : bound;
 }
 // PPM4 (iii): CW84 Eq.(1.10), straight-line, in difference form.  With x = aR - a, y = a - aL (same sign
 // unless the cell is an extremum) one has d = aR - aL = x + y, 6 mu = 3 (y - x), hence
@@ -149,6 +150,78 @@ __device__ __forceinline__ void flux2_12(const GasConst& g, bool d2, const doubl
   F[2] = d2 ? f[1] : f[2];
   F[3] = d2 ? f[2] : f[3];
   F[4] = f[4];
+}
+
+// N independent faces solved in lock step: every statement of hllc2 is written as a loop over the faces, so
+// that the N dependency chains (about 45 FP64 operations deep at ~9 cycles each on sm_100a) are adjacent in
+// the instruction stream and ptxas can interleave them.  Same arithmetic per face as hllc2, bit for bit.
+template <int N>
+__device__ __forceinline__ void hllc2n(const GasConst& g, const double WL[N][5], const double WR[N][5], double F[N][5]) {
+  const double ggm1 = g.gamma * g.gm1, ggq = g.gamma * g.gq;
+  double pL[N], pR[N], gpL[N], gpR[N], cL[N], cR[N], ppv[N], cqL[N], cqR[N], SL[N], SR[N], mL[N], mR[N], Ss[N];
+#pragma unroll
+  for (int f = 0; f < N; f++) { pL[f] = g.gm1 * WL[f][4]; pR[f] = g.gm1 * WR[f][4]; }
+#pragma unroll
+  for (int f = 0; f < N; f++) { gpL[f] = ggm1 * WL[f][4]; gpR[f] = ggm1 * WR[f][4]; }
+#pragma unroll
+  for (int f = 0; f < N; f++) { cL[f] = sqrt_ratio(gpL[f], WL[f][0]); cR[f] = sqrt_ratio(gpR[f], WR[f][0]); }
+#pragma unroll
+  for (int f = 0; f < N; f++)
+    ppv[f] = fma(0.125, ((WL[f][1] - WR[f][1]) * (WL[f][0] + WR[f][0])) * (cL[f] + cR[f]), 0.5 * (pL[f] + pR[f]));
+#pragma unroll
+  for (int f = 0; f < N; f++) {
+    cqL[f] = sqrt_ratio(fma(ggq, max0(ppv[f] - pL[f]), gpL[f]), WL[f][0]);
+    cqR[f] = sqrt_ratio(fma(ggq, max0(ppv[f] - pR[f]), gpR[f]), WR[f][0]);
+  }
+#pragma unroll
+  for (int f = 0; f < N; f++) {
+    SL[f] = WL[f][1] - cqL[f]; SR[f] = WR[f][1] + cqR[f];
+    mL[f] = WL[f][0] * cqL[f]; mR[f] = WR[f][0] * cqR[f];
+  }
+#pragma unroll
+  for (int f = 0; f < N; f++)
+    Ss[f] = div2((pL[f] - pR[f]) + fma(mL[f], WL[f][1], mR[f] * WR[f][1]), mL[f] + mR[f]);
+  double ps[N], rK[N], uK[N], vK[N], wK[N], eK[N], pK[N], b[N];
+#pragma unroll
+  for (int f = 0; f < N; f++) {
+    const double psL = fma(-mL[f], Ss[f] - WL[f][1], pL[f]);
+    const double psR = fma(mR[f], Ss[f] - WR[f][1], pR[f]);
+    ps[f] = max0(0.5 * (psL + psR));
+    const bool left = !neg(Ss[f]);
+    rK[f] = left ? WL[f][0] : WR[f][0]; uK[f] = left ? WL[f][1] : WR[f][1];
+    vK[f] = left ? WL[f][2] : WR[f][2]; wK[f] = left ? WL[f][3] : WR[f][3];
+    eK[f] = left ? WL[f][4] : WR[f][4]; pK[f] = left ? pL[f] : pR[f];
+    b[f] = left ? min0(SL[f]) : max0(SR[f]);
+  }
+  double EK[N], mom[N], inv[N];
+#pragma unroll
+  for (int f = 0; f < N; f++) {
+    EK[f] = fma(0.5 * rK[f], fma(uK[f], uK[f], fma(vK[f], vK[f], wK[f] * wK[f])), eK[f]);
+    mom[f] = rK[f] * uK[f];
+    inv[f] = rcp2(Ss[f] - b[f]);
+  }
+#pragma unroll
+  for (int f = 0; f < N; f++) {
+    const double w = Ss[f] * inv[f];               // S*/(S* - b)
+    const double bps = b[f] * ps[f];
+    const double f0 = fma(-b[f], rK[f], mom[f]) * w;
+    F[f][0] = f0;
+    F[f][1] = fma(Ss[f], fma(-b[f], mom[f], fma(mom[f], uK[f], pK[f])), -bps) * inv[f];
+    F[f][2] = f0 * vK[f];
+    F[f][3] = f0 * wK[f];
+    F[f][4] = (fma(-b[f], EK[f], (EK[f] + pK[f]) * uK[f]) - bps) * w;
+  }
+}
+
+// the lower x1 and x2 faces of one cell, solved together
+__device__ __forceinline__ void flux2_x1x2(const GasConst& g, const double L1[5], const double R1[5], const double L2[5],
+                                           const double R2[5], double F1[5], double F2[5]) {
+  const double l[2][5] = {{L1[0], L1[1], L1[2], L1[3], L1[4]}, {L2[0], L2[2], L2[3], L2[1], L2[4]}};
+  const double r[2][5] = {{R1[0], R1[1], R1[2], R1[3], R1[4]}, {R2[0], R2[2], R2[3], R2[1], R2[4]}};
+  double f[2][5];
+  hllc2n<2>(g, l, r, f);
+  F1[0] = f[0][0]; F1[1] = f[0][1]; F1[2] = f[0][2]; F1[3] = f[0][3]; F1[4] = f[0][4];
+  F2[0] = f[1][0]; F2[2] = f[1][1]; F2[3] = f[1][2]; F2[1] = f[1][3]; F2[4] = f[1][4];
 }
 
 }  // namespace ak

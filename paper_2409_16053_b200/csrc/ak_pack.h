@@ -53,6 +53,9 @@ struct ak_pack {
   // tensor maps over u[0], u[1] for the TMA stage kernel, rebuilt when the staging box changes
   mutable CUtensorMap tmap[2];
   mutable int tmap_box[2] = {0, 0};
+  // ... and the halo-free U0 boxes of the v3 kernel's stage 2
+  mutable CUtensorMap tmap0[2];
+  mutable int tmap0_box[2] = {0, 0};
 };
 
 namespace ak {

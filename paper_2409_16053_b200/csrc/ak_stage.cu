@@ -8,6 +8,7 @@
 #include "ak_stage_tiled.cuh"
 #include "ak_stage_tma.cuh"
 #include "ak_stage_v2.cuh"
+#include "ak_stage_v3.cuh"
 
 #include <cstdlib>
 
@@ -32,6 +33,31 @@ static cudaError_t launch_stage_v2(const ak_pack& p, const double* Uin, const do
   }
 }
 
+// tile shape of the v3 kernel (workers + one edge warp): the one that wastes the fewest lanes on the ragged
+// last tile row and on the edge warp.  0 = 16x10 (6 warps), 1 = 16x8 (5 warps)
+static int pick_tile_v3(const ak_pack& p) {
+  static int forced = -2;
+  if (forced == -2) { const char* e = std::getenv("AK_TILE"); forced = e ? std::atoi(e) : -1; }
+  if (forced >= 0) return forced;
+  const int n = p.d.nx[1];
+  const double e10 = (double)n / (((n + 9) / 10) * 10) * (160.0 / 192.0);
+  const double e8 = (double)n / (((n + 7) / 8) * 8) * (128.0 / 160.0);
+  return e10 >= e8 ? 0 : 1;
+}
+
+template <int RECON>
+static cudaError_t launch_stage_v3(const ak_pack& p, const double* Uin, const double* U0, double* Uout,
+                                   const StageCoef& sc) {
+  const bool stage2 = (Uin != U0);
+  switch (pick_tile_v3(p)) {
+    case 1:  return launch_v3<RECON, 16, 8, 2>(p, Uin, U0, Uout, sc, stage2);
+    case 2:  return launch_v3<RECON, 16, 22, 1>(p, Uin, U0, Uout, sc, stage2);
+    case 3:  return launch_v3<RECON, 32, 11, 1>(p, Uin, U0, Uout, sc, stage2);
+    case 4:  return launch_v3<RECON, 16, 10, 1>(p, Uin, U0, Uout, sc, stage2);
+    default: return launch_v3<RECON, 16, 10, 2>(p, Uin, U0, Uout, sc, stage2);
+  }
+}
+
 cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, double* Uout, const StageCoef& sc) {
   if (p.variant == 1) return launch_stage_simple(p, Uin, U0, Uout, sc);
   // TMA box origins must be 16-byte aligned in the innermost dimension: (ng - R) even.  The unusual case of
@@ -39,7 +65,8 @@ cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, 
   const int R = (p.recon == 0) ? 2 : 3;
   if (p.variant == 2 || ((p.d.ng - R) & 1)) return launch_stage_tiled(p, Uin, U0, Uout, sc);
   if (p.variant == 3) return launch_stage_tma(p, Uin, U0, Uout, sc);
-  return p.recon == 0 ? launch_stage_v2<0>(p, Uin, U0, Uout, sc) : launch_stage_v2<1>(p, Uin, U0, Uout, sc);
+  if (p.variant == 4) return p.recon == 0 ? launch_stage_v2<0>(p, Uin, U0, Uout, sc) : launch_stage_v2<1>(p, Uin, U0, Uout, sc);
+  return p.recon == 0 ? launch_stage_v3<0>(p, Uin, U0, Uout, sc) : launch_stage_v3<1>(p, Uin, U0, Uout, sc);
 }
 
 int stage_launches_per_call(const ak_pack&) { return 1; }
