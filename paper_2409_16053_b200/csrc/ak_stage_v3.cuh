@@ -126,7 +126,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
       }
     }
     int it = 0;
-    for (int s = k0 - R; s < send; s++, it++) {
+    for (int s = k0 - R; s < send - 1; s++, it++) {   // (iteration send-1 would have nothing to do)
       const int b = it & 1;
       const bool inplane = (s >= k0) && (s < k1);
       const double* Ws = sm + b * S::nUpad;
@@ -206,26 +206,28 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
 
   // L(s): conserved -> primitive of plane s in ring slot it & 1, T-ring bookkeeping, x3 pipeline
   int tslot = 0;                                        // T-ring slot of the plane being converted
+  // Straight-line on purpose: the x3 pipeline (wk, qlow, qp3, G) is updated unconditionally and only the
+  // stores are predicated, so that no conditional assignment of loop-carried registers (= register copies
+  // at every join) is left.  Threads outside a ragged tile and planes outside [k0, k1] compute on whatever
+  // the (zero-filled) staging holds; nothing of that is ever stored.
   auto phaseL = [&](int s, int it) {
     const bool inplane = (s >= k0) && (s < k1);
     double* Ws = sm + (it & 1) * S::nUpad;
     mbar_wait(&bars[it & 1], (it >> 1) & 1);
-    double wp[5] = {1.0, 0.0, 0.0, 0.0, 1.0};
-    if (valid) {
+    double wp[5];
+    {
       double u[5];
 #pragma unroll
       for (int n = 0; n < 5; n++) u[n] = Ws[n * (WJ * WI) + oW];
       const int f = c2p_lean(u, wp, g.ug_floor);
-      if (inplane) {
-        nfl += f;
-        double* Tn = sm + S::oT + tslot * (5 * NT) + tid;
-        const double* U0s = sm + S::oU0 + (it & 1) * S::nU0pad + oU0;
+      nfl += (inplane && valid) ? f : 0;
+      double* Tn = sm + S::oT + tslot * (5 * NT) + tid;
+      const double* U0s = sm + S::oU0 + (it & 1) * S::nU0pad + oU0;
 #pragma unroll
-        for (int n = 0; n < 5; n++) {
-          Ws[n * (WJ * WI) + oW] = wp[n];
-          if constexpr (STAGE2) Tn[n * NT] = fma(sc.g0, u[n], sc.g1 * U0s[n * (TJ * S::W0)]);
-          else Tn[n * NT] = u[n];                  // 0*U + 1*U of the stage-1 weights, exactly
-        }
+      for (int n = 0; n < 5; n++) {
+        if (valid) Ws[n * (WJ * WI) + oW] = wp[n];   // (outside a ragged tile this cell is another thread's halo)
+        if constexpr (STAGE2) Tn[n * NT] = fma(sc.g0, u[n], sc.g1 * U0s[n * (TJ * S::W0)]);
+        else Tn[n * NT] = u[n];                    // 0*U + 1*U of the stage-1 weights, exactly
       }
     }
     if (inplane) {
@@ -242,37 +244,31 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
       }
     }
     // x3: plane c = s-(R-1) becomes reconstructible; its lower face flux completes plane c-1
-    if (valid) {
-      double qm3[5], qpn[5];
+    double qm3[5], qpn[5];
 #pragma unroll
-      for (int n = 0; n < 5; n++) {
-        if constexpr (RECON == 0) {
-          plm_lean(wk[0][n], wk[1][n], wp[n], qm3[n], qpn[n]);
-        } else {
-          double hi = iface_lean(wk[0][n], wk[1][n], wk[2][n], wp[n]);
-          double lo = qlow[n];
-          qlow[n] = hi;
-          limit_lean(wk[1][n], lo, hi);
-          qm3[n] = lo; qpn[n] = hi;
-        }
+    for (int n = 0; n < 5; n++) {
+      if constexpr (RECON == 0) {
+        plm_lean(wk[0][n], wk[1][n], wp[n], qm3[n], qpn[n]);
+      } else {
+        double hi = iface_lean(wk[0][n], wk[1][n], wk[2][n], wp[n]);
+        double lo = qlow[n];
+        qlow[n] = hi;
+        limit_lean(wk[1][n], lo, hi);
+        qm3[n] = lo; qpn[n] = hi;
       }
-      const int c = s - (R - 1);
-      if (c >= k0 && c <= k1) {                    // uniform over the CTA
-        double Gn[5];
-        flux2<2>(g, qp3, qm3, Gn);
-        if (c > k0) {                              // plane c-1 complete: its slot is the one after tslot
-          const int ts = (tslot + 1 == NS) ? 0 : tslot + 1;
-          const double* Tc = sm + S::oT + ts * (5 * NT) + tid;
-          double* o = Uout + col + (long long)(c - 1 + ng) * plane;
-#pragma unroll
-          for (int n = 0; n < 5; n++) o[n * nc] = fma(-c3, Gn[n] - G[n], Tc[n * NT]);
-        }
-#pragma unroll
-        for (int n = 0; n < 5; n++) G[n] = Gn[n];
-      }
-#pragma unroll
-      for (int n = 0; n < 5; n++) qp3[n] = qpn[n];
     }
+    const int c = s - (R - 1);
+    double Gn[5];
+    flux2<2>(g, qp3, qm3, Gn);
+    if (c > k0 && c <= k1 && valid) {              // plane c-1 complete: its slot is the one after tslot
+      const int ts = (tslot + 1 == NS) ? 0 : tslot + 1;
+      const double* Tc = sm + S::oT + ts * (5 * NT) + tid;
+      double* o = Uout + col + (long long)(c - 1 + ng) * plane;
+#pragma unroll
+      for (int n = 0; n < 5; n++) o[n * nc] = fma(-c3, Gn[n] - G[n], Tc[n * NT]);
+    }
+#pragma unroll
+    for (int n = 0; n < 5; n++) { G[n] = Gn[n]; qp3[n] = qpn[n]; }
 #pragma unroll
     for (int a = 0; a + 1 < R; a++)
 #pragma unroll
@@ -284,7 +280,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
   int it = 0;
   phaseL(k0 - R, 0);
   int dslot = 0;                                        // T-ring slot of plane s (the one D(s) updates)
-  for (int s = k0 - R; s < send; s++, it++) {
+  for (int s = k0 - R; s < send - 1; s++, it++) {     // (iteration send-1 would have nothing to do)
     const int b = it & 1;
     const bool inplane = (s >= k0) && (s < k1);
     const double* Ws = sm + b * S::nUpad;
@@ -314,10 +310,8 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
       for (int n = 0; n < 5; n++) { Q1[n * (TJ * (TI + 1)) + oQ1] = F1[n]; Q2[n * ((TJ + 1) * TI) + oQ2] = F2[n]; }
     }
     // ---- L(s+1) ------------------------------------------------------------------------------------
-    if (s + 1 < send) {
-      tslot = (dslot + 1 == NS) ? 0 : dslot + 1;
-      phaseL(s + 1, it + 1);
-    }
+    tslot = (dslot + 1 == NS) ? 0 : dslot + 1;
+    phaseL(s + 1, it + 1);
     cta_sync(NTH);                                      // fluxes of plane s visible
     // ---- D(s) --------------------------------------------------------------------------------------
     if (inplane && valid) {
