@@ -27,6 +27,12 @@ METRIC = "3D hydro cell-updates/sec (fp64)"
 UNIT = "cell-updates/s"
 BYTES_PER_CELL_UPDATE = 200.0      # 5 streams x 5 vars x 8 B per RK2 cell-update
 BYTES_STAGE = {1: 80.0, 2: 120.0}  # per active cell: stage 1 reads U^n writes U^(1); stage 2 reads U^(1),U^n writes
+# FP64-pipe thread instructions per active cell per stage launch of the PPM4+HLLC kernel, counted by ncu on
+# cfg3 (profiles/r01_v3_stage_cfg3.md: 656 in stage 1, 666 in stage 2), and the same capture's DRAM bytes per
+# stage launch (12.31 GB and 17.71 GB); both are properties of the committed kernel, not of this run
+FP64_INSTR_PER_CELL_STAGE_PPM = 661.0
+NCU_DRAM_BYTES_PER_STAGE_LAUNCH_CFG3 = 15.01e9
+FP64_LANES_PER_SM = 64             # DESIGN.md 6.1 (ncu peak_sustained of the dfma counter / SM count)
 
 
 def workloads():
@@ -151,12 +157,12 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
 
     # ---- device-resident timing ------------------------------------------------------------------
+    sampler = ClockSampler(local)
+    sampler.start()                    # nvidia-smi needs a few 100 ms to come up: start it under the warm-up load
     for _ in range(args.warmup):
         pack.step(w.cfl)
     stage_ev = []
-    sampler = ClockSampler(local)
     barrier()
-    sampler.start()
     l0 = pack.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(pack.stream)
@@ -187,12 +193,26 @@ def run_ours(args):
     alg_bytes = 0.5 * (BYTES_STAGE[1] + BYTES_STAGE[2]) * ncell
     peaks, which = measured_peaks()
     achieved = alg_bytes / (stage_ms * 1e-3) / 1e9
+    traffic = args.traffic
+    if traffic is None and args.workload == "cfg3" and args.variant == 0:
+        traffic = NCU_DRAM_BYTES_PER_STAGE_LAUNCH_CFG3
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": achieved / peaks["hbm_gbs"], "traffic": args.traffic, "peak_source": which + " (MEASURED_PEAKS.json hbm_gbs)",
+                "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "peak_source": which + " (MEASURED_PEAKS.json hbm_gbs)",
                 "kernel": "ak_hydro_stage", "kernel_ms": stage_ms, "kernel_share_of_step": 2 * stage_ms * args.steps / elapsed_ms,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "whole_step": {"achieved": BYTES_PER_CELL_UPDATE * value / world / 1e9,
                                "frac": BYTES_PER_CELL_UPDATE * value / world / 1e9 / peaks["hbm_gbs"]}}
+
+    # the unit that actually binds the stage kernel is the FP64 pipe (plain ALU work)
+    roofline_alu = None
+    if w.recon == 1:
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak_alu = sms * FP64_LANES_PER_SM * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+        ach_alu = FP64_INSTR_PER_CELL_STAGE_PPM * ncell / (stage_ms * 1e-3) / 1e12
+        roofline_alu = {"bound": "alu", "achieved": ach_alu, "peak": peak_alu, "unit": "T FP64-pipe thread-instr/s",
+                        "frac": ach_alu / peak_alu, "kernel": "ak_hydro_stage",
+                        "instr_per_cell_launch": FP64_INSTR_PER_CELL_STAGE_PPM,
+                        "peak_source": f"{sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x sm_max_mhz (DESIGN.md 6.1)"}
 
     # ---- end to end through the C-ABI with HOST buffers ------------------------------------------
     e2e = None
@@ -227,7 +247,7 @@ def run_ours(args):
                        "cells": ncell, "state_bytes": state_bytes, "l2_policy": "inputs larger than L2 (no flush needed)"
                        if state_bytes > 4e8 else "state fits L2: numbers are L2-resident", "variant": args.variant,
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
-            "roofline": roofline, "cpu_baseline": cb, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "roofline": roofline, "roofline_alu": roofline_alu, "cpu_baseline": cb, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
             "stage_ms": st_ms, "floor_activations": floors,
         }))
     if world > 1:
@@ -237,7 +257,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3")
