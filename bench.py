@@ -110,6 +110,23 @@ def cpu_baseline(threads=1, target_s=12.0):
                       f"{el:.1f} s, single-threaded C++ oracle"}
 
 
+def max_over_ranks(x: float, device=None) -> float:
+    """Timing rule of the bench contract: a multi-rank time is the MAX over ranks (all-reduce on `device`;
+    identity when no process group exists)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([x], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(ncell_per_rank: int, steps: int, elapsed_ms_max: float, world: int) -> float:
+    """Whole-job cell-updates/s of `world` independent replicas (weak scaling)."""
+    return world * ncell_per_rank * steps / (elapsed_ms_max * 1e-3)
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -179,13 +196,9 @@ def run_ours(args):
     barrier()
     clocks = sampler.stop()
     launches = pack.launch_count() - l0
-    elapsed_ms = e0.elapsed_time(e1)
-    t = torch.tensor([elapsed_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    elapsed_ms = float(t.item())
+    elapsed_ms = max_over_ranks(e0.elapsed_time(e1), dev)
     floors = pack.floor_count()
-    value = world * ncell * args.steps / (elapsed_ms * 1e-3)
+    value = aggregate_value(ncell, args.steps, elapsed_ms, world)
 
     # dominant kernel = the stage kernel: algorithmic bytes per launch / mean launch duration
     st_ms = {s: statistics.mean(a.elapsed_time(b) for ss, a, b in stage_ev if ss == s) for s in (1, 2)}
@@ -228,11 +241,8 @@ def run_ours(args):
             pack.step(w.cfl)
             pack.download(host)            # D2H of the step's result; synchronises
         torch.cuda.synchronize(dev)
-        el = time.perf_counter() - t0
-        t = torch.tensor([el], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * ncell * nst / float(t.item()), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+        el = max_over_ranks(time.perf_counter() - t0, dev)
+        e2e = {"value": aggregate_value(ncell, nst, el * 1e3, world), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
                "d2h_bytes_per_step": state_bytes, "steps": nst}
         del host
 
