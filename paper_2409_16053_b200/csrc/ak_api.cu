@@ -20,8 +20,8 @@ extern "C" const char* ak_last_error(void) { return g_err.c_str(); }
 
 static size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
 
-// scratch layout: [0,256) reduction cells | block table int4[nmb] | leaf0 | leaf1
-struct ScratchLayout { size_t blk, leaf0, leaf1, total; };
+// scratch layout: [0,256) reduction cells | block table int4[nmb] | leaf0 | leaf1 | same-level neighbours int[nmb][27]
+struct ScratchLayout { size_t blk, leaf0, leaf1, nbr, total; };
 static ScratchLayout scratch_layout(const ak_pack* p) {
   ScratchLayout s;
   const ak::PackDev& d = p->d;
@@ -29,7 +29,8 @@ static ScratchLayout scratch_layout(const ak_pack* p) {
   s.blk = 256;
   s.leaf0 = s.blk + align256(sizeof(int4) * (size_t)d.nmb);
   s.leaf1 = s.leaf0 + align256(sizeof(int) * n0);
-  s.total = s.leaf1 + align256(sizeof(int) * 8 * n0);
+  s.nbr = s.leaf1 + align256(sizeof(int) * 8 * n0);
+  s.total = s.nbr + align256(sizeof(int) * 27 * (size_t)d.nmb);
   return s;
 }
 
@@ -133,8 +134,22 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
   cudaStream_t st = (cudaStream_t)cuda_stream;
   std::vector<int4> blk(d.nmb);
   for (int m = 0; m < d.nmb; m++) blk[m] = make_int4(p->level[m], p->lx[3 * m], p->lx[3 * m + 1], p->lx[3 * m + 2]);
+  // same-level neighbour of block m in direction (d1, d2, d3) in {-1,0,1}^3 (periodic wrap), or -1 where the
+  // position is covered by a leaf of another level (the ghost fill then takes the general path)
+  std::vector<int> nbr(27 * (size_t)d.nmb, -1);
+  for (int m = 0; m < d.nmb; m++) {
+    const int lev = p->level[m];
+    const int nb[3] = {d.nrb[0] << lev, d.nrb[1] << lev, d.nrb[2] << lev};
+    const std::vector<int>& leaf = lev ? leaf1 : leaf0;
+    for (int d3 = -1; d3 <= 1; d3++) for (int d2 = -1; d2 <= 1; d2++) for (int d1 = -1; d1 <= 1; d1++) {
+      const int b1 = (p->lx[3 * m] + d1 + nb[0]) % nb[0], b2 = (p->lx[3 * m + 1] + d2 + nb[1]) % nb[1];
+      const int b3 = (p->lx[3 * m + 2] + d3 + nb[2]) % nb[2];
+      nbr[27 * (size_t)m + (d3 + 1) * 9 + (d2 + 1) * 3 + (d1 + 1)] = leaf[((size_t)b3 * nb[1] + b2) * nb[0] + b1];
+    }
+  }
   char* s = (char*)scratch;
   AK_CUDA(cudaMemsetAsync(s, 0, 256, st), "memset scratch");
+  AK_CUDA(cudaMemcpyAsync(s + sl.nbr, nbr.data(), sizeof(int) * nbr.size(), cudaMemcpyHostToDevice, st), "upload neighbour table");
   AK_CUDA(cudaMemcpyAsync(s + sl.blk, blk.data(), sizeof(int4) * d.nmb, cudaMemcpyHostToDevice, st), "upload block table");
   AK_CUDA(cudaMemcpyAsync(s + sl.leaf0, leaf0.data(), sizeof(int) * n0, cudaMemcpyHostToDevice, st), "upload leaf map 0");
   AK_CUDA(cudaMemcpyAsync(s + sl.leaf1, leaf1.data(), sizeof(int) * 8 * n0, cudaMemcpyHostToDevice, st), "upload leaf map 1");
@@ -144,6 +159,7 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
   d.blk = (const int4*)(s + sl.blk);
   d.leaf0 = (const int*)(s + sl.leaf0);
   d.leaf1 = (const int*)(s + sl.leaf1);
+  d.nbr = (const int*)(s + sl.nbr);
   int dev = 0;
   AK_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
   AK_CUDA(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev), "query SM count");

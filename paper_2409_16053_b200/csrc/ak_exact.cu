@@ -60,9 +60,93 @@ __device__ __forceinline__ double minmod(double a, double b) {
   return a > 0.0 ? m : -m;
 }
 
-// One thread per ghost cell (all 5 variables).  The ghost shell of a block is enumerated as
-// k-slabs, then j-slabs, then i-slabs so that consecutive threads touch consecutive i.
-__global__ void __launch_bounds__(256) fill_ghosts_kernel(PackDev P, double* __restrict__ U, int nghost) {
+// General path (G1-G4 of DESIGN.md): value of ghost cell (i, j, k) of block m from the leaf maps.
+__device__ void ghost_general(const PackDev& P, const double* __restrict__ U, int m, int i, int j, int k, double val[5]) {
+  const int ng = P.ng;
+  const int4 b = P.blk[m];
+  const int lev = b.x;
+  // G1: which leaf covers the periodic image of this ghost cell?
+  const int G1 = wrap1(b.y * P.nx[0] + i - ng, nglob(P, lev, 0));
+  const int G2 = wrap1(b.z * P.nx[1] + j - ng, nglob(P, lev, 1));
+  const int G3 = wrap1(b.w * P.nx[2] + k - ng, nglob(P, lev, 2));
+  const int src = find_leaf(P, lev, G1 / P.nx[0], G2 / P.nx[1], G3 / P.nx[2]);
+  if (src >= 0) {                                           // G2: same level, copy
+    long long a = leaf_cell(P, src, P.blk[src], G1, G2, G3);
+    for (int n = 0; n < 5; n++) val[n] = U[a + n * P.ncell];
+  } else if (lev == 0) {                                    // G3: finer neighbour
+    restrict5(P, U, 0, G1, G2, G3, val);
+  } else {                                                  // G4: coarser neighbour
+    const int C1 = G1 >> 1, C2 = G2 >> 1, C3 = G3 >> 1;
+    const double s1 = (double)(2 * (G1 & 1) - 1), s2 = (double)(2 * (G2 & 1) - 1), s3 = (double)(2 * (G3 & 1) - 1);
+    double c0[5], cm[5], cp[5], g1[5], g2[5], g3[5];
+    coarse5(P, U, lev - 1, C1, C2, C3, c0);
+    coarse5(P, U, lev - 1, C1 - 1, C2, C3, cm); coarse5(P, U, lev - 1, C1 + 1, C2, C3, cp);
+    for (int n = 0; n < 5; n++) g1[n] = 0.25 * minmod(c0[n] - cm[n], cp[n] - c0[n]);
+    coarse5(P, U, lev - 1, C1, C2 - 1, C3, cm); coarse5(P, U, lev - 1, C1, C2 + 1, C3, cp);
+    for (int n = 0; n < 5; n++) g2[n] = 0.25 * minmod(c0[n] - cm[n], cp[n] - c0[n]);
+    coarse5(P, U, lev - 1, C1, C2, C3 - 1, cm); coarse5(P, U, lev - 1, C1, C2, C3 + 1, cp);
+    for (int n = 0; n < 5; n++) g3[n] = 0.25 * minmod(c0[n] - cm[n], cp[n] - c0[n]);
+    for (int n = 0; n < 5; n++) val[n] = ((c0[n] + s1 * g1[n]) + s2 * g2[n]) + s3 * g3[n];
+  }
+}
+
+// One ghost cell, all 5 variables.  Fast path: the same-level neighbour table built at bind time says which
+// block holds the periodic image, and the source cell is the ghost index shifted by one block length (no
+// division, one table load).  Where the table holds -1 (another level covers the position) the general
+// path classifies the cell from the leaf maps.
+// (Uniform meshes only: every table entry is a block there, so the kernel needs no general path and keeps a
+// small register footprint -- 48 registers against 128 -- and with it the occupancy a copy kernel wants.)
+__device__ __forceinline__ void fill_cell(const PackDev& P, double* __restrict__ U, const int* __restrict__ nb,
+                                          int m, int i, int j, int k) {
+  const int ng = P.ng, n1 = P.nt[0], n2 = P.nt[1];
+  const int d1 = (i < ng) ? -1 : (i >= P.nx[0] + ng ? 1 : 0);
+  const int d2 = (j < ng) ? -1 : (j >= P.nx[1] + ng ? 1 : 0);
+  const int d3 = (k < ng) ? -1 : (k >= P.nx[2] + ng ? 1 : 0);
+  const int src = nb[(d3 + 1) * 9 + (d2 + 1) * 3 + (d1 + 1)];
+  double val[5];
+  if (src < 0) return;                 // cannot happen on a uniform mesh
+  const int si = i - d1 * P.nx[0], sj = j - d2 * P.nx[1], sk = k - d3 * P.nx[2];
+  const double* q = U + (long long)src * 5 * P.ncell + ((long long)sk * n2 + sj) * n1 + si;
+#pragma unroll
+  for (int n = 0; n < 5; n++) val[n] = q[n * P.ncell];
+  double* o = U + (long long)m * 5 * P.ncell + ((long long)k * n2 + j) * n1 + i;
+#pragma unroll
+  for (int n = 0; n < 5; n++) o[n * P.ncell] = val[n];
+}
+
+// One warp per row of the ghost shell: the 2 ng n2 rows of the two k-slabs and the nx3 2 ng rows of the two
+// j-slabs are full rows of n1 cells (lanes stride along i: coalesced); the nx3 nx2 interior rows have only
+// their 2 ng end cells in the shell, and one warp takes 32 / (2 ng) of those rows at once.
+__global__ void __launch_bounds__(256) fill_ghosts_kernel(PackDev P, double* __restrict__ U, int rowsA, int rowsB,
+                                                          int groupsC, int rpg) {
+  const int m = blockIdx.y, lane = threadIdx.x & 31;
+
+  const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int ng = P.ng, n1 = P.nt[0], n2 = P.nt[1];
+  const int* nb = P.nbr + 27 * m;
+  if (w < rowsA + rowsB) {
+    int j, k;
+    if (w < rowsA) { const int kk = w / n2; j = w - kk * n2; k = kk < ng ? kk : kk + P.nx[2]; }
+    else { const int r = w - rowsA; const int kk = r / (2 * ng), jj = r - kk * (2 * ng); k = ng + kk; j = jj < ng ? jj : jj + P.nx[1]; }
+    for (int i = lane; i < n1; i += 32) fill_cell(P, U, nb, m, i, j, k);
+  } else if (w < rowsA + rowsB + groupsC) {
+    const int g = w - rowsA - rowsB;
+    for (int c = lane; c < rpg * 2 * ng; c += 32) {     // one pass unless 2 ng > 32
+      const int sub = c / (2 * ng), ii = c - sub * (2 * ng);
+      const int row = g * rpg + sub;
+      if (row < P.nx[2] * P.nx[1]) {
+        const int kk = row / P.nx[1], jj = row - kk * P.nx[1];
+        fill_cell(P, U, nb, m, ii < ng ? ii : ii + P.nx[0], ng + jj, ng + kk);
+      }
+    }
+  }
+}
+
+// Refined meshes: one thread per ghost cell, every cell through the general path (copy, restriction or
+// prolongation decided per cell from the leaf maps).  The ghost shell of a block is enumerated as k-slabs,
+// then j-slabs, then i-slabs so that consecutive threads touch consecutive i; the few expensive
+// prolongation cells are spread over many warps and overlap with the cheap copies of the same launch.
+__global__ void __launch_bounds__(256) fill_ghosts_flat_kernel(PackDev P, double* __restrict__ U, int nghost) {
   const int m = blockIdx.y;
   int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= nghost) return;
@@ -87,41 +171,26 @@ __global__ void __launch_bounds__(256) fill_ghosts_kernel(PackDev P, double* __r
     j = ng + jj;
     i = ii < ng ? ii : ii + P.nx[0];
   }
-  const int4 b = P.blk[m];
-  const int lev = b.x;
-  // G1: which leaf covers the periodic image of this ghost cell?
-  const int G1 = wrap1(b.y * P.nx[0] + i - ng, nglob(P, lev, 0));
-  const int G2 = wrap1(b.z * P.nx[1] + j - ng, nglob(P, lev, 1));
-  const int G3 = wrap1(b.w * P.nx[2] + k - ng, nglob(P, lev, 2));
   double val[5];
-  const int src = find_leaf(P, lev, G1 / P.nx[0], G2 / P.nx[1], G3 / P.nx[2]);
-  if (src >= 0) {                                           // G2: same level, copy
-    long long a = leaf_cell(P, src, P.blk[src], G1, G2, G3);
-    for (int n = 0; n < 5; n++) val[n] = U[a + n * P.ncell];
-  } else if (lev == 0) {                                    // G3: finer neighbour
-    restrict5(P, U, 0, G1, G2, G3, val);
-  } else {                                                  // G4: coarser neighbour
-    const int C1 = G1 >> 1, C2 = G2 >> 1, C3 = G3 >> 1;
-    const double s1 = (double)(2 * (G1 & 1) - 1), s2 = (double)(2 * (G2 & 1) - 1), s3 = (double)(2 * (G3 & 1) - 1);
-    double c0[5], cm[5], cp[5], g1[5], g2[5], g3[5];
-    coarse5(P, U, lev - 1, C1, C2, C3, c0);
-    coarse5(P, U, lev - 1, C1 - 1, C2, C3, cm); coarse5(P, U, lev - 1, C1 + 1, C2, C3, cp);
-    for (int n = 0; n < 5; n++) g1[n] = 0.25 * minmod(c0[n] - cm[n], cp[n] - c0[n]);
-    coarse5(P, U, lev - 1, C1, C2 - 1, C3, cm); coarse5(P, U, lev - 1, C1, C2 + 1, C3, cp);
-    for (int n = 0; n < 5; n++) g2[n] = 0.25 * minmod(c0[n] - cm[n], cp[n] - c0[n]);
-    coarse5(P, U, lev - 1, C1, C2, C3 - 1, cm); coarse5(P, U, lev - 1, C1, C2, C3 + 1, cp);
-    for (int n = 0; n < 5; n++) g3[n] = 0.25 * minmod(c0[n] - cm[n], cp[n] - c0[n]);
-    for (int n = 0; n < 5; n++) val[n] = ((c0[n] + s1 * g1[n]) + s2 * g2[n]) + s3 * g3[n];
-  }
+  ghost_general(P, U, m, i, j, k, val);
   const long long o = (long long)m * 5 * P.ncell + ((long long)k * n2 + j) * n1 + i;
   for (int n = 0; n < 5; n++) U[o + n * P.ncell] = val[n];
 }
 
 cudaError_t launch_fill_ghosts(const ak_pack& p, double* U) {
   const PackDev& P = p.d;
-  long long nghost = P.ncell - (long long)P.nx[0] * P.nx[1] * P.nx[2];
-  dim3 grid((unsigned)((nghost + 255) / 256), (unsigned)P.nmb);
-  fill_ghosts_kernel<<<grid, 256, 0, p.stream>>>(P, U, (int)nghost);
+  if (P.max_level > 0) {
+    long long nghost = P.ncell - (long long)P.nx[0] * P.nx[1] * P.nx[2];
+    dim3 grid((unsigned)((nghost + 255) / 256), (unsigned)P.nmb);
+    fill_ghosts_flat_kernel<<<grid, 256, 0, p.stream>>>(P, U, (int)nghost);
+    return cudaGetLastError();
+  }
+  const int rowsA = 2 * P.ng * P.nt[1], rowsB = P.nx[2] * 2 * P.ng;
+  const int rpg = 32 / (2 * P.ng) > 0 ? 32 / (2 * P.ng) : 1;
+  const int groupsC = (P.nx[2] * P.nx[1] + rpg - 1) / rpg;
+  const int warps = rowsA + rowsB + groupsC;
+  dim3 grid((unsigned)((warps + 7) / 8), (unsigned)P.nmb);
+  fill_ghosts_kernel<<<grid, 256, 0, p.stream>>>(P, U, rowsA, rowsB, groupsC, rpg);
   return cudaGetLastError();
 }
 
@@ -133,22 +202,27 @@ __global__ void dt_init_kernel(PackDev P) { *P.dtmin_bits = 0x7FF0000000000000ul
 __global__ void __launch_bounds__(256) new_dt_kernel(PackDev P, const double* __restrict__ U, long long nrows) {
   const double ug_floor = P_FLOOR / (P.gamma - 1.0);
   double best = __longlong_as_double(0x7FF0000000000000ll);
-  // one warp per row of nx1 active cells; rows enumerated over (m, k, j)
+  // one warp per group of rpw rows of nx1 active cells (rpw = 32 / nx1 rows of one block when nx1 <= 16, so
+  // that short rows still fill the warp; else 1); groups enumerated over (m, k, j-group)
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+  const int rpw = P.nx[0] <= 16 ? 32 / P.nx[0] : 1;
+  const int jg = (P.nx[1] + rpw - 1) / rpw;
+  const int lj = rpw > 1 ? lane / P.nx[0] : 0, li = rpw > 1 ? lane - lj * P.nx[0] : lane;
   for (long long row = (long long)blockIdx.x * wpb + wib; row < nrows; row += (long long)gridDim.x * wpb) {
     long long r = row;
-    int j = (int)(r % P.nx[1]); r /= P.nx[1];
+    int j = (int)(r % jg) * rpw + lj; r /= jg;
     int k = (int)(r % P.nx[2]); r /= P.nx[2];
     int m = (int)r;
     const int lev = P.blk[m].x;
     const double sc = lev ? 0.5 : 1.0;
     const double dx1 = sc * P.dx0[0], dx2 = sc * P.dx0[1], dx3 = sc * P.dx0[2];
+    const bool rowok = (j < P.nx[1]) && (lj < rpw);
     const double* q = U + (long long)m * 5 * P.ncell + ((long long)(k + P.ng) * P.nt[1] + (j + P.ng)) * P.nt[0] + P.ng;
     // dx_d / s is monotone in s > 0 (IEEE division rounds monotonically), so the row's min over cells of
     // dx_d / (|v_d| + c_s) is dx_d / max(|v_d| + c_s), bit for bit: three divisions per row instead of per cell
     double s1 = 0.0, s2 = 0.0, s3 = 0.0;
 #pragma unroll 2
-    for (int i = lane; i < P.nx[0]; i += 32) {
+    for (int i = li; rowok && i < P.nx[0]; i += 32) {
       double u[5], w[5];
       for (int n = 0; n < 5; n++) u[n] = q[i + n * P.ncell];
       c2p(u, w, ug_floor);
@@ -173,7 +247,8 @@ __global__ void __launch_bounds__(256) new_dt_kernel(PackDev P, const double* __
 cudaError_t launch_new_dt(const ak_pack& p, const double* U) {
   const PackDev& P = p.d;
   dt_init_kernel<<<1, 1, 0, p.stream>>>(P);
-  long long nrows = (long long)P.nmb * P.nx[1] * P.nx[2];
+  const int rpw = P.nx[0] <= 16 ? 32 / P.nx[0] : 1;
+  long long nrows = (long long)P.nmb * ((P.nx[1] + rpw - 1) / rpw) * P.nx[2];
   long long want = (nrows + 7) / 8;
   int grid = (int)(want < (long long)p.sm_count * 8 ? want : (long long)p.sm_count * 8);
   new_dt_kernel<<<grid, 256, 0, p.stream>>>(P, U, nrows);

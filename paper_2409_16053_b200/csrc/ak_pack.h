@@ -23,6 +23,7 @@ struct PackDev {
   const int4* blk;  // (level, lx1, lx2, lx3) per block
   const int* leaf0; // [nrb3][nrb2][nrb1]       -> block index or -1
   const int* leaf1; // [2nrb3][2nrb2][2nrb1]    -> block index or -1
+  const int* nbr;   // [nmb][27] same-level neighbour in direction (d3+1)*9+(d2+1)*3+(d1+1), or -1
   double dx0[3];    // level-0 cell size; level 1 is exactly half
   double gamma;
   unsigned long long* dtmin_bits;   // scratch cell: min candidate dt as ordered bits
