@@ -114,10 +114,19 @@ int ak_pack_download(ak_pack*, void* host_u);
  * (diagnostic; 0 on all BASELINE configs).  Synchronises the stream.  Negative on error. */
 long long ak_pack_floor_count(ak_pack*);
 
-/* Selects the implementation of ak_hydro_stage: 0 = tiled plane-marching kernel (default),
- * 1 = straightforward one-thread-per-cell kernel kept as a cross-check.  Both give the same
- * results to rounding. */
+/* Selects the implementation of ak_hydro_stage (all of them CUDA kernels of this library; they give the
+ * same results to rounding and exist as independent cross-checks for the tests):
+ *   0 = production kernel: TMA-staged plane marching, worker threads + edge warp (default)
+ *   1 = one thread per cell, recomputes everything        2 = tiled plane marching, LDG staging
+ *   3 = first TMA-staged kernel                            4 = second generation (edge faces on warp 0)
+ * AK_EINVAL for any other value. */
 int ak_pack_set_variant(ak_pack*, int variant);
+
+/* Tile shape of the production kernel (variant 0): -1 = chosen from the block size (default);
+ * 0 = 16x10 columns, 2 CTAs per SM; 1 = 16x8, 2 CTAs per SM; 2 = 16x22 and 3 = 32x11, 1 CTA per SM.
+ * Results are bit-identical for every tile shape (tile-edge faces are solved with the same instruction
+ * sequence by both tiles that share them).  AK_EINVAL for any other value. */
+int ak_pack_set_tile(ak_pack*, int tile);
 
 /* Number of kernel launches issued through this pack since bind (for bench.py's gpu_launches). */
 long long ak_pack_launch_count(const ak_pack*);

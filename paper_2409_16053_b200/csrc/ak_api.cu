@@ -177,6 +177,13 @@ extern "C" int ak_pack_set_variant(ak_pack* p, int variant) {
   return AK_OK;
 }
 
+extern "C" int ak_pack_set_tile(ak_pack* p, int tile) {
+  if (!p) return fail(AK_EINVAL, "null pack");
+  if (tile < -1 || tile > 3) return fail(AK_EINVAL, "unknown tile shape");
+  p->tile = tile;
+  return AK_OK;
+}
+
 extern "C" int ak_fill_ghosts(ak_pack* p) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
   AK_CUDA(ak::launch_fill_ghosts(*p, p->u[p->cur]), "ak_fill_ghosts launch");

@@ -49,6 +49,7 @@ struct ak_pack {
   cudaStream_t stream = nullptr;
   int cur = 0;
   int variant = 0;
+  int tile = -1;                  // -1 = automatic (ak_pack_set_tile)
   long long launches = 0;
   int sm_count = 148;
   // tensor maps over u[0], u[1] for the TMA stage kernel, rebuilt when the staging box changes

@@ -16,9 +16,6 @@ namespace ak {
 
 // tile shape of the production kernel: 0 = 16x12 (2 CTAs/SM), 1 = 16x8 (3 CTAs/SM), 2 = 32x6 (2 CTAs/SM)
 static int pick_tile(const ak_pack& p) {
-  static int forced = -2;
-  if (forced == -2) { const char* e = std::getenv("AK_TILE"); forced = e ? std::atoi(e) : -1; }
-  if (forced >= 0) return forced;
   return (p.d.nx[1] % 12 == 0 || p.d.nx[1] >= 48) ? 0 : 1;
 }
 
@@ -36,9 +33,7 @@ static cudaError_t launch_stage_v2(const ak_pack& p, const double* Uin, const do
 // tile shape of the v3 kernel (workers + one edge warp): the one that wastes the fewest lanes on the ragged
 // last tile row and on the edge warp.  0 = 16x10 (6 warps), 1 = 16x8 (5 warps)
 static int pick_tile_v3(const ak_pack& p) {
-  static int forced = -2;
-  if (forced == -2) { const char* e = std::getenv("AK_TILE"); forced = e ? std::atoi(e) : -1; }
-  if (forced >= 0) return forced;
+  if (p.tile >= 0) return p.tile;
   const int n = p.d.nx[1];
   const double e10 = (double)n / (((n + 9) / 10) * 10) * (160.0 / 192.0);
   const double e8 = (double)n / (((n + 7) / 8) * 8) * (128.0 / 160.0);
@@ -53,7 +48,6 @@ static cudaError_t launch_stage_v3(const ak_pack& p, const double* Uin, const do
     case 1:  return launch_v3<RECON, 16, 8, 2>(p, Uin, U0, Uout, sc, stage2);
     case 2:  return launch_v3<RECON, 16, 22, 1>(p, Uin, U0, Uout, sc, stage2);
     case 3:  return launch_v3<RECON, 32, 11, 1>(p, Uin, U0, Uout, sc, stage2);
-    case 4:  return launch_v3<RECON, 16, 10, 1>(p, Uin, U0, Uout, sc, stage2);
     default: return launch_v3<RECON, 16, 10, 2>(p, Uin, U0, Uout, sc, stage2);
   }
 }

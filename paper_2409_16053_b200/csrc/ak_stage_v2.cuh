@@ -30,10 +30,6 @@
 #include "ak_lean.cuh"
 #include "ak_tma.cuh"
 
-#ifndef AK_EXP
-#define AK_EXP 0
-#endif
-#define AK_SYNC() do { if (!(AK_EXP & 2)) __syncthreads(); } while (0)
 namespace ak {
 
 template <int RECON>
@@ -131,7 +127,7 @@ stage_v2_kernel(const __grid_constant__ CUtensorMap tmU, PackDev P, const double
   }
   // tile-edge faces: thread e < wJ solves the upper x1 face of row e, thread wJ <= e < wJ+wI the upper x2 face
   // of column e-wJ; both kinds share one instruction stream (stride / offsets differ)
-  const bool extra = (AK_EXP & 1) ? false : (tid < wI + wJ);
+  const bool extra = tid < wI + wJ;
   const bool ex2 = tid >= wJ;
   int eA = 0, eB = 0, eSt = 1, eQlo = 0, eQhi = 0, eQn = 0;
   if (extra) {
@@ -272,7 +268,7 @@ stage_v2_kernel(const __grid_constant__ CUtensorMap tmU, PackDev P, const double
         }
       }
     }
-    AK_SYNC();                                    // q+ visible; every read of W(s) is done
+    __syncthreads();                                    // q+ visible; every read of W(s) is done
     if (tid == 0 && s + 2 < send) {                     // refill slot b with plane s+2
       fence_proxy_async();
       mbar_expect_tx(&bars[b], S::tx_bytes);
@@ -307,7 +303,7 @@ stage_v2_kernel(const __grid_constant__ CUtensorMap tmU, PackDev P, const double
       tslot = (dslot + 1 == NS) ? 0 : dslot + 1;
       phaseL(s + 1, it + 1);
     }
-    AK_SYNC();                                    // fluxes of plane s visible
+    __syncthreads();                                    // fluxes of plane s visible
     // ---- D(s) --------------------------------------------------------------------------------------
     if (inplane && valid) {
       double* Td = sm + S::oT + dslot * (5 * NT) + tid;

@@ -27,7 +27,6 @@
 #include "ak_lean.cuh"
 #include "ak_tma.cuh"
 #include "ak_stage_v2.cuh"     // recon2<>
-#include <cstdlib>
 
 namespace ak {
 
@@ -348,9 +347,7 @@ cudaError_t launch_v3(const ak_pack& p, const double* Uin, const double* U0, dou
   }
   const CUtensorMap& tm = (Uin == p.u[0]) ? p.tmap[0] : p.tmap[1];
   const CUtensorMap& tm0 = (U0 == p.u[0]) ? p.tmap0[0] : p.tmap0[1];
-  static int pad = -1;
-  if (pad < 0) { const char* e = getenv("AK_SMEM_PAD"); pad = e ? atoi(e) : 0; }
-  const size_t smem = S::bytes + pad;
+  const size_t smem = S::bytes;
   auto k1 = stage_v3_kernel<RECON, TI, TJ, MINB, false>;
   auto k2 = stage_v3_kernel<RECON, TI, TJ, MINB, true>;
   static bool attr_set = false;
