@@ -276,3 +276,72 @@ def test_older_kernel_generations_still_match_the_oracle(orc, ak, variant):
     for w in (I.config3(nrb=2, nx=32), I.config1(nrb=2, nx=32)):
         errs, *_ = run_lockstep(orc, ak, w, 2, variant, check_ghosts=False)
         assert max(errs) <= TOL_RUN, (variant, w.name, errs)
+
+
+# ------------------------------------------------------- config 3 at full size, bench launch configuration --------
+def _assemble(mesh, U):
+    """(nmb, 5, nt3, nt2, nt1) block state -> (5, N3, N2, N1) global array of active cells (uniform mesh), on U's device."""
+    g, nx = mesh.ng, mesh.nx
+    G = torch.empty((5, mesh.nrb[2] * nx[2], mesh.nrb[1] * nx[1], mesh.nrb[0] * nx[0]), dtype=U.dtype, device=U.device)
+    for m, (_, l1, l2, l3) in enumerate(mesh.blocks):
+        G[:, l3 * nx[2]:(l3 + 1) * nx[2], l2 * nx[1]:(l2 + 1) * nx[1], l1 * nx[0]:(l1 + 1) * nx[0]] = \
+            U[m][:, g:-g, g:-g, g:-g]
+    return G
+
+
+def _subbox(G, origin, n):
+    """n^3 periodic sub-box of the global array with lower corner `origin` = (o1, o2, o3) -> host numpy (5, n, n, n)."""
+    idx = [(torch.arange(n, device=G.device) + o) % G.shape[3 - d] for d, o in enumerate(origin)]
+    return G.index_select(1, idx[2]).index_select(2, idx[1]).index_select(3, idx[0]).cpu().numpy()
+
+
+def test_config3_full_size_sampled(orc, ak):
+    """BASELINE config 3 at its full size (64 MeshBlocks of 128^3, the launch configuration bench.py times):
+    one RK2 step on the GPU, checked on sampled 32^3 sub-boxes that the oracle advances one by one.  A cell's RK2
+    update depends on cells within 2 x 3 of it (two PPM4 stages), so the oracle, run on a sub-box as its own small
+    periodic block with the same dx and dt, is exact on the cells >= 6 away from the sub-box faces.  The boxes
+    sit on a corner where 8 blocks meet, on the periodic wrap of the domain, on the shear layers and inside a
+    block (every box spans several 16 x 10 tiles).  Plus what holds at any size: conservation and no floors."""
+    w = I.config3()
+    dev = torch.device("cuda", 0)
+    pg = ak.Pack(w.mesh, w.gamma, w.recon, device=dev)
+    U0 = w.state(device=dev)
+    pg.load(U0)
+    G0 = _assemble(w.mesh, U0)
+    del U0
+    n, pad = 32, 8
+    origins = [(112, 112, 112), (496, 496, 496), (300, 112, 200), (40, 368, 500), (200, 50, 60), (240, 250, 260)]
+    subs0 = [_subbox(G0, o, n) for o in origins]
+    tot0 = G0.sum(dim=(1, 2, 3)).cpu().numpy()
+    rho, mom, E = G0[0], G0[1:4], G0[4]
+    p = (w.gamma - 1.0) * (E - 0.5 * (mom ** 2).sum(0) / rho)
+    cs = torch.sqrt(w.gamma * p / rho)
+    dx = w.mesh.dx(0)
+    dt_ref = w.cfl * min(float((dx[d] / (mom[d].abs() / rho + cs)).min()) for d in range(3))
+    mnorm = float((mom.norm(dim=0) + rho * cs).sum())
+    del G0, rho, mom, E, p, cs
+    dt = pg.new_dt(w.cfl)
+    assert abs(dt - dt_ref) <= 1e-13 * dt_ref
+    pg.step(w.cfl, dt)
+    assert pg.floor_count() == 0
+    G1 = _assemble(w.mesh, pg.current())
+    tot1 = G1.sum(dim=(1, 2, 3)).cpu().numpy()
+    scale = np.array([tot0[0], mnorm, mnorm, mnorm, tot0[4]])
+    assert (np.abs(tot1 - tot0) / scale).max() <= TOL_TOTALS
+    sub_mesh = I.Mesh((1, 1, 1), (n, n, n), w.mesh.ng, [(0, 0, 0, 0)], xmax=(n * dx[0], n * dx[1], n * dx[2]))
+    assert sub_mesh.dx(0) == dx
+    g = w.mesh.ng
+    worst = 0.0
+    for o, s0 in zip(origins, subs0):
+        po = orc.OrcPack(sub_mesh, w.gamma, w.recon, threads=1)
+        u = np.zeros(sub_mesh.state_shape())
+        u[0][:, g:-g, g:-g, g:-g] = s0
+        po.load(u)
+        po.step(w.cfl, dt)
+        ref = po.current()[0][:, g + pad:-g - pad, g + pad:-g - pad, g + pad:-g - pad]
+        got = _subbox(G1, o, n)[:, pad:-pad, pad:-pad, pad:-pad]
+        e = P.q14(got[None], ref[None], w.gamma)
+        worst = max(worst, e)
+        assert e <= 2 * TOL_STAGE, (o, e)
+        po.close()
+    print(f"cfg3 full size: worst sampled Q14 after one RK2 step = {worst:.2e}")
