@@ -129,6 +129,7 @@ struct orc_pack {
   int cur = 0;
   long long floor_count = 0;
   int nthreads = 1;
+  bool flux_correction = false;          // SURVEY 8(f) f1, off by default (north_star's stage list omits it)
 
   size_t ncell() const { return (size_t)nt[0] * nt[1] * nt[2]; }
   size_t idx(int m, int n, int k, int j, int i) const {
@@ -206,6 +207,7 @@ extern "C" int orc_pack_bind(orc_pack* p, double* u_a, double* u_b) {
 }
 
 extern "C" int orc_set_threads(orc_pack* p, int n) { if (!p || n < 1) return fail("bad thread count"); p->nthreads = n; return 0; }
+extern "C" int orc_set_flux_correction(orc_pack* p, int on) { if (!p) return fail("null pack"); p->flux_correction = on != 0; return 0; }
 extern "C" double* orc_pack_current(orc_pack* p) { return (p && p->bound) ? p->u[p->cur] : nullptr; }
 extern "C" long long orc_pack_floor_count(const orc_pack* p) { return p ? p->floor_count : -1; }
 extern "C" int orc_pack_destroy(orc_pack* p) { delete p; return 0; }
@@ -302,8 +304,15 @@ extern "C" int orc_fill_ghosts(orc_pack* p) {
 // ------------------------------------------------------------------------------------------------
 // S1-S4  one Runge-Kutta stage (P:99 reconstruct-solve-advance; P:105 SSP-RK2 in two registers)
 // ------------------------------------------------------------------------------------------------
-static long long stage_block(const orc_pack* p, const double* Uin, const double* U0, double* Uout, int m,
-                             double g0, double g1, double beta, double dt) {
+// F[d][n*ncell + c]: flux of direction d at the LOWER d-face of cell c
+struct FaceFlux {
+  std::vector<double> v[3];
+  std::vector<double>& operator[](int d) { return v[d]; }
+  const std::vector<double>& operator[](int d) const { return v[d]; }
+};
+
+// S1-S3 for block m: primitives, reconstruction and the Riemann flux at every face of the active region
+static long long block_fluxes(const orc_pack* p, const double* Uin, int m, FaceFlux& F) {
   const int ng = p->ng, n1 = p->nt[0], n2 = p->nt[1], n3 = p->nt[2];
   const size_t nc = p->ncell();
   long long nfl = 0;
@@ -318,7 +327,6 @@ static long long stage_block(const orc_pack* p, const double* Uin, const double*
     for (int n = 0; n < 5; n++) W[n * nc + c] = w[n];
   }
   // S2 + S3: flux of direction d at the lower face of cell (k,j,i), stored at that cell's index
-  std::vector<double> F[3];
   const int str[3] = { 1, n1, n1 * n2 };
   for (int d = 0; d < 3; d++) {
     F[d].assign(5 * nc, 0.0);
@@ -345,7 +353,15 @@ static long long stage_block(const orc_pack* p, const double* Uin, const double*
       for (int n = 0; n < 5; n++) F[d][n * nc + c] = Fl[n];
     }
   }
-  // S4: weighted update of the active cells, evaluated left to right
+  return nfl;
+}
+
+// S4 for block m: weighted update of the active cells, evaluated left to right
+static void block_update(const orc_pack* p, const double* Uin, const double* U0, double* Uout, int m, const FaceFlux& F,
+                         double g0, double g1, double beta, double dt) {
+  const int ng = p->ng, n1 = p->nt[0], n2 = p->nt[1];
+  const size_t nc = p->ncell();
+  const int str[3] = { 1, n1, n1 * n2 };
   const int lev = p->level[m];
   const double c1 = beta * dt / p->dx(lev, 0), c2 = beta * dt / p->dx(lev, 1), c3 = beta * dt / p->dx(lev, 2);
   for (int n = 0; n < 5; n++)
@@ -358,7 +374,51 @@ static long long stage_block(const orc_pack* p, const double* Uin, const double*
       v = v - c3 * (F[2][n * nc + c + str[2]] - F[2][n * nc + c]);
       Uout[g] = v;
     }
-  return nfl;
+}
+
+// f1 ("flux correction"): at a face between a level-0 block and level-1 blocks the coarse
+// block's flux is replaced by the mean of the four fine-block fluxes through the same area (equal areas),
+// summed in a fixed order, so that what leaves the fine cells is exactly what enters the coarse cell.
+static void correct_coarse_fluxes(const orc_pack* p, std::vector<FaceFlux>& F) {
+  const int ng = p->ng;
+  const size_t nc = p->ncell();
+  const int n1 = p->nt[0], n2 = p->nt[1];
+  for (int m = 0; m < p->nmb; m++) {
+    if (p->level[m] != 0) continue;
+    for (int d = 0; d < 3; d++) for (int side = 0; side < 2; side++) {
+      long nb[3] = { p->lx[3 * (size_t)m], p->lx[3 * (size_t)m + 1], p->lx[3 * (size_t)m + 2] };
+      nb[d] = wrapl(nb[d] + (side ? 1 : -1), p->nrb[d]);
+      if (p->find_leaf(0, nb[0], nb[1], nb[2]) >= 0) continue;           // same-level neighbour: nothing to do
+      const int t1 = (d == 0) ? 1 : 0, t2 = (d == 2) ? 1 : 2;             // tangential directions, t1 faster
+      for (int b = 0; b < p->nx[t2]; b++) for (int a = 0; a < p->nx[t1]; a++) {
+        int cc[3];                                                        // coarse cell on the + side of the face
+        cc[d] = side ? p->nx[d] + ng : ng; cc[t1] = a + ng; cc[t2] = b + ng;
+        const size_t c = ((size_t)cc[2] * n2 + cc[1]) * n1 + cc[0];
+        // level-1 global index of the fine cell that stores the fine face: the cell on the + side of the face
+        long Gc[3];
+        for (int e = 0; e < 3; e++) Gc[e] = (long)p->lx[3 * (size_t)m + e] * p->nx[e] + (cc[e] - ng);
+        double f[2][2][5];
+        for (int s2 = 0; s2 < 2; s2++) for (int s1 = 0; s1 < 2; s1++) {
+          long Gf[3];
+          Gf[d] = 2 * Gc[d]; Gf[t1] = 2 * Gc[t1] + s1; Gf[t2] = 2 * Gc[t2] + s2;
+          // upper coarse face: the fine cell on the + side is active in the fine neighbour (its lower boundary
+          // face); lower coarse face: the fine face is the UPPER boundary face of the fine neighbour on the - side,
+          // stored at that block's first upper ghost index
+          long Gown[3] = { Gf[0], Gf[1], Gf[2] };
+          if (!side) Gown[d] = Gf[d] - 1;                                 // an active cell of the fine neighbour
+          for (int e = 0; e < 3; e++) Gown[e] = wrapl(Gown[e], p->nglob(1, e));
+          const int mf = p->find_leaf(1, Gown[0] / p->nx[0], Gown[1] / p->nx[1], Gown[2] / p->nx[2]);
+          int cf[3];
+          for (int e = 0; e < 3; e++) cf[e] = (int)(Gown[e] - (long)p->lx[3 * (size_t)mf + e] * p->nx[e]) + ng;
+          if (!side) cf[d] += 1;                                          // = nx[d] + ng
+          const size_t cfi = ((size_t)cf[2] * n2 + cf[1]) * n1 + cf[0];
+          for (int n = 0; n < 5; n++) f[s2][s1][n] = F[mf][d][n * nc + cfi];
+        }
+        for (int n = 0; n < 5; n++)
+          F[m][d][n * nc + c] = 0.25 * ((f[0][0][n] + f[0][1][n]) + (f[1][0][n] + f[1][1][n]));
+      }
+    }
+  }
 }
 
 extern "C" int orc_hydro_stage(orc_pack* p, int stage, double dt) {
@@ -372,8 +432,22 @@ extern "C" int orc_hydro_stage(orc_pack* p, int stage, double dt) {
   const double* U0 = p->u[0];
   double* Uout = p->u[1 - p->cur];          // stage 2 writes A in place: each cell's A value is read only for itself
   long long nfl = 0;
+  if (p->flux_correction && p->max_level > 0) {
+    // all fluxes first, then the coarse faces at level boundaries are replaced, then every block is advanced
+    std::vector<FaceFlux> F(p->nmb);
 #pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) reduction(+ : nfl) if (p->nthreads > 1)
-  for (int m = 0; m < p->nmb; m++) nfl += stage_block(p, Uin, U0, Uout, m, g0, g1, beta, dt);
+    for (int m = 0; m < p->nmb; m++) nfl += block_fluxes(p, Uin, m, F[m]);
+    correct_coarse_fluxes(p, F);
+#pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) if (p->nthreads > 1)
+    for (int m = 0; m < p->nmb; m++) block_update(p, Uin, U0, Uout, m, F[m], g0, g1, beta, dt);
+  } else {
+#pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) reduction(+ : nfl) if (p->nthreads > 1)
+    for (int m = 0; m < p->nmb; m++) {
+      FaceFlux F;
+      nfl += block_fluxes(p, Uin, m, F);
+      block_update(p, Uin, U0, Uout, m, F, g0, g1, beta, dt);
+    }
+  }
   p->floor_count += nfl;
   p->cur = 1 - p->cur;
   return 0;

@@ -41,6 +41,8 @@ int orc_pack_set_block(orc_pack*, int m, int level, int lx1, int lx2, int lx3);
 /* u_a holds U^n on entry; u_b is the second register.  Validates that the leaves tile the domain. */
 int orc_pack_bind(orc_pack*, double* u_a, double* u_b);
 int orc_set_threads(orc_pack*, int nthreads);
+/* f1: replace the coarse flux at level-boundary faces by the mean of the four fine fluxes.  Off by default. */
+int orc_set_flux_correction(orc_pack*, int on);
 int orc_fill_ghosts(orc_pack*);                           /* G1-G4 on the current buffer           */
 int orc_hydro_stage(orc_pack*, int stage, double dt);     /* S1-S4; stage 1: A->B, stage 2: B,A->A */
 int orc_new_dt(orc_pack*, double cfl, double* dt_out);    /* S0 on the current buffer              */

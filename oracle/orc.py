@@ -39,6 +39,7 @@ def lib():
     L.orc_pack_set_block.argtypes = [C.c_void_p] + [C.c_int] * 5
     L.orc_pack_bind.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     L.orc_set_threads.argtypes = [C.c_void_p, C.c_int]
+    L.orc_set_flux_correction.argtypes = [C.c_void_p, C.c_int]
     L.orc_fill_ghosts.argtypes = [C.c_void_p]
     L.orc_hydro_stage.argtypes = [C.c_void_p, C.c_int, C.c_double]
     L.orc_new_dt.argtypes = [C.c_void_p, C.c_double, dp]
@@ -126,6 +127,10 @@ class OrcPack:
         _chk(L.orc_pack_bind(self._h, self.ua.ctypes.data, self.ub.ctypes.data))
         if threads != 1:
             _chk(L.orc_set_threads(self._h, threads))
+
+    def set_flux_correction(self, on=True):
+        """f1 of SURVEY 8(f): coarse fluxes at level-boundary faces <- mean of the four fine fluxes (off by default)."""
+        _chk(lib().orc_set_flux_correction(self._h, 1 if on else 0))
 
     def load(self, U):
         """Copy U^n (numpy or CPU torch tensor of the state shape) into buffer A and make it current."""
