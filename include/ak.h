@@ -122,6 +122,13 @@ long long ak_pack_floor_count(ak_pack*);
  * AK_EINVAL for any other value. */
 int ak_pack_set_variant(ak_pack*, int variant);
 
+/* Flux correction at coarse-fine faces (paper P:57).  on != 0: after every ak_hydro_stage on a
+ * refined mesh, the flux a level-0 cell used at a face shared with level-1 blocks is replaced by the mean of the
+ * four fine fluxes through that face (three small extra launches per stage), which makes the update
+ * conservative across level boundaries.  Off by default (north_star's stage list omits it); no effect on
+ * single-level meshes. */
+int ak_pack_set_flux_correction(ak_pack*, int on);
+
 /* Tile shape of the production kernel (variant 0): -1 = chosen from the block size (default);
  * 0 = 16x10 columns, 2 CTAs per SM; 1 = 16x8, 2 CTAs per SM; 2 = 16x22 and 3 = 32x11, 1 CTA per SM.
  * Results are bit-identical for every tile shape (tile-edge faces are solved with the same instruction

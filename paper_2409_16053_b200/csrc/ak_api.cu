@@ -177,6 +177,12 @@ extern "C" int ak_pack_set_variant(ak_pack* p, int variant) {
   return AK_OK;
 }
 
+extern "C" int ak_pack_set_flux_correction(ak_pack* p, int on) {
+  if (!p) return fail(AK_EINVAL, "null pack");
+  p->flux_correction = on != 0;
+  return AK_OK;
+}
+
 extern "C" int ak_pack_set_tile(ak_pack* p, int tile) {
   if (!p) return fail(AK_EINVAL, "null pack");
   if (tile < -1 || tile > 3) return fail(AK_EINVAL, "unknown tile shape");
@@ -211,6 +217,10 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
     }
   AK_CUDA(ak::launch_stage(*p, p->u[p->cur], p->u[0], p->u[1 - p->cur], sc), "ak_hydro_stage launch");
   p->launches += ak::stage_launches_per_call(*p);
+  if (p->flux_correction && p->d.max_level > 0) {
+    AK_CUDA(ak::launch_flux_correction(*p, p->u[p->cur], p->u[1 - p->cur], sc), "flux correction launch");
+    p->launches += 3;
+  }
   p->cur = 1 - p->cur;
   p->ghosts_ok = false;
   return AK_OK;

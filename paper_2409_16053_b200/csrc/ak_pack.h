@@ -49,6 +49,7 @@ struct ak_pack {
   cudaStream_t stream = nullptr;
   int cur = 0;
   int variant = 0;
+  bool flux_correction = false;   // ak_pack_set_flux_correction
   int tile = -1;                  // -1 = automatic (ak_pack_set_tile)
   long long launches = 0;
   int sm_count = 148;
@@ -67,4 +68,6 @@ cudaError_t launch_new_dt(const ak_pack& p, const double* U);       // leaves th
 cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, double* Uout,
                          const StageCoef& sc);
 int stage_launches_per_call(const ak_pack& p);
+// refined meshes, optional: three launches (one per direction) after launch_stage
+cudaError_t launch_flux_correction(const ak_pack& p, const double* Uin, double* Uout, const StageCoef& sc);
 }  // namespace ak

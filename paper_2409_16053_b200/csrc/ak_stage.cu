@@ -9,6 +9,7 @@
 #include "ak_stage_tma.cuh"
 #include "ak_stage_v2.cuh"
 #include "ak_stage_v3.cuh"
+#include "ak_fluxcorr.cuh"
 
 #include <cstdlib>
 
@@ -61,6 +62,10 @@ cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, 
   if (p.variant == 3) return launch_stage_tma(p, Uin, U0, Uout, sc);
   if (p.variant == 4) return p.recon == 0 ? launch_stage_v2<0>(p, Uin, U0, Uout, sc) : launch_stage_v2<1>(p, Uin, U0, Uout, sc);
   return p.recon == 0 ? launch_stage_v3<0>(p, Uin, U0, Uout, sc) : launch_stage_v3<1>(p, Uin, U0, Uout, sc);
+}
+
+cudaError_t launch_flux_correction(const ak_pack& p, const double* Uin, double* Uout, const StageCoef& sc) {
+  return p.recon == 0 ? launch_flux_correction_t<0>(p, Uin, Uout, sc) : launch_flux_correction_t<1>(p, Uin, Uout, sc);
 }
 
 int stage_launches_per_call(const ak_pack&) { return 1; }
