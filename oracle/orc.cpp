@@ -112,6 +112,56 @@ extern "C" void orc_hllc(double gamma, int dir, const double WL[5], const double
 }
 
 // ------------------------------------------------------------------------------------------------
+// S3'  the other two-state solvers of the paper's option list ("LLF ... HLLE, HLLC ...").
+// Textbook forms (Toro 2013 ch.10), restated because the paper defers them:
+//   LLF (Rusanov): F = 1/2 [(F_L + F_R) - a (U_R - U_L)],  a = max(|u_L| + c_L, |u_R| + c_R)
+//   HLLE: F = [b+ F_L - b- F_R + b+ b- (U_R - U_L)] / (b+ - b-),  b- = min(S_L, 0), b+ = max(S_R, 0),
+//         Einfeldt's speeds S_L = min(u_L - c_L, u~ - c~), S_R = max(u_R + c_R, u~ + c~) from the Roe averages
+//         (weights sqrt(rho)):  u~, v~, w~, H~ = (E + p)/rho averaged,  c~^2 = (gamma - 1)(H~ - 1/2 |v~|^2)
+// ------------------------------------------------------------------------------------------------
+static void rotated_states(double gamma, int dir, const double W[5], double U[5], double Fx[5], double* c) {
+  const int iu = 1 + dir, iv = 1 + (dir + 1) % 3, iw = 1 + (dir + 2) % 3;
+  const double r = W[0], u = W[iu], v = W[iv], w = W[iw], e = W[4];
+  const double p = (gamma - 1.0) * e;
+  const double E = e + 0.5 * r * (u * u + (v * v + w * w));
+  U[0] = r; U[1] = r * u; U[2] = r * v; U[3] = r * w; U[4] = E;
+  Fx[0] = r * u; Fx[1] = r * u * u + p; Fx[2] = r * u * v; Fx[3] = r * u * w; Fx[4] = (E + p) * u;
+  *c = std::sqrt(gamma * p / r);
+}
+static void unrotate(int dir, const double Fn[5], double F[5]) {
+  const int iu = 1 + dir, iv = 1 + (dir + 1) % 3, iw = 1 + (dir + 2) % 3;
+  F[0] = Fn[0]; F[iu] = Fn[1]; F[iv] = Fn[2]; F[iw] = Fn[3]; F[4] = Fn[4];
+}
+
+extern "C" void orc_llf(double gamma, int dir, const double WL[5], const double WR[5], double F[5]) {
+  double UL[5], UR[5], FL[5], FR[5], cL, cR, Fn[5];
+  rotated_states(gamma, dir, WL, UL, FL, &cL);
+  rotated_states(gamma, dir, WR, UR, FR, &cR);
+  const double a = std::fmax(std::fabs(WL[1 + dir]) + cL, std::fabs(WR[1 + dir]) + cR);
+  for (int n = 0; n < 5; n++) Fn[n] = 0.5 * ((FL[n] + FR[n]) - a * (UR[n] - UL[n]));
+  unrotate(dir, Fn, F);
+}
+
+extern "C" void orc_hlle(double gamma, int dir, const double WL[5], const double WR[5], double F[5]) {
+  double UL[5], UR[5], FL[5], FR[5], cL, cR, Fn[5];
+  rotated_states(gamma, dir, WL, UL, FL, &cL);
+  rotated_states(gamma, dir, WR, UR, FR, &cR);
+  const double gm1 = gamma - 1.0;
+  const double sL = std::sqrt(WL[0]), sR = std::sqrt(WR[0]), isum = 1.0 / (sL + sR);
+  // Roe averages; velocities from the rotated conserved states, enthalpy H = (E + p) / rho
+  const double uL = UL[1] / UL[0], vL = UL[2] / UL[0], wL = UL[3] / UL[0];
+  const double uR = UR[1] / UR[0], vR = UR[2] / UR[0], wR = UR[3] / UR[0];
+  const double HL = (UL[4] + gm1 * WL[4]) / UL[0], HR = (UR[4] + gm1 * WR[4]) / UR[0];
+  const double ut = (sL * uL + sR * uR) * isum, vt = (sL * vL + sR * vR) * isum, wt = (sL * wL + sR * wR) * isum;
+  const double Ht = (sL * HL + sR * HR) * isum;
+  const double ct = std::sqrt(gm1 * (Ht - 0.5 * (ut * ut + (vt * vt + wt * wt))));
+  const double SL = std::fmin(uL - cL, ut - ct), SR = std::fmax(uR + cR, ut + ct);
+  const double bm = std::fmin(SL, 0.0), bp = std::fmax(SR, 0.0);
+  for (int n = 0; n < 5; n++) Fn[n] = ((bp * FL[n] - bm * FR[n]) + bp * bm * (UR[n] - UL[n])) / (bp - bm);
+  unrotate(dir, Fn, F);
+}
+
+// ------------------------------------------------------------------------------------------------
 // Pack descriptor
 // ------------------------------------------------------------------------------------------------
 struct orc_pack {
@@ -149,7 +199,7 @@ extern "C" orc_pack* orc_pack_create(int nmb, int nx1, int nx2, int nx3, int ng,
   for (int d = 0; d < 3; d++) if (nx[d] < ng || (nx[d] & 1)) { fail("nx_d must be even and >= ng"); return nullptr; }
   if (!(gamma > 1.0)) { fail("gamma <= 1"); return nullptr; }
   if (recon != 0 && recon != 1) { fail("unknown recon"); return nullptr; }
-  if (rsolver != 0) { fail("unknown rsolver"); return nullptr; }
+  if (rsolver < 0 || rsolver > 2) { fail("unknown rsolver"); return nullptr; }
   if ((recon == 0 && ng < 2) || (recon == 1 && ng < 3)) { fail("ng too small for the reconstruction"); return nullptr; }
   orc_pack* p = new orc_pack;
   p->nmb = nmb; p->ng = ng; p->gamma = gamma; p->recon = recon; p->rsolver = rsolver;
@@ -349,7 +399,9 @@ static long long block_fluxes(const orc_pack* p, const double* Uin, int m, FaceF
           orc_ppm4(sR, &qm, &qp);                                             WR[n] = qm;
         }
       }
-      orc_hllc(p->gamma, d, WL, WR, Fl);
+      if (p->rsolver == 0) orc_hllc(p->gamma, d, WL, WR, Fl);
+      else if (p->rsolver == 1) orc_llf(p->gamma, d, WL, WR, Fl);
+      else orc_hlle(p->gamma, d, WL, WR, Fl);
       for (int n = 0; n < 5; n++) F[d][n * nc + c] = Fl[n];
     }
   }

@@ -59,6 +59,9 @@ def lib():
     L.orc_ppm4_iface.restype = None
     L.orc_hllc.argtypes = [C.c_double, C.c_int, dp, dp, dp]
     L.orc_hllc.restype = None
+    for f in (L.orc_llf, L.orc_hlle):
+        f.argtypes = [C.c_double, C.c_int, dp, dp, dp]
+        f.restype = None
     _lib = L
     return L
 
@@ -105,6 +108,18 @@ def ppm4_iface(qm1, q0, qp1, qp2):
 def hllc(gamma, direction, WL, WR):
     F = (C.c_double * 5)()
     lib().orc_hllc(gamma, direction, _arr5(WL), _arr5(WR), F)
+    return np.array(F[:])
+
+
+def llf(gamma, direction, WL, WR):
+    F = (C.c_double * 5)()
+    lib().orc_llf(gamma, direction, _arr5(WL), _arr5(WR), F)
+    return np.array(F[:])
+
+
+def hlle(gamma, direction, WL, WR):
+    F = (C.c_double * 5)()
+    lib().orc_hlle(gamma, direction, _arr5(WL), _arr5(WR), F)
     return np.array(F[:])
 
 

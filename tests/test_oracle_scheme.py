@@ -25,8 +25,8 @@ def act(mesh):
     return (slice(None), slice(None), slice(g, -g), slice(g, -g), slice(g, -g))
 
 
-def run(orc, mesh, U0, recon, gamma=I.GAMMA, cfl=0.3, nsteps=None, tend=None):
-    p = orc.OrcPack(mesh, gamma, recon)
+def run(orc, mesh, U0, recon, gamma=I.GAMMA, cfl=0.3, nsteps=None, tend=None, rsolver=0):
+    p = orc.OrcPack(mesh, gamma, recon, rsolver=rsolver)
     p.load(U0)
     t, n = 0.0, 0
     while True:
@@ -97,7 +97,7 @@ def test_exact_riemann_fixture_is_reproduced_by_independent_solver(key, g):
         assert d[k] == pytest.approx(ref[k], rel=1e-11)
 
 
-def sod_run(orc, N, recon, ng, direction=0):
+def sod_run(orc, N, recon, ng, direction=0, rsolver=0):
     """Periodic line with two mirrored Sod problems: left state on [0.25,0.75)."""
     g = 1.4
     nx = [4, 4, 4]
@@ -113,7 +113,7 @@ def sod_run(orc, N, recon, ng, direction=0):
         return (rho, z, z, z, P)
 
     U0 = I.make_state(mesh, prim, gamma=g).numpy()
-    U = run(orc, mesh, U0, recon, gamma=g, cfl=0.3, tend=0.1)
+    U = run(orc, mesh, U0, recon, gamma=g, cfl=0.3, tend=0.1, rsolver=rsolver)
     a = [ng, ng, ng]
     sl = [0, slice(None), ng, ng, ng]
     sl[4 - direction] = slice(ng, -ng)
