@@ -162,7 +162,8 @@ def run_ours(args):
 
     w = workloads()[args.workload]()
     mesh = w.mesh
-    pack = ak.Pack(mesh, w.gamma, w.recon, device=dev, variant=args.variant)
+    pack = ak.Pack(mesh, w.gamma, w.recon, rsolver={"hllc": 0, "llf": 1, "hlle": 2}[args.rsolver], device=dev,
+                   variant=args.variant)
     if args.flux_correction:
         pack.set_flux_correction(True)
     U0 = w.state(device=dev)
@@ -255,7 +256,7 @@ def run_ours(args):
             "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{args.workload}: {w.name}", "nmb": mesh.nmb, "nx": list(mesh.nx), "ng": mesh.ng,
-                       "recon": "PPM4" if w.recon else "PLM", "rsolver": "HLLC", "integrator": "SSPRK2", "cfl": w.cfl,
+                       "recon": "PPM4" if w.recon else "PLM", "rsolver": args.rsolver.upper(), "integrator": "SSPRK2", "cfl": w.cfl,
                        "cells": ncell, "state_bytes": state_bytes, "l2_policy": "inputs larger than L2 (no flush needed)"
                        if state_bytes > 4e8 else "state fits L2: numbers are L2-resident", "variant": args.variant, "flux_correction": bool(args.flux_correction),
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
@@ -277,6 +278,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--rsolver", default="hllc", choices=["hllc", "llf", "hlle"],
+                    help="Riemann solver (headline metric: hllc; llf / hlle are the f2 variants on the same kernel)")
     ap.add_argument("--flux-correction", action="store_true",
                     help="refined meshes (cfg4): flux correction at coarse-fine faces on (SURVEY 8(f) f1; off by default)")
     ap.add_argument("--traffic", type=float, default=None,

@@ -42,7 +42,7 @@ extern "C" ak_pack* ak_pack_create(int nmb, int nx1, int nx2, int nx3, int ng, d
     if (nx[d] < ng || (nx[d] & 1) || nx[d] < 2) { fail(AK_EINVAL, "nx_d must be even and >= ng"); return nullptr; }
   if (!(gamma > 1.0)) { fail(AK_EINVAL, "gamma <= 1"); return nullptr; }
   if (recon != AK_RECON_PLM && recon != AK_RECON_PPM4) { fail(AK_EINVAL, "unknown recon"); return nullptr; }
-  if (rsolver != AK_RSOLVER_HLLC) { fail(AK_EINVAL, "unknown rsolver"); return nullptr; }
+  if (rsolver < AK_RSOLVER_HLLC || rsolver > AK_RSOLVER_HLLE) { fail(AK_EINVAL, "unknown rsolver"); return nullptr; }
   if ((recon == AK_RECON_PLM && ng < 2) || (recon == AK_RECON_PPM4 && ng < 3)) {
     fail(AK_EINVAL, "ng too small for the reconstruction stencil"); return nullptr;
   }
@@ -205,6 +205,8 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
   if (stage == 1 && p->cur != 0) return fail(AK_ESTATE, "stage 1 expects U^n in buffer A (call stage 2 first)");
   if (stage == 2 && p->cur != 1) return fail(AK_ESTATE, "stage 2 expects U^(1) in buffer B (call stage 1 first)");
   if (!p->ghosts_ok) return fail(AK_ESTATE, "ak_fill_ghosts must precede ak_hydro_stage");
+  if (p->rsolver != AK_RSOLVER_HLLC && (p->variant != 0 || ((p->d.ng - (p->recon == 0 ? 2 : 3)) & 1)))
+    return fail(AK_EUNSUPPORTED, "LLF / HLLE exist in the production kernel only (variant 0, ng - stencil radius even)");
   // SSPRK(2,2) in two registers (Q1): (g0, g1, beta) = (0,1,1) then (1/2,1/2,1/2)
   ak::StageCoef sc;
   const double beta = (stage == 1) ? 1.0 : 0.5;

@@ -18,7 +18,7 @@
 namespace ak {
 
 // flux of direction D at the lower D-face of cell `c` (index of variable 0 inside one block's U, stride st along D)
-template <int RECON, int D>
+template <int RECON, int RS, int D>
 __device__ __forceinline__ void face_flux_from_u(const GasConst& g, const double* __restrict__ Ub, long long nc, long long c,
                                                  long long st, double F[5]) {
   constexpr int R = (RECON == 0) ? 2 : 3;
@@ -39,10 +39,10 @@ __device__ __forceinline__ void face_flux_from_u(const GasConst& g, const double
     recon2<RECON>(&w[n][R - 1], 1, qm, qp); L[n] = qp;      // q+ of the cell on the - side
     recon2<RECON>(&w[n][R], 1, qm, qp);     Rr[n] = qm;     // q- of the cell on the + side
   }
-  flux2<D>(g, L, Rr, F);
+  flux3<RS, D>(g, L, Rr, F);
 }
 
-template <int RECON, int D>
+template <int RECON, int RS, int D>
 __global__ void __launch_bounds__(128) flux_correct_kernel(PackDev P, const double* __restrict__ Uin, double* __restrict__ Uout,
                                                            double cd) {
   constexpr int T1 = (D == 0) ? 1 : 0, T2 = (D == 2) ? 1 : 2;       // tangential directions, T1 faster
@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(128) flux_correct_kernel(PackDev P, const doub
 
   const long long c = cc[2] * str[2] + cc[1] * str[1] + cc[0];
   double Fc[5];
-  face_flux_from_u<RECON, D>(g, Uin + (long long)m * 5 * nc, nc, c, str[D], Fc);
+  face_flux_from_u<RECON, RS, D>(g, Uin + (long long)m * 5 * nc, nc, c, str[D], Fc);
 
   const int lxm[3] = {b.y, b.z, b.w};
   long long Gc[3];
@@ -90,7 +90,7 @@ __global__ void __launch_bounds__(128) flux_correct_kernel(PackDev P, const doub
         const int mf = P.leaf1[((long long)bf[2] * (2 * P.nrb[1]) + bf[1]) * (2 * P.nrb[0]) + bf[0]];
         if (!side) cf[D] += 1;                                       // the fine block's upper boundary face
         const long long cfi = cf[2] * str[2] + cf[1] * str[1] + cf[0];
-        face_flux_from_u<RECON, D>(g, Uin + (long long)mf * 5 * nc, nc, cfi, str[D], f[s2][s1]);
+        face_flux_from_u<RECON, RS, D>(g, Uin + (long long)mf * 5 * nc, nc, cfi, str[D], f[s2][s1]);
       }
 #pragma unroll
     for (int n = 0; n < 5; n++) Fm[n] = 0.25 * ((f[0][0][n] + f[0][1][n]) + (f[1][0][n] + f[1][1][n]));
@@ -102,20 +102,20 @@ __global__ void __launch_bounds__(128) flux_correct_kernel(PackDev P, const doub
   for (int n = 0; n < 5; n++) Uout[cell + n * nc] = fma(sgn, Fm[n] - Fc[n], Uout[cell + n * nc]);
 }
 
-template <int RECON>
+template <int RECON, int RS>
 cudaError_t launch_flux_correction_t(const ak_pack& p, const double* Uin, double* Uout, const StageCoef& sc) {
   const PackDev& P = p.d;
   {
     dim3 grid((unsigned)((P.nx[1] * P.nx[2] + 127) / 128), 2, (unsigned)P.nmb);
-    flux_correct_kernel<RECON, 0><<<grid, 128, 0, p.stream>>>(P, Uin, Uout, sc.c[0][0]);
+    flux_correct_kernel<RECON, RS, 0><<<grid, 128, 0, p.stream>>>(P, Uin, Uout, sc.c[0][0]);
   }
   {
     dim3 grid((unsigned)((P.nx[0] * P.nx[2] + 127) / 128), 2, (unsigned)P.nmb);
-    flux_correct_kernel<RECON, 1><<<grid, 128, 0, p.stream>>>(P, Uin, Uout, sc.c[0][1]);
+    flux_correct_kernel<RECON, RS, 1><<<grid, 128, 0, p.stream>>>(P, Uin, Uout, sc.c[0][1]);
   }
   {
     dim3 grid((unsigned)((P.nx[0] * P.nx[1] + 127) / 128), 2, (unsigned)P.nmb);
-    flux_correct_kernel<RECON, 2><<<grid, 128, 0, p.stream>>>(P, Uin, Uout, sc.c[0][2]);
+    flux_correct_kernel<RECON, RS, 2><<<grid, 128, 0, p.stream>>>(P, Uin, Uout, sc.c[0][2]);
   }
   return cudaGetLastError();
 }

@@ -224,4 +224,79 @@ __device__ __forceinline__ void flux2_x1x2(const GasConst& g, const double L1[5]
   F2[0] = f[1][0]; F2[2] = f[1][1]; F2[3] = f[1][2]; F2[1] = f[1][3]; F2[4] = f[1][4];
 }
 
+// ---- S3'  LLF and HLLE (paper P:103 option list), rotated states (rho, u_normal, v, w, u_g) ----
+// conserved state, physical flux and sound speed of one rotated primitive state
+__device__ __forceinline__ void state_flux(const GasConst& g, const double W[5], double U[5], double F[5], double& c, double& p) {
+  const double r = W[0], u = W[1], v = W[2], w = W[3], e = W[4];
+  p = g.gm1 * e;
+  const double E = fma(0.5 * r, fma(u, u, fma(v, v, w * w)), e);
+  const double m = r * u;
+  U[0] = r; U[1] = m; U[2] = r * v; U[3] = r * w; U[4] = E;
+  F[0] = m; F[1] = fma(m, u, p); F[2] = m * v; F[3] = m * w; F[4] = (E + p) * u;
+  c = sqrt_ratio(g.gamma * p, r);
+}
+// LLF (Rusanov): F = 1/2 [(F_L + F_R) - a (U_R - U_L)], a = max(|u_L| + c_L, |u_R| + c_R)
+__device__ __forceinline__ void llf2(const GasConst& g, const double WL[5], const double WR[5], double F[5]) {
+  double UL[5], UR[5], FL[5], FR[5], cL, cR, pL, pR;
+  state_flux(g, WL, UL, FL, cL, pL);
+  state_flux(g, WR, UR, FR, cR, pR);
+  const double aL = fabs(WL[1]) + cL, aR = fabs(WR[1]) + cR;
+  const double a = aL > aR ? aL : aR;
+#pragma unroll
+  for (int n = 0; n < 5; n++) F[n] = 0.5 * ((FL[n] + FR[n]) - a * (UR[n] - UL[n]));
+}
+// HLLE with Einfeldt's speeds from the Roe averages (weights sqrt(rho)), bounded by the L/R characteristic speeds
+__device__ __forceinline__ void hlle2(const GasConst& g, const double WL[5], const double WR[5], double F[5]) {
+  double UL[5], UR[5], FL[5], FR[5], cL, cR, pL, pR;
+  state_flux(g, WL, UL, FL, cL, pL);
+  state_flux(g, WR, UR, FR, cR, pR);
+  const double sL = sqrt_ratio(WL[0], 1.0), sR = sqrt_ratio(WR[0], 1.0), isum = rcp2(sL + sR);
+  const double HL = (UL[4] + pL) * rcp2(WL[0]), HR = (UR[4] + pR) * rcp2(WR[0]);
+  const double ut = fma(sL, WL[1], sR * WR[1]) * isum, vt = fma(sL, WL[2], sR * WR[2]) * isum;
+  const double wt = fma(sL, WL[3], sR * WR[3]) * isum, Ht = fma(sL, HL, sR * HR) * isum;
+  const double ct = sqrt_ratio(g.gm1 * fma(-0.5, fma(ut, ut, fma(vt, vt, wt * wt)), Ht), 1.0);
+  const double l1 = WL[1] - cL, l2 = ut - ct, r1 = WR[1] + cR, r2 = ut + ct;
+  const double bm = min0(l1 < l2 ? l1 : l2), bp = max0(r1 > r2 ? r1 : r2);
+  const double inv = rcp2(bp - bm), bb = bp * bm;
+#pragma unroll
+  for (int n = 0; n < 5; n++) F[n] = (fma(bp, FL[n], -(bm * FR[n])) + bb * (UR[n] - UL[n])) * inv;
+}
+
+// solver chosen at compile time: RS = 0 HLLC, 1 LLF, 2 HLLE
+template <int RS>
+__device__ __forceinline__ void riemann2(const GasConst& g, const double l[5], const double r[5], double f[5]) {
+  if constexpr (RS == 0) hllc2(g, l, r, f);
+  else if constexpr (RS == 1) llf2(g, l, r, f);
+  else hlle2(g, l, r, f);
+}
+template <int RS, int D>
+__device__ __forceinline__ void flux3(const GasConst& g, const double L[5], const double Rr[5], double F[5]) {
+  if constexpr (RS == 0) { flux2<D>(g, L, Rr, F); return; }
+  const double l[5] = {L[0], L[1 + D], L[1 + (D + 1) % 3], L[1 + (D + 2) % 3], L[4]};
+  const double r[5] = {Rr[0], Rr[1 + D], Rr[1 + (D + 1) % 3], Rr[1 + (D + 2) % 3], Rr[4]};
+  double f[5];
+  riemann2<RS>(g, l, r, f);
+  F[0] = f[0]; F[1 + D] = f[1]; F[1 + (D + 1) % 3] = f[2]; F[1 + (D + 2) % 3] = f[3]; F[4] = f[4];
+}
+template <int RS>
+__device__ __forceinline__ void flux3_12(const GasConst& g, bool d2, const double L[5], const double Rr[5], double F[5]) {
+  if constexpr (RS == 0) { flux2_12(g, d2, L, Rr, F); return; }
+  const double l[5] = {L[0], d2 ? L[2] : L[1], d2 ? L[3] : L[2], d2 ? L[1] : L[3], L[4]};
+  const double r[5] = {Rr[0], d2 ? Rr[2] : Rr[1], d2 ? Rr[3] : Rr[2], d2 ? Rr[1] : Rr[3], Rr[4]};
+  double f[5];
+  riemann2<RS>(g, l, r, f);
+  F[0] = f[0];
+  F[1] = d2 ? f[3] : f[1];
+  F[2] = d2 ? f[1] : f[2];
+  F[3] = d2 ? f[2] : f[3];
+  F[4] = f[4];
+}
+template <int RS>
+__device__ __forceinline__ void flux3_x1x2(const GasConst& g, const double L1[5], const double R1[5], const double L2[5],
+                                           const double R2[5], double F1[5], double F2[5]) {
+  if constexpr (RS == 0) { flux2_x1x2(g, L1, R1, L2, R2, F1, F2); return; }
+  flux3<RS, 0>(g, L1, R1, F1);
+  flux3<RS, 1>(g, L2, R2, F2);
+}
+
 }  // namespace ak

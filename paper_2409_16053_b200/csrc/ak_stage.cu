@@ -41,15 +41,27 @@ static int pick_tile_v3(const ak_pack& p) {
   return e10 >= e8 ? 0 : 1;
 }
 
-template <int RECON>
+template <int RECON, int RS>
 static cudaError_t launch_stage_v3(const ak_pack& p, const double* Uin, const double* U0, double* Uout,
                                    const StageCoef& sc) {
   const bool stage2 = (Uin != U0);
-  switch (pick_tile_v3(p)) {
-    case 1:  return launch_v3<RECON, 16, 8, 2>(p, Uin, U0, Uout, sc, stage2);
-    case 2:  return launch_v3<RECON, 16, 22, 1>(p, Uin, U0, Uout, sc, stage2);
-    case 3:  return launch_v3<RECON, 32, 11, 1>(p, Uin, U0, Uout, sc, stage2);
-    default: return launch_v3<RECON, 16, 10, 2>(p, Uin, U0, Uout, sc, stage2);
+  int tile = pick_tile_v3(p);
+  if constexpr (RS != 0) { if (tile > 1) tile = 0; }   // LLF / HLLE: only the two 2-CTA/SM tiles are instantiated
+  switch (tile) {
+    case 1:  return launch_v3<RECON, RS, 16, 8, 2>(p, Uin, U0, Uout, sc, stage2);
+    case 2:  if constexpr (RS == 0) return launch_v3<RECON, RS, 16, 22, 1>(p, Uin, U0, Uout, sc, stage2);
+    case 3:  if constexpr (RS == 0) return launch_v3<RECON, RS, 32, 11, 1>(p, Uin, U0, Uout, sc, stage2);
+    default: return launch_v3<RECON, RS, 16, 10, 2>(p, Uin, U0, Uout, sc, stage2);
+  }
+}
+
+template <int RECON>
+static cudaError_t launch_stage_v3_rs(const ak_pack& p, const double* Uin, const double* U0, double* Uout,
+                                      const StageCoef& sc) {
+  switch (p.rsolver) {
+    case 1:  return launch_stage_v3<RECON, 1>(p, Uin, U0, Uout, sc);
+    case 2:  return launch_stage_v3<RECON, 2>(p, Uin, U0, Uout, sc);
+    default: return launch_stage_v3<RECON, 0>(p, Uin, U0, Uout, sc);
   }
 }
 
@@ -61,11 +73,15 @@ cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, 
   if (p.variant == 2 || ((p.d.ng - R) & 1)) return launch_stage_tiled(p, Uin, U0, Uout, sc);
   if (p.variant == 3) return launch_stage_tma(p, Uin, U0, Uout, sc);
   if (p.variant == 4) return p.recon == 0 ? launch_stage_v2<0>(p, Uin, U0, Uout, sc) : launch_stage_v2<1>(p, Uin, U0, Uout, sc);
-  return p.recon == 0 ? launch_stage_v3<0>(p, Uin, U0, Uout, sc) : launch_stage_v3<1>(p, Uin, U0, Uout, sc);
+  return p.recon == 0 ? launch_stage_v3_rs<0>(p, Uin, U0, Uout, sc) : launch_stage_v3_rs<1>(p, Uin, U0, Uout, sc);
 }
 
 cudaError_t launch_flux_correction(const ak_pack& p, const double* Uin, double* Uout, const StageCoef& sc) {
-  return p.recon == 0 ? launch_flux_correction_t<0>(p, Uin, Uout, sc) : launch_flux_correction_t<1>(p, Uin, Uout, sc);
+  switch (p.rsolver) {
+    case 1:  return p.recon == 0 ? launch_flux_correction_t<0, 1>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 1>(p, Uin, Uout, sc);
+    case 2:  return p.recon == 0 ? launch_flux_correction_t<0, 2>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 2>(p, Uin, Uout, sc);
+    default: return p.recon == 0 ? launch_flux_correction_t<0, 0>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 0>(p, Uin, Uout, sc);
+  }
 }
 
 int stage_launches_per_call(const ak_pack&) { return 1; }

@@ -54,7 +54,7 @@ __device__ __forceinline__ void cta_sync(int nthreads) {
   asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }
 
-template <int RECON, int TI, int TJ, int MINB, bool STAGE2>
+template <int RECON, int RS, int TI, int TJ, int MINB, bool STAGE2>
 __global__ void __launch_bounds__(TI * TJ + 32, MINB)
 stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmU0, PackDev P,
                 double* __restrict__ Uout, StageCoef sc, int KC, int ntile_i) {
@@ -154,7 +154,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
           double L[5], F[5];
 #pragma unroll
           for (int n = 0; n < 5; n++) L[n] = Q[n * eQn[q] + eQhi[q]];
-          flux2_12(g, ex2[q], L, qmE[q], F);
+          flux3_12<RS>(g, ex2[q], L, qmE[q], F);
 #pragma unroll
           for (int n = 0; n < 5; n++) Q[n * eQn[q] + eQhi[q]] = F[n];
         }
@@ -258,7 +258,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
     }
     const int c = s - (R - 1);
     double Gn[5];
-    flux2<2>(g, qp3, qm3, Gn);
+    flux3<RS, 2>(g, qp3, qm3, Gn);
     if (c > k0 && c <= k1 && valid) {              // plane c-1 complete: its slot is the one after tslot
       const int ts = (tslot + 1 == NS) ? 0 : tslot + 1;
       const double* Tc = sm + S::oT + ts * (5 * NT) + tid;
@@ -304,7 +304,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
       double L1[5], L2[5], F1[5], F2[5];
 #pragma unroll
       for (int n = 0; n < 5; n++) { L1[n] = Q1[n * (TJ * (TI + 1)) + oQ1]; L2[n] = Q2[n * ((TJ + 1) * TI) + oQ2]; }
-      flux2_x1x2(g, L1, qm1, L2, qm2, F1, F2);     // the two solves interleaved
+      flux3_x1x2<RS>(g, L1, qm1, L2, qm2, F1, F2); // HLLC: the two solves interleaved
 #pragma unroll
       for (int n = 0; n < 5; n++) { Q1[n * (TJ * (TI + 1)) + oQ1] = F1[n]; Q2[n * ((TJ + 1) * TI) + oQ2] = F2[n]; }
     }
@@ -330,7 +330,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
   if (nfl) atomicAdd(P.floor_cnt, (unsigned long long)nfl);
 }
 
-template <int RECON, int TI, int TJ, int MINB>
+template <int RECON, int RS, int TI, int TJ, int MINB>
 cudaError_t launch_v3(const ak_pack& p, const double* Uin, const double* U0, double* Uout, const StageCoef& sc,
                       bool stage2) {
   using S = V3Tile<RECON, TI, TJ>;
@@ -348,8 +348,8 @@ cudaError_t launch_v3(const ak_pack& p, const double* Uin, const double* U0, dou
   const CUtensorMap& tm = (Uin == p.u[0]) ? p.tmap[0] : p.tmap[1];
   const CUtensorMap& tm0 = (U0 == p.u[0]) ? p.tmap0[0] : p.tmap0[1];
   const size_t smem = S::bytes;
-  auto k1 = stage_v3_kernel<RECON, TI, TJ, MINB, false>;
-  auto k2 = stage_v3_kernel<RECON, TI, TJ, MINB, true>;
+  auto k1 = stage_v3_kernel<RECON, RS, TI, TJ, MINB, false>;
+  auto k2 = stage_v3_kernel<RECON, RS, TI, TJ, MINB, true>;
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -51,10 +51,10 @@ def momentum_norm(mesh, U: np.ndarray, gamma: float) -> float:
     return s
 
 
-def make_pair(orc, ak, w: I.Workload, U0: torch.Tensor, variant=0):
-    po = orc.OrcPack(w.mesh, w.gamma, w.recon, threads=NTHREADS)
+def make_pair(orc, ak, w: I.Workload, U0: torch.Tensor, variant=0, rsolver=0):
+    po = orc.OrcPack(w.mesh, w.gamma, w.recon, rsolver=rsolver, threads=NTHREADS)
     po.load(U0.numpy())
-    pg = ak.Pack(w.mesh, w.gamma, w.recon, variant=variant)
+    pg = ak.Pack(w.mesh, w.gamma, w.recon, rsolver=rsolver, variant=variant)
     pg.load(U0)
     return po, pg
 

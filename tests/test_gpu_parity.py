@@ -21,10 +21,10 @@ def ak():
     return _ak
 
 
-def run_lockstep(orc, ak, w, nsteps, variant=0, check_ghosts=True):
+def run_lockstep(orc, ak, w, nsteps, variant=0, check_ghosts=True, rsolver=0):
     """Oracle computes dt; both sides take it.  Returns per-step Q14 and the two final states."""
     U0 = w.state()
-    po, pg = P.make_pair(orc, ak, w, U0, variant)
+    po, pg = P.make_pair(orc, ak, w, U0, variant, rsolver)
     a = P.active(w.mesh)
     errs = []
     for step in range(nsteps):
@@ -409,3 +409,36 @@ def test_flux_correction_keeps_uniform_state_bit_exact_on_gpu(ak):
         pg.step(0.3)
     a = P.active(mesh)
     assert np.array_equal(P.gpu_state(pg)[a], U0.numpy()[a])
+
+
+# ------------------------------------------------------------ LLF / HLLE --------
+@pytest.mark.parametrize("rsolver", [1, 2])
+def test_llf_and_hlle_match_the_oracle(orc, ak, rsolver):
+    """Same kernel skeleton, other two-state solver: PLM on the config-1 recipe and on ragged blocks, PPM4 on the
+    config-3 recipe, the SMR mesh with structure on the level boundaries and flux correction on."""
+    for w in (I.config1(nrb=2, nx=32), I.config3(nrb=2, nx=32)):
+        errs, po, pg, U0 = run_lockstep(orc, ak, w, 4, rsolver=rsolver)
+        assert max(errs) <= TOL_RUN, (rsolver, w.name, errs)
+        check_totals(w, U0, po, pg)
+    w = I.config1(nrb=2, nx=32)
+    w.mesh = I.uniform_mesh((2, 1, 3), (24, 40, 6), 2)
+    errs, *_ = run_lockstep(orc, ak, w, 2, rsolver=rsolver)
+    assert max(errs) <= TOL_RUN, errs
+    w = I.smr_parity(nx=16)
+    U0 = w.state()
+    po, pg = P.make_pair(orc, ak, w, U0, rsolver=rsolver)
+    po.set_flux_correction(True); pg.set_flux_correction(True)
+    for _ in range(3):
+        dt = po.new_dt(w.cfl)
+        po.step(w.cfl, dt); pg.step(w.cfl, dt)
+    assert P.q14(P.gpu_state(pg)[P.active(w.mesh)], po.current()[P.active(w.mesh)], w.gamma) <= TOL_RUN
+    assert check_totals(w, U0, po, pg).max() <= 1e-13
+
+
+def test_llf_hlle_only_in_the_production_kernel(ak):
+    w = I.config1(nrb=1, nx=16)
+    pg = ak.Pack(w.mesh, w.gamma, w.recon, rsolver=1, variant=1)
+    pg.load(w.state())
+    pg.fill_ghosts()
+    with pytest.raises(ak.AkError):
+        pg.hydro_stage(1, 1e-3)
