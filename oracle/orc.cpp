@@ -179,6 +179,7 @@ struct orc_pack {
   int cur = 0;
   long long floor_count = 0;
   int nthreads = 1;
+  int bc[6] = { 0, 0, 0, 0, 0, 0 };      // per face x1min,x1max,...: 0 periodic, 1 outflow, 2 reflect
   bool flux_correction = false;          // SURVEY 8(f) f1, off by default (north_star's stage list omits it)
 
   size_t ncell() const { return (size_t)nt[0] * nt[1] * nt[2]; }
@@ -252,11 +253,20 @@ extern "C" int orc_pack_bind(orc_pack* p, double* u_a, double* u_b) {
   }
   if (vol != (double)p->nrb[0] * p->nrb[1] * p->nrb[2]) return fail("leaves do not cover the domain");
   if (p->max_level > 0 && (p->ng & 1)) return fail("static refinement needs even ng");
+  for (int f = 0; f < 6; f++) if (p->bc[f] != 0 && p->max_level > 0) return fail("physical boundaries need a single-level mesh");
   p->u[0] = u_a; p->u[1] = u_b; p->cur = 0; p->bound = true; p->floor_count = 0;
   return 0;
 }
 
 extern "C" int orc_set_threads(orc_pack* p, int n) { if (!p || n < 1) return fail("bad thread count"); p->nthreads = n; return 0; }
+extern "C" int orc_pack_set_boundaries(orc_pack* p, const int bc[6]) {
+  if (!p || !bc) return fail("null argument");
+  for (int f = 0; f < 6; f++) if (bc[f] < 0 || bc[f] > 2) return fail("unknown boundary condition");
+  for (int d = 0; d < 3; d++) if ((bc[2 * d] == 0) != (bc[2 * d + 1] == 0)) return fail("periodic faces come in pairs");
+  for (int f = 0; f < 6; f++) p->bc[f] = bc[f];
+  p->bound = false;
+  return 0;
+}
 extern "C" int orc_set_flux_correction(orc_pack* p, int on) { if (!p) return fail("null pack"); p->flux_correction = on != 0; return 0; }
 extern "C" double* orc_pack_current(orc_pack* p) { return (p && p->bound) ? p->u[p->cur] : nullptr; }
 extern "C" long long orc_pack_floor_count(const orc_pack* p) { return p ? p->floor_count : -1; }
@@ -310,8 +320,20 @@ static int fill_block(const orc_pack* p, double* U, int m) {
     bool ghost = false;
     for (int d = 0; d < 3; d++) if (a[d] < 0 || a[d] >= p->nx[d]) ghost = true;
     if (!ghost) continue;
+    // position of the cell's image inside the domain: periodic wrap, or -- SURVEY 8(f) f3, the paper's
+    // outflow / reflecting boundary functions -- the nearest active cell (outflow: zero gradient) or the mirror
+    // image across the boundary face with the normal momentum negated (reflect)
     long G[3];
-    for (int d = 0; d < 3; d++) G[d] = wrapl((long)p->lx[3 * (size_t)m + d] * p->nx[d] + a[d], p->nglob(lev, d));
+    double sgn[5] = { 1.0, 1.0, 1.0, 1.0, 1.0 };
+    for (int d = 0; d < 3; d++) {
+      const long N = p->nglob(lev, d);
+      long g = (long)p->lx[3 * (size_t)m + d] * p->nx[d] + a[d];
+      if (g >= 0 && g < N) { G[d] = g; continue; }
+      const int kind = p->bc[2 * d + (g < 0 ? 0 : 1)];
+      if (kind == 0) G[d] = wrapl(g, N);
+      else if (kind == 1) G[d] = g < 0 ? 0 : N - 1;
+      else { G[d] = g < 0 ? -1 - g : 2 * N - 1 - g; sgn[1 + d] = -sgn[1 + d]; }
+    }
     // G1: which leaf covers this position?
     int src = p->find_leaf(lev, G[0] / p->nx[0], G[1] / p->nx[1], G[2] / p->nx[2]);
     for (int n = 0; n < 5; n++) {
@@ -336,7 +358,7 @@ static int fill_block(const orc_pack* p, double* U, int m) {
         }
         val = ((c0 + s[0] * g[0]) + s[1] * g[1]) + s[2] * g[2];
       }
-      U[p->idx(m, n, k, j, i)] = val;
+      U[p->idx(m, n, k, j, i)] = sgn[n] * val;
     }
   }
   return 0;

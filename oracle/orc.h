@@ -38,6 +38,9 @@ orc_pack* orc_pack_create(int nmb, int nx1, int nx2, int nx3, int ng, double gam
 int orc_pack_set_mesh(orc_pack*, int nrb1, int nrb2, int nrb3,
                       double x1min, double x1max, double x2min, double x2max, double x3min, double x3max);
 int orc_pack_set_block(orc_pack*, int m, int level, int lx1, int lx2, int lx3);
+/* f3: boundary condition per face (x1min, x1max, x2min, x2max, x3min, x3max): 0 periodic (default), 1 outflow,
+ * 2 reflect.  Periodic faces come in pairs; non-periodic boundaries need a single-level mesh.  Call before bind. */
+int orc_pack_set_boundaries(orc_pack*, const int bc[6]);
 /* u_a holds U^n on entry; u_b is the second register.  Validates that the leaves tile the domain. */
 int orc_pack_bind(orc_pack*, double* u_a, double* u_b);
 int orc_set_threads(orc_pack*, int nthreads);

@@ -38,6 +38,7 @@ def lib():
     L.orc_pack_set_mesh.argtypes = [C.c_void_p] + [C.c_int] * 3 + [C.c_double] * 6
     L.orc_pack_set_block.argtypes = [C.c_void_p] + [C.c_int] * 5
     L.orc_pack_bind.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.orc_pack_set_boundaries.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
     L.orc_set_threads.argtypes = [C.c_void_p, C.c_int]
     L.orc_set_flux_correction.argtypes = [C.c_void_p, C.c_int]
     L.orc_fill_ghosts.argtypes = [C.c_void_p]
@@ -137,6 +138,9 @@ class OrcPack:
                                  mesh.xmin[2], mesh.xmax[2]))
         for m, (lev, l1, l2, l3) in enumerate(mesh.blocks):
             _chk(L.orc_pack_set_block(self._h, m, lev, l1, l2, l3))
+        bc = tuple(getattr(mesh, "bc", (0,) * 6))
+        if any(bc):
+            _chk(L.orc_pack_set_boundaries(self._h, (C.c_int * 6)(*bc)))
         self.ua = np.zeros(mesh.state_shape(), dtype=np.float64)
         self.ub = np.zeros(mesh.state_shape(), dtype=np.float64)
         _chk(L.orc_pack_bind(self._h, self.ua.ctypes.data, self.ub.ctypes.data))

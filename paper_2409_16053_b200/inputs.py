@@ -42,6 +42,8 @@ class Mesh:
     blocks: List[Tuple[int, int, int, int]]
     xmin: Tuple[float, float, float] = (0.0, 0.0, 0.0)
     xmax: Tuple[float, float, float] = (1.0, 1.0, 1.0)
+    # boundary condition per face (x1min, x1max, x2min, x2max, x3min, x3max): 0 periodic, 1 outflow, 2 reflect
+    bc: Tuple[int, int, int, int, int, int] = (0, 0, 0, 0, 0, 0)
 
     @property
     def nmb(self) -> int:
