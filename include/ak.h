@@ -124,6 +124,12 @@ long long ak_pack_floor_count(ak_pack*);
  * AK_EINVAL for any other value. */
 int ak_pack_set_variant(ak_pack*, int variant);
 
+/* Boundary condition per domain face, in the order x1min, x1max, x2min, x2max, x3min, x3max (paper P:67; SURVEY
+ * 8(f) f3): 0 = periodic (default), 1 = outflow (ghost <- nearest active cell), 2 = reflect (ghost <- mirror image
+ * across the face, normal momentum negated).  Periodic faces come in pairs (AK_EINVAL otherwise).  Call before
+ * ak_pack_bind (a bound pack becomes unbound); outflow / reflect need a single-level mesh (bind: AK_EUNSUPPORTED). */
+int ak_pack_set_boundaries(ak_pack*, const int bc[6]);
+
 /* Flux correction at coarse-fine faces (paper P:57).  on != 0: after every ak_hydro_stage on a
  * refined mesh, the flux a level-0 cell used at a face shared with level-1 blocks is replaced by the mean of the
  * four fine fluxes through that face (three small extra launches per stage), which makes the update

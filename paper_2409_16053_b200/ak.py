@@ -23,7 +23,7 @@ RSOLVER_HLLC, RSOLVER_LLF, RSOLVER_HLLE = 0, 1, 2
 SYMBOLS = [
     "ak_last_error", "ak_pack_create", "ak_pack_set_mesh", "ak_pack_set_block", "ak_pack_state_bytes",
     "ak_pack_scratch_bytes", "ak_pack_bind", "ak_fill_ghosts", "ak_hydro_stage", "ak_new_dt", "ak_step",
-    "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_floor_count", "ak_pack_set_variant", "ak_pack_set_tile", "ak_pack_set_flux_correction",
+    "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_floor_count", "ak_pack_set_variant", "ak_pack_set_tile", "ak_pack_set_flux_correction", "ak_pack_set_boundaries",
     "ak_pack_launch_count", "ak_pack_destroy",
 ]
 
@@ -60,6 +60,7 @@ def lib():
         "ak_pack_set_variant": (i, [vp, i]),
         "ak_pack_set_tile": (i, [vp, i]),
         "ak_pack_set_flux_correction": (i, [vp, i]),
+        "ak_pack_set_boundaries": (i, [vp, C.POINTER(C.c_int)]),
         "ak_pack_launch_count": (ll, [vp]),
         "ak_pack_destroy": (i, [vp]),
     }
@@ -91,6 +92,9 @@ class Pack:
                                 mesh.xmin[2], mesh.xmax[2]))
         for m, (lev, l1, l2, l3) in enumerate(mesh.blocks):
             _chk(L.ak_pack_set_block(self._h, m, lev, l1, l2, l3))
+        bc = tuple(getattr(mesh, "bc", (0,) * 6))
+        if any(bc):
+            _chk(L.ak_pack_set_boundaries(self._h, (C.c_int * 6)(*bc)))
         nbytes = L.ak_pack_state_bytes(self._h)
         assert nbytes == 8 * int(torch.tensor(mesh.state_shape()).prod())
         with torch.cuda.device(self.device):

@@ -21,7 +21,7 @@ extern "C" const char* ak_last_error(void) { return g_err.c_str(); }
 static size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
 
 // scratch layout: [0,256) reduction cells | block table int4[nmb] | leaf0 | leaf1 | same-level neighbours int[nmb][27]
-struct ScratchLayout { size_t blk, leaf0, leaf1, nbr, total; };
+struct ScratchLayout { size_t blk, leaf0, leaf1, nbr, nbc, total; };
 static ScratchLayout scratch_layout(const ak_pack* p) {
   ScratchLayout s;
   const ak::PackDev& d = p->d;
@@ -30,7 +30,8 @@ static ScratchLayout scratch_layout(const ak_pack* p) {
   s.leaf0 = s.blk + align256(sizeof(int4) * (size_t)d.nmb);
   s.leaf1 = s.leaf0 + align256(sizeof(int) * n0);
   s.nbr = s.leaf1 + align256(sizeof(int) * 8 * n0);
-  s.total = s.nbr + align256(sizeof(int) * 27 * (size_t)d.nmb);
+  s.nbc = s.nbr + align256(sizeof(int) * 27 * (size_t)d.nmb);
+  s.total = s.nbc + align256(sizeof(int) * 27 * (size_t)d.nmb);
   return s;
 }
 
@@ -130,26 +131,39 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
     if (!root_leaf && nchild != 8) return fail(AK_EINVAL, "leaves do not cover the domain");
   }
   if (d.max_level > 0 && (d.ng & 1)) return fail(AK_EUNSUPPORTED, "static refinement needs even ng");
+  for (int f = 0; f < 6; f++)
+    if (p->bc[f] != 0 && d.max_level > 0) return fail(AK_EUNSUPPORTED, "outflow / reflecting boundaries need a single-level mesh");
   // ---- upload tables ----
   cudaStream_t st = (cudaStream_t)cuda_stream;
   std::vector<int4> blk(d.nmb);
   for (int m = 0; m < d.nmb; m++) blk[m] = make_int4(p->level[m], p->lx[3 * m], p->lx[3 * m + 1], p->lx[3 * m + 2]);
   // same-level neighbour of block m in direction (d1, d2, d3) in {-1,0,1}^3 (periodic wrap), or -1 where the
   // position is covered by a leaf of another level (the ghost fill then takes the general path)
-  std::vector<int> nbr(27 * (size_t)d.nmb, -1);
+  std::vector<int> nbr(27 * (size_t)d.nmb, -1), nbc(27 * (size_t)d.nmb, 0);
   for (int m = 0; m < d.nmb; m++) {
     const int lev = p->level[m];
     const int nb[3] = {d.nrb[0] << lev, d.nrb[1] << lev, d.nrb[2] << lev};
     const std::vector<int>& leaf = lev ? leaf1 : leaf0;
     for (int d3 = -1; d3 <= 1; d3++) for (int d2 = -1; d2 <= 1; d2++) for (int d1 = -1; d1 <= 1; d1++) {
-      const int b1 = (p->lx[3 * m] + d1 + nb[0]) % nb[0], b2 = (p->lx[3 * m + 1] + d2 + nb[1]) % nb[1];
-      const int b3 = (p->lx[3 * m + 2] + d3 + nb[2]) % nb[2];
-      nbr[27 * (size_t)m + (d3 + 1) * 9 + (d2 + 1) * 3 + (d1 + 1)] = leaf[((size_t)b3 * nb[1] + b2) * nb[0] + b1];
+      const int dd[3] = {d1, d2, d3};
+      int b[3], code = 0;
+      for (int e = 0; e < 3; e++) {
+        b[e] = p->lx[3 * m + e] + dd[e];
+        if (b[e] < 0 || b[e] >= nb[e]) {
+          const int kind = p->bc[2 * e + (b[e] < 0 ? 0 : 1)];
+          if (kind == 0) b[e] = (b[e] + nb[e]) % nb[e];              // periodic wrap
+          else { b[e] = p->lx[3 * m + e]; code |= kind << (2 * e); }  // image lies in the boundary block itself
+        }
+      }
+      const size_t k = 27 * (size_t)m + (d3 + 1) * 9 + (d2 + 1) * 3 + (d1 + 1);
+      nbr[k] = leaf[((size_t)b[2] * nb[1] + b[1]) * nb[0] + b[0]];
+      nbc[k] = code;
     }
   }
   char* s = (char*)scratch;
   AK_CUDA(cudaMemsetAsync(s, 0, 256, st), "memset scratch");
   AK_CUDA(cudaMemcpyAsync(s + sl.nbr, nbr.data(), sizeof(int) * nbr.size(), cudaMemcpyHostToDevice, st), "upload neighbour table");
+  AK_CUDA(cudaMemcpyAsync(s + sl.nbc, nbc.data(), sizeof(int) * nbc.size(), cudaMemcpyHostToDevice, st), "upload boundary table");
   AK_CUDA(cudaMemcpyAsync(s + sl.blk, blk.data(), sizeof(int4) * d.nmb, cudaMemcpyHostToDevice, st), "upload block table");
   AK_CUDA(cudaMemcpyAsync(s + sl.leaf0, leaf0.data(), sizeof(int) * n0, cudaMemcpyHostToDevice, st), "upload leaf map 0");
   AK_CUDA(cudaMemcpyAsync(s + sl.leaf1, leaf1.data(), sizeof(int) * 8 * n0, cudaMemcpyHostToDevice, st), "upload leaf map 1");
@@ -160,6 +174,7 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
   d.leaf0 = (const int*)(s + sl.leaf0);
   d.leaf1 = (const int*)(s + sl.leaf1);
   d.nbr = (const int*)(s + sl.nbr);
+  d.nbc = (const int*)(s + sl.nbc);
   int dev = 0;
   AK_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
   AK_CUDA(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev), "query SM count");
@@ -174,6 +189,16 @@ extern "C" int ak_pack_set_variant(ak_pack* p, int variant) {
   if (!p) return fail(AK_EINVAL, "null pack");
   if (variant < 0 || variant > 4) return fail(AK_EINVAL, "unknown variant");
   p->variant = variant;
+  return AK_OK;
+}
+
+extern "C" int ak_pack_set_boundaries(ak_pack* p, const int bc[6]) {
+  if (!p || !bc) return fail(AK_EINVAL, "null argument");
+  for (int f = 0; f < 6; f++) if (bc[f] < 0 || bc[f] > 2) return fail(AK_EINVAL, "unknown boundary condition");
+  for (int e = 0; e < 3; e++)
+    if ((bc[2 * e] == 0) != (bc[2 * e + 1] == 0)) return fail(AK_EINVAL, "periodic faces come in pairs");
+  for (int f = 0; f < 6; f++) p->bc[f] = bc[f];
+  p->bound = false;                     // the neighbour tables are built at bind
   return AK_OK;
 }
 

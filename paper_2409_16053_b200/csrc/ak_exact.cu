@@ -102,13 +102,29 @@ __device__ __forceinline__ void fill_cell(const PackDev& P, double* __restrict__
   const int d1 = (i < ng) ? -1 : (i >= P.nx[0] + ng ? 1 : 0);
   const int d2 = (j < ng) ? -1 : (j >= P.nx[1] + ng ? 1 : 0);
   const int d3 = (k < ng) ? -1 : (k >= P.nx[2] + ng ? 1 : 0);
-  const int src = nb[(d3 + 1) * 9 + (d2 + 1) * 3 + (d1 + 1)];
+  const int dir = (d3 + 1) * 9 + (d2 + 1) * 3 + (d1 + 1);
+  const int src = nb[dir];
   double val[5];
   if (src < 0) return;                 // cannot happen on a uniform mesh
-  const int si = i - d1 * P.nx[0], sj = j - d2 * P.nx[1], sk = k - d3 * P.nx[2];
-  const double* q = U + (long long)src * 5 * P.ncell + ((long long)sk * n2 + sj) * n1 + si;
+  const int code = P.nbc[27 * m + dir];
+  int si = i - d1 * P.nx[0], sj = j - d2 * P.nx[1], sk = k - d3 * P.nx[2];      // image one block length away
+  if (code) {                          // the ghost lies outside a non-periodic domain boundary
+    const int c1 = code & 3, c2 = (code >> 2) & 3, c3 = (code >> 4) & 3;
+    // outflow: the nearest active cell; reflect: the mirror image across the boundary face
+    if (c1) si = (c1 == 1) ? (d1 < 0 ? ng : P.nx[0] + ng - 1) : (d1 < 0 ? 2 * ng - 1 - i : 2 * (P.nx[0] + ng) - 1 - i);
+    if (c2) sj = (c2 == 1) ? (d2 < 0 ? ng : P.nx[1] + ng - 1) : (d2 < 0 ? 2 * ng - 1 - j : 2 * (P.nx[1] + ng) - 1 - j);
+    if (c3) sk = (c3 == 1) ? (d3 < 0 ? ng : P.nx[2] + ng - 1) : (d3 < 0 ? 2 * ng - 1 - k : 2 * (P.nx[2] + ng) - 1 - k);
+    const double* q = U + (long long)src * 5 * P.ncell + ((long long)sk * n2 + sj) * n1 + si;
 #pragma unroll
-  for (int n = 0; n < 5; n++) val[n] = q[n * P.ncell];
+    for (int n = 0; n < 5; n++) val[n] = q[n * P.ncell];
+    if (c1 == 2) val[1] = -val[1];     // the normal momentum of a reflected image changes sign
+    if (c2 == 2) val[2] = -val[2];
+    if (c3 == 2) val[3] = -val[3];
+  } else {
+    const double* q = U + (long long)src * 5 * P.ncell + ((long long)sk * n2 + sj) * n1 + si;
+#pragma unroll
+    for (int n = 0; n < 5; n++) val[n] = q[n * P.ncell];
+  }
   double* o = U + (long long)m * 5 * P.ncell + ((long long)k * n2 + j) * n1 + i;
 #pragma unroll
   for (int n = 0; n < 5; n++) o[n * P.ncell] = val[n];

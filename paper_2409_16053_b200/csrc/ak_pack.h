@@ -24,6 +24,8 @@ struct PackDev {
   const int* leaf0; // [nrb3][nrb2][nrb1]       -> block index or -1
   const int* leaf1; // [2nrb3][2nrb2][2nrb1]    -> block index or -1
   const int* nbr;   // [nmb][27] same-level neighbour in direction (d3+1)*9+(d2+1)*3+(d1+1), or -1
+  const int* nbc;   // [nmb][27] how to map the ghost index per direction: 2 bits each (d1 | d2<<2 | d3<<4),
+                    // 0 = shift by one block length (periodic / interior), 1 = outflow, 2 = reflect
   double dx0[3];    // level-0 cell size; level 1 is exactly half
   double gamma;
   unsigned long long* dtmin_bits;   // scratch cell: min candidate dt as ordered bits
@@ -49,6 +51,7 @@ struct ak_pack {
   cudaStream_t stream = nullptr;
   int cur = 0;
   int variant = 0;
+  int bc[6] = {0, 0, 0, 0, 0, 0};  // ak_pack_set_boundaries: x1min,x1max,x2min,x2max,x3min,x3max
   bool flux_correction = false;   // ak_pack_set_flux_correction
   int tile = -1;                  // -1 = automatic (ak_pack_set_tile)
   long long launches = 0;
