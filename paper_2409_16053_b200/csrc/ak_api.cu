@@ -170,6 +170,7 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
   AK_CUDA(cudaStreamSynchronize(st), "bind sync");
   d.dtmin_bits = (unsigned long long*)s;
   d.floor_cnt = (unsigned long long*)(s + 8);
+  d.smax_bits = (unsigned long long*)(s + 64);
   d.blk = (const int4*)(s + sl.blk);
   d.leaf0 = (const int*)(s + sl.leaf0);
   d.leaf1 = (const int*)(s + sl.leaf1);
@@ -179,7 +180,7 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
   AK_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
   AK_CUDA(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev), "query SM count");
   p->u[0] = (double*)u_a; p->u[1] = (double*)u_b; p->scratch = scratch; p->stream = st;
-  p->cur = 0; p->ghosts_ok = false; p->bound = true; p->launches = 0;
+  p->cur = 0; p->ghosts_ok = false; p->bound = true; p->launches = 0; p->dt_cached = false;
   p->tmap_box[0] = p->tmap_box[1] = 0;
   p->tmap0_box[0] = p->tmap0_box[1] = 0;
   return AK_OK;
@@ -242,11 +243,17 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
       double dx = (p->xmax[d] - p->xmin[d]) / ((double)p->d.nrb[d] * p->d.nx[d] * (double)(1 << lev));
       sc.c[lev][d] = beta * dt / dx;
     }
+  // stage 2 of the production kernel also leaves the max signal speeds of U^{n+1} for the next ak_new_dt
+  const bool v3 = p->variant == 0 && !((p->d.ng - (p->recon == 0 ? 2 : 3)) & 1);
+  p->dt_cached = false;
+  if (stage == 2 && v3) AK_CUDA(cudaMemsetAsync(p->d.smax_bits, 0, 48, p->stream), "reset signal speeds");
   AK_CUDA(ak::launch_stage(*p, p->u[p->cur], p->u[0], p->u[1 - p->cur], sc), "ak_hydro_stage launch");
   p->launches += ak::stage_launches_per_call(*p);
+  if (stage == 2 && v3) p->dt_cached = true;
   if (p->flux_correction && p->d.max_level > 0) {
     AK_CUDA(ak::launch_flux_correction(*p, p->u[p->cur], p->u[1 - p->cur], sc), "flux correction launch");
     p->launches += 3;
+    p->dt_cached = false;               // the correction changed cells after their signal speeds were taken
   }
   p->cur = 1 - p->cur;
   p->ghosts_ok = false;
@@ -257,11 +264,25 @@ extern "C" int ak_new_dt(ak_pack* p, double cfl, double* dt_out) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
   if (!dt_out) return fail(AK_EINVAL, "null dt_out");
   if (!(cfl > 0.0)) return fail(AK_EINVAL, "cfl must be positive");
-  AK_CUDA(ak::launch_new_dt(*p, p->u[p->cur]), "ak_new_dt launch");
-  p->launches += 2;
   double dtmin = 0.0;
-  AK_CUDA(cudaMemcpyAsync(&dtmin, p->d.dtmin_bits, 8, cudaMemcpyDeviceToHost, p->stream), "ak_new_dt copy");
-  AK_CUDA(cudaStreamSynchronize(p->stream), "ak_new_dt sync");
+  if (p->dt_cached) {
+    // min over cells of dx_d / (|v_d| + c_s) = dx_d / max(|v_d| + c_s), bit for bit (IEEE division is monotone in
+    // its divisor); the maxima per level and direction were taken by stage 2 from the values it wrote
+    double s[6];
+    AK_CUDA(cudaMemcpyAsync(s, p->d.smax_bits, 48, cudaMemcpyDeviceToHost, p->stream), "ak_new_dt copy");
+    AK_CUDA(cudaStreamSynchronize(p->stream), "ak_new_dt sync");
+    dtmin = HUGE_VAL;
+    for (int lev = 0; lev < 2; lev++)
+      for (int d = 0; d < 3; d++) {
+        const double dx = (lev ? 0.5 : 1.0) * p->d.dx0[d];
+        if (s[3 * lev + d] > 0.0) dtmin = std::fmin(dtmin, dx / s[3 * lev + d]);
+      }
+  } else {
+    AK_CUDA(ak::launch_new_dt(*p, p->u[p->cur]), "ak_new_dt launch");
+    p->launches += 2;
+    AK_CUDA(cudaMemcpyAsync(&dtmin, p->d.dtmin_bits, 8, cudaMemcpyDeviceToHost, p->stream), "ak_new_dt copy");
+    AK_CUDA(cudaStreamSynchronize(p->stream), "ak_new_dt sync");
+  }
   if (!(dtmin > 0.0) || !std::isfinite(dtmin)) return fail(AK_ECUDA, "non-finite time step (state corrupted?)");
   *dt_out = cfl * dtmin;
   return AK_OK;
@@ -284,7 +305,7 @@ extern "C" int ak_pack_upload(ak_pack* p, const void* host_u) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
   if (!host_u) return fail(AK_EINVAL, "null host buffer");
   AK_CUDA(cudaMemcpyAsync(p->u[0], host_u, ak_pack_state_bytes(p), cudaMemcpyHostToDevice, p->stream), "ak_pack_upload");
-  p->cur = 0; p->ghosts_ok = false;
+  p->cur = 0; p->ghosts_ok = false; p->dt_cached = false;
   return AK_OK;
 }
 

@@ -30,6 +30,7 @@ struct PackDev {
   double gamma;
   unsigned long long* dtmin_bits;   // scratch cell: min candidate dt as ordered bits
   unsigned long long* floor_cnt;    // scratch cell: floor activations
+  unsigned long long* smax_bits;    // 6 scratch cells [level][d]: max |v_d| + c_s of U^{n+1} as ordered bits (stage 2)
 };
 
 struct StageCoef {
@@ -44,6 +45,7 @@ struct ak_pack {
   int recon = 0, rsolver = 0;
   double xmin[3]{}, xmax[3]{};
   bool mesh_set = false, bound = false, ghosts_ok = false;
+  bool dt_cached = false;         // smax_bits describe the current state (set by stage 2 of the production kernel)
   std::vector<int> level, lx;     // lx[3m+d]
   std::vector<char> blk_set;
   double* u[2] = {nullptr, nullptr};

@@ -195,6 +195,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
   }
 
   double wk[R][5], qlow[5], qp3[5], G[5];
+  double smax[3] = {0.0, 0.0, 0.0};                     // stage 2: max signal speed per direction over this thread's cells
   int nfl = 0;
 #pragma unroll
   for (int a = 0; a < R; a++)
@@ -263,8 +264,23 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
       const int ts = (tslot + 1 == NS) ? 0 : tslot + 1;
       const double* Tc = sm + S::oT + ts * (5 * NT) + tid;
       double* o = Uout + col + (long long)(c - 1 + ng) * plane;
+      double un[5];
 #pragma unroll
-      for (int n = 0; n < 5; n++) o[n * nc] = fma(-c3, Gn[n] - G[n], Tc[n * NT]);
+      for (int n = 0; n < 5; n++) { un[n] = fma(-c3, Gn[n] - G[n], Tc[n * NT]); o[n * nc] = un[n]; }
+      if constexpr (STAGE2) {
+        // S0 of the NEXT step (Eq.(3)) on U^{n+1} while it is in registers: the cell's signal speeds
+        // |v_d| + c_s in the oracle's arithmetic (IEEE division and sqrt, no contraction: this translation unit
+        // is compiled with -fmad=false), so that ak_new_dt need not read the state again
+        double rho = un[0];
+        if (!(rho >= RHO_FLOOR)) rho = RHO_FLOOR;
+        const double rinv = 1.0 / rho;
+        double ug = un[4] - 0.5 * rinv * (un[1] * un[1] + (un[2] * un[2] + un[3] * un[3]));
+        if (!(ug >= g.ug_floor)) ug = g.ug_floor;
+        const double cs = sqrt(g.gamma * (g.gm1 * ug) / rho);
+        smax[0] = fmax(smax[0], fabs(un[1] * rinv) + cs);
+        smax[1] = fmax(smax[1], fabs(un[2] * rinv) + cs);
+        smax[2] = fmax(smax[2], fabs(un[3] * rinv) + cs);
+      }
     }
 #pragma unroll
     for (int n = 0; n < 5; n++) { G[n] = Gn[n]; qp3[n] = qpn[n]; }
@@ -328,6 +344,16 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
     dslot = (dslot + 1 == NS) ? 0 : dslot + 1;
   }
   if (nfl) atomicAdd(P.floor_cnt, (unsigned long long)nfl);
+  if constexpr (STAGE2) {
+    // positive doubles order like their bit patterns: warp max by shuffles, one atomicMax per warp and direction
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+      double v = smax[d];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+      if ((tid & 31) == 0 && v > 0.0) atomicMax(P.smax_bits + 3 * lev + d, (unsigned long long)__double_as_longlong(v));
+    }
+  }
 }
 
 template <int RECON, int RS, int TI, int TJ, int MINB>

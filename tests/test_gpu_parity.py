@@ -393,7 +393,8 @@ def test_flux_correction_off_drifts_and_on_is_inert_on_uniform_mesh(ak):
         l0 = pu.launch_count()
         for _ in range(2):
             pu.step(wu.cfl)
-        assert pu.launch_count() - l0 == 2 * 6  # dt_init + new_dt + 2 x (fill + stage): no correction launches
+        # step 1: dt_init + new_dt + 2 x (fill + stage); step 2: the dt comes from stage 2 of step 1; no correction launches
+        assert pu.launch_count() - l0 == 6 + 4
         res.append(P.gpu_state(pu))
     assert np.array_equal(res[0], res[1])
 
@@ -498,3 +499,28 @@ def test_boundary_argument_errors(ak):
         ak.Pack(dataclasses.replace(I.uniform_mesh((1, 1, 1), (8, 8, 8), 2), bc=(1, 0, 0, 0, 0, 0)), I.GAMMA, 0)
     with pytest.raises(ak.AkError):
         ak.Pack(dataclasses.replace(I.smr_mesh((2, 2, 2), (8, 8, 8), 2, (0, 0, 0), (1, 1, 1)), bc=(1, 1, 0, 0, 0, 0)), I.GAMMA, 0)
+
+
+# ------------------------------------------------------------ dt taken by stage 2 --------
+@pytest.mark.parametrize("which", ["cfg1", "cfg3", "smr", "walls"])
+def test_dt_from_stage2_is_bit_identical_to_the_reduction_over_the_state(orc, ak, which):
+    """After a step, ak_new_dt answers from the signal speeds stage 2 left behind (no kernel launch).  It must equal,
+    bit for bit, the oracle's Eq.(3) reduction over the GPU's own state -- and the stand-alone reduction kernel."""
+    import dataclasses
+    w = {"cfg1": lambda: I.config1(nrb=2, nx=32), "cfg3": lambda: I.config3(nrb=2, nx=32), "smr": lambda: I.smr_parity(nx=16),
+         "walls": lambda: I.config1(nrb=2, nx=16)}[which]()
+    if which == "walls":
+        w.mesh = dataclasses.replace(w.mesh, bc=(2, 2, 1, 1, 0, 0))
+    pg = ak.Pack(w.mesh, w.gamma, w.recon)
+    pg.load(w.state())
+    for step in range(3):
+        pg.step(w.cfl)
+        l0 = pg.launch_count()
+        dt_fused = pg.new_dt(w.cfl)
+        assert pg.launch_count() == l0                      # answered without a launch
+        po = orc.OrcPack(w.mesh, w.gamma, w.recon, threads=P.NTHREADS)
+        po.load(P.gpu_state(pg))
+        assert po.new_dt(w.cfl) == dt_fused, (which, step)
+        po.close()
+        pg.upload(pg.current().cpu().contiguous())          # invalidates the cache: the reduction kernel runs
+        assert pg.new_dt(w.cfl) == dt_fused and pg.launch_count() == l0 + 2
