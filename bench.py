@@ -28,10 +28,11 @@ UNIT = "cell-updates/s"
 BYTES_PER_CELL_UPDATE = 200.0      # 5 streams x 5 vars x 8 B per RK2 cell-update
 BYTES_STAGE = {1: 80.0, 2: 120.0}  # per active cell: stage 1 reads U^n writes U^(1); stage 2 reads U^(1),U^n writes
 # FP64-pipe thread instructions per active cell per stage launch of the PPM4+HLLC kernel, counted by ncu on
-# cfg3 (profiles/r01_v3_stage_cfg3.md: 656 in stage 1, 666 in stage 2), and the same capture's DRAM bytes per
-# stage launch (12.31 GB and 17.71 GB); both are properties of the committed kernel, not of this run
-FP64_INSTR_PER_CELL_STAGE_PPM = 661.0
-NCU_DRAM_BYTES_PER_STAGE_LAUNCH_CFG3 = 15.01e9
+# cfg3 (profiles/r01_v3_stage_cfg3.md: 656 in stage 1, 708 in stage 2, which also takes the next step's CFL
+# reduction), and the same capture's DRAM bytes per stage launch (12.29 GB and 17.69 GB); both are properties of
+# the committed kernel, not of this run
+FP64_INSTR_PER_CELL_STAGE_PPM = 682.0
+NCU_DRAM_BYTES_PER_STAGE_LAUNCH_CFG3 = 14.99e9
 FP64_LANES_PER_SM = 64             # DESIGN.md 6.1 (ncu peak_sustained of the dfma counter / SM count)
 
 
