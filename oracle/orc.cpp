@@ -175,7 +175,8 @@ struct orc_pack {
   std::vector<char> blk_set;
   std::map<std::tuple<int, int, int, int>, int> leaf;   // (level, l1, l2, l3) -> m
   int max_level = 0;
-  double* u[2] = { nullptr, nullptr };
+  double* u[3] = { nullptr, nullptr, nullptr };   // A (U^n at the start of a step), B, and C (third register, RK3 only)
+  int integrator = 2;                             // number of stages: 2 = SSPRK(2,2) (default), 3 = SSPRK(3,3) (f2)
   int cur = 0;
   long long floor_count = 0;
   int nthreads = 1;
@@ -265,6 +266,14 @@ extern "C" int orc_pack_set_boundaries(orc_pack* p, const int bc[6]) {
   for (int d = 0; d < 3; d++) if ((bc[2 * d] == 0) != (bc[2 * d + 1] == 0)) return fail("periodic faces come in pairs");
   for (int f = 0; f < 6; f++) p->bc[f] = bc[f];
   p->bound = false;
+  return 0;
+}
+extern "C" int orc_set_integrator(orc_pack* p, int nstages, double* u_c) {
+  if (!p) return fail("null pack");
+  if (nstages != 2 && nstages != 3) return fail("integrator must be 2 (SSPRK(2,2)) or 3 (SSPRK(3,3))");
+  if (nstages == 3 && !u_c) return fail("SSPRK(3,3) needs a third state buffer");
+  if (p->bound && p->cur != 0) return fail("change the integrator between steps");
+  p->integrator = nstages; p->u[2] = u_c;
   return 0;
 }
 extern "C" int orc_set_flux_correction(orc_pack* p, int on) { if (!p) return fail("null pack"); p->flux_correction = on != 0; return 0; }
@@ -497,14 +506,21 @@ static void correct_coarse_fluxes(const orc_pack* p, std::vector<FaceFlux>& F) {
 
 extern "C" int orc_hydro_stage(orc_pack* p, int stage, double dt) {
   if (!p || !p->bound) return fail("pack not bound");
-  if (stage != 1 && stage != 2) return fail("stage must be 1 or 2");
-  if (stage == 1 && p->cur != 0) return fail("stage 1 expects U^n in buffer A");
-  if (stage == 2 && p->cur != 1) return fail("stage 2 expects U^(1) in buffer B");
-  // SSPRK(2,2): U1 = U^n + dt L(U^n);  U^{n+1} = 1/2 U^n + 1/2 [U1 + dt L(U1)]
-  const double g0 = (stage == 1) ? 0.0 : 0.5, g1 = (stage == 1) ? 1.0 : 0.5, beta = (stage == 1) ? 1.0 : 0.5;
+  if (stage < 1 || stage > p->integrator) return fail("stage out of range for the integrator");
+  if (p->cur != stage - 1) return fail("stages must be called in order, starting from U^n in buffer A");
+  // Shu-Osher forms (P:105 names the family; coefficients: SURVEY Q1 and, for three stages, Q27), every
+  // stage  U_out = g0 U_in + g1 U^n + beta dt L(U_in):
+  //   SSPRK(2,2): U1 = U^n + dt L(U^n);  U^{n+1} = 1/2 U^n + 1/2 [U1 + dt L(U1)]
+  //   SSPRK(3,3): U1 = U^n + dt L(U^n);  U2 = 3/4 U^n + 1/4 [U1 + dt L(U1)];  U^{n+1} = 1/3 U^n + 2/3 [U2 + dt L(U2)]
+  static const double C2[2][3] = { { 0.0, 1.0, 1.0 }, { 0.5, 0.5, 0.5 } };
+  static const double C3[3][3] = { { 0.0, 1.0, 1.0 }, { 0.25, 0.75, 0.25 }, { 2.0 / 3.0, 1.0 / 3.0, 2.0 / 3.0 } };
+  const double* cf = (p->integrator == 2) ? C2[stage - 1] : C3[stage - 1];
+  const double g0 = cf[0], g1 = cf[1], beta = cf[2];
   const double* Uin = p->u[p->cur];
   const double* U0 = p->u[0];
-  double* Uout = p->u[1 - p->cur];          // stage 2 writes A in place: each cell's A value is read only for itself
+  // the last stage writes A in place (each cell's A value is read only for itself); the others write the next buffer
+  const int out = (stage == p->integrator) ? 0 : stage;
+  double* Uout = p->u[out];
   long long nfl = 0;
   if (p->flux_correction && p->max_level > 0) {
     // all fluxes first, then the coarse faces at level boundaries are replaced, then every block is advanced
@@ -523,7 +539,7 @@ extern "C" int orc_hydro_stage(orc_pack* p, int stage, double dt) {
     }
   }
   p->floor_count += nfl;
-  p->cur = 1 - p->cur;
+  p->cur = out;
   return 0;
 }
 

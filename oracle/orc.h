@@ -47,7 +47,9 @@ int orc_set_threads(orc_pack*, int nthreads);
 /* f1: replace the coarse flux at level-boundary faces by the mean of the four fine fluxes.  Off by default. */
 int orc_set_flux_correction(orc_pack*, int on);
 int orc_fill_ghosts(orc_pack*);                           /* G1-G4 on the current buffer           */
-int orc_hydro_stage(orc_pack*, int stage, double dt);     /* S1-S4; stage 1: A->B, stage 2: B,A->A */
+int orc_hydro_stage(orc_pack*, int stage, double dt);     /* S1-S4; stage 1: A->B, stage 2: B,A->A (RK3: B,A->C; C,A->A) */
+/* f2: number of stages, 2 = SSPRK(2,2) (default) or 3 = SSPRK(3,3), which needs a third caller-owned buffer u_c. */
+int orc_set_integrator(orc_pack*, int nstages, double* u_c);
 int orc_new_dt(orc_pack*, double cfl, double* dt_out);    /* S0 on the current buffer              */
 double* orc_pack_current(orc_pack*);
 long long orc_pack_floor_count(const orc_pack*);

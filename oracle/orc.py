@@ -41,6 +41,7 @@ def lib():
     L.orc_pack_set_boundaries.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
     L.orc_set_threads.argtypes = [C.c_void_p, C.c_int]
     L.orc_set_flux_correction.argtypes = [C.c_void_p, C.c_int]
+    L.orc_set_integrator.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
     L.orc_fill_ghosts.argtypes = [C.c_void_p]
     L.orc_hydro_stage.argtypes = [C.c_void_p, C.c_int, C.c_double]
     L.orc_new_dt.argtypes = [C.c_void_p, C.c_double, dp]
@@ -147,6 +148,12 @@ class OrcPack:
         if threads != 1:
             _chk(L.orc_set_threads(self._h, threads))
 
+    def set_integrator(self, nstages):
+        """2 = SSPRK(2,2) (default), 3 = SSPRK(3,3) (allocates the third register)."""
+        self.nstages = nstages
+        self.uc = np.zeros(self.mesh.state_shape(), dtype=np.float64) if nstages == 3 else None
+        _chk(lib().orc_set_integrator(self._h, nstages, self.uc.ctypes.data if nstages == 3 else None))
+
     def set_flux_correction(self, on=True):
         """f1 of SURVEY 8(f): coarse fluxes at level-boundary faces <- mean of the four fine fluxes (off by default)."""
         _chk(lib().orc_set_flux_correction(self._h, 1 if on else 0))
@@ -158,6 +165,8 @@ class OrcPack:
 
     def current(self):
         p = lib().orc_pack_current(self._h)
+        if getattr(self, "uc", None) is not None and p == self.uc.ctypes.data:
+            return self.uc
         return self.ua if p == self.ua.ctypes.data else self.ub
 
     def fill_ghosts(self):
@@ -175,10 +184,10 @@ class OrcPack:
         return lib().orc_pack_floor_count(self._h)
 
     def step(self, cfl, dt=None):
-        """One RK2 step in the call order of SURVEY section 3: dt; 2 x (fill, stage).  Returns dt."""
+        """One RK step in the call order of SURVEY section 3: dt; nstages x (fill, stage).  Returns dt."""
         if dt is None:
             dt = self.new_dt(cfl)
-        for stage in (1, 2):
+        for stage in range(1, getattr(self, "nstages", 2) + 1):
             self.fill_ghosts()
             self.hydro_stage(stage, dt)
         return dt
