@@ -167,6 +167,8 @@ def run_ours(args):
                    variant=args.variant)
     if args.flux_correction:
         pack.set_flux_correction(True)
+    if args.integrator == 3:
+        pack.set_integrator(3)
     U0 = w.state(device=dev)
     pack.load(U0)
     ncell = mesh.ncells_active
@@ -189,7 +191,7 @@ def run_ours(args):
     e0.record(pack.stream)
     for _ in range(args.steps):
         dt = pack.new_dt(w.cfl)
-        for stage in (1, 2):
+        for stage in range(1, args.integrator + 1):
             pack.fill_ghosts()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(pack.stream)
@@ -205,9 +207,11 @@ def run_ours(args):
     value = aggregate_value(ncell, args.steps, elapsed_ms, world)
 
     # dominant kernel = the stage kernel: algorithmic bytes per launch / mean launch duration
-    st_ms = {s: statistics.mean(a.elapsed_time(b) for ss, a, b in stage_ev if ss == s) for s in (1, 2)}
-    stage_ms = 0.5 * (st_ms[1] + st_ms[2])
-    alg_bytes = 0.5 * (BYTES_STAGE[1] + BYTES_STAGE[2]) * ncell
+    nst = args.integrator
+    st_ms = {s: statistics.mean(a.elapsed_time(b) for ss, a, b in stage_ev if ss == s) for s in range(1, nst + 1)}
+    stage_ms = sum(st_ms.values()) / nst
+    # stage 1 moves 80 B per cell, every later stage (which also reads U^n) 120 B
+    alg_bytes = (BYTES_STAGE[1] + (nst - 1) * BYTES_STAGE[2]) / nst * ncell
     peaks, which = measured_peaks()
     achieved = alg_bytes / (stage_ms * 1e-3) / 1e9
     traffic = args.traffic
@@ -215,7 +219,7 @@ def run_ours(args):
         traffic = NCU_DRAM_BYTES_PER_STAGE_LAUNCH_CFG3
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "peak_source": which + " (MEASURED_PEAKS.json hbm_gbs)",
-                "kernel": "ak_hydro_stage", "kernel_ms": stage_ms, "kernel_share_of_step": 2 * stage_ms * args.steps / elapsed_ms,
+                "kernel": "ak_hydro_stage", "kernel_ms": stage_ms, "kernel_share_of_step": nst * stage_ms * args.steps / elapsed_ms,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "whole_step": {"achieved": BYTES_PER_CELL_UPDATE * value / world / 1e9,
                                "frac": BYTES_PER_CELL_UPDATE * value / world / 1e9 / peaks["hbm_gbs"]}}
@@ -257,7 +261,7 @@ def run_ours(args):
             "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{args.workload}: {w.name}", "nmb": mesh.nmb, "nx": list(mesh.nx), "ng": mesh.ng,
-                       "recon": "PPM4" if w.recon else "PLM", "rsolver": args.rsolver.upper(), "integrator": "SSPRK2", "cfl": w.cfl,
+                       "recon": "PPM4" if w.recon else "PLM", "rsolver": args.rsolver.upper(), "integrator": "SSPRK2" if args.integrator == 2 else "SSPRK3", "cfl": w.cfl,
                        "cells": ncell, "state_bytes": state_bytes, "l2_policy": "inputs larger than L2 (no flush needed)"
                        if state_bytes > 4e8 else "state fits L2: numbers are L2-resident", "variant": args.variant, "flux_correction": bool(args.flux_correction),
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
@@ -281,6 +285,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--rsolver", default="hllc", choices=["hllc", "llf", "hlle"],
                     help="Riemann solver (headline metric: hllc; llf / hlle are the f2 variants on the same kernel)")
+    ap.add_argument("--integrator", type=int, default=2, choices=[2, 3],
+                    help="stages per step: 2 = SSPRK(2,2) (headline), 3 = SSPRK(3,3) (f2 variant, third state register)")
     ap.add_argument("--flux-correction", action="store_true",
                     help="refined meshes (cfg4): flux correction at coarse-fine faces on (SURVEY 8(f) f1; off by default)")
     ap.add_argument("--traffic", type=float, default=None,

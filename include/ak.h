@@ -124,6 +124,13 @@ long long ak_pack_floor_count(ak_pack*);
  * AK_EINVAL for any other value. */
 int ak_pack_set_variant(ak_pack*, int variant);
 
+/* Time integrator (paper P:105: low-storage SSP Runge-Kutta schemes): nstages = 2 selects
+ * SSPRK(2,2) (default, two registers), nstages = 3 SSPRK(3,3), which needs a third caller-owned device buffer u_c
+ * of ak_pack_state_bytes() (256-byte aligned; ignored for nstages = 2).  Stages are then ak_hydro_stage(p, 1..3, dt):
+ * stage 1 A -> B, stage 2 B (and U^n in A) -> C, stage 3 C (and A) -> A.  Call on a bound pack between steps
+ * (AK_ESTATE otherwise).  SSPRK(3,3) runs in the production kernel only (AK_EUNSUPPORTED with other variants). */
+int ak_pack_set_integrator(ak_pack*, int nstages, void* u_c);
+
 /* Boundary condition per domain face, in the order x1min, x1max, x2min, x2max, x3min, x3max (paper P:67; SURVEY
  * 8(f) f3): 0 = periodic (default), 1 = outflow (ghost <- nearest active cell), 2 = reflect (ghost <- mirror image
  * across the face, normal momentum negated).  Periodic faces come in pairs (AK_EINVAL otherwise).  Call before

@@ -23,7 +23,7 @@ RSOLVER_HLLC, RSOLVER_LLF, RSOLVER_HLLE = 0, 1, 2
 SYMBOLS = [
     "ak_last_error", "ak_pack_create", "ak_pack_set_mesh", "ak_pack_set_block", "ak_pack_state_bytes",
     "ak_pack_scratch_bytes", "ak_pack_bind", "ak_fill_ghosts", "ak_hydro_stage", "ak_new_dt", "ak_step",
-    "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_floor_count", "ak_pack_set_variant", "ak_pack_set_tile", "ak_pack_set_flux_correction", "ak_pack_set_boundaries",
+    "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_floor_count", "ak_pack_set_variant", "ak_pack_set_tile", "ak_pack_set_flux_correction", "ak_pack_set_boundaries", "ak_pack_set_integrator",
     "ak_pack_launch_count", "ak_pack_destroy",
 ]
 
@@ -61,6 +61,7 @@ def lib():
         "ak_pack_set_tile": (i, [vp, i]),
         "ak_pack_set_flux_correction": (i, [vp, i]),
         "ak_pack_set_boundaries": (i, [vp, C.POINTER(C.c_int)]),
+        "ak_pack_set_integrator": (i, [vp, i, vp]),
         "ak_pack_launch_count": (ll, [vp]),
         "ak_pack_destroy": (i, [vp]),
     }
@@ -119,7 +120,16 @@ class Pack:
 
     def current(self) -> torch.Tensor:
         p = lib().ak_pack_current(self._h)
+        if getattr(self, "uc", None) is not None and p == self.uc.data_ptr():
+            return self.uc
         return self.ua if p == self.ua.data_ptr() else self.ub
+
+    def set_integrator(self, nstages):
+        """2 = SSPRK(2,2) (default), 3 = SSPRK(3,3): allocates the third state register."""
+        with torch.cuda.device(self.device):
+            self.uc = torch.zeros(self.mesh.state_shape(), dtype=torch.float64, device=self.device) if nstages == 3 else None
+        _chk(lib().ak_pack_set_integrator(self._h, nstages, self.uc.data_ptr() if nstages == 3 else None))
+        self.nstages = nstages
 
     def upload(self, host_tensor):
         """ak_pack_upload: HOST (ideally pinned) tensor -> buffer A through the C-ABI."""

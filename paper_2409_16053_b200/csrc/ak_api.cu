@@ -193,6 +193,23 @@ extern "C" int ak_pack_set_variant(ak_pack* p, int variant) {
   return AK_OK;
 }
 
+extern "C" int ak_pack_set_integrator(ak_pack* p, int nstages, void* u_c) {
+  if (!p) return fail(AK_EINVAL, "null pack");
+  if (nstages != 2 && nstages != 3) return fail(AK_EINVAL, "integrator must be 2 (SSPRK(2,2)) or 3 (SSPRK(3,3))");
+  if (nstages == 3) {
+    if (!u_c) return fail(AK_EINVAL, "SSPRK(3,3) needs a third state buffer");
+    if ((uintptr_t)u_c & 255) return fail(AK_EINVAL, "buffers must be 256-byte aligned");
+    if (!p->bound) return fail(AK_ESTATE, "bind the pack first");
+    if (u_c == (void*)p->u[0] || u_c == (void*)p->u[1]) return fail(AK_EINVAL, "device buffers overlap");
+  }
+  if (p->bound && p->cur != 0) return fail(AK_ESTATE, "change the integrator between steps");
+  p->integrator = nstages;
+  p->u[2] = (nstages == 3) ? (double*)u_c : nullptr;
+  p->tmap_box[0] = p->tmap_box[1] = 0;          // tensor maps are rebuilt over all bound buffers
+  p->tmap0_box[0] = p->tmap0_box[1] = 0;
+  return AK_OK;
+}
+
 extern "C" int ak_pack_set_boundaries(ak_pack* p, const int bc[6]) {
   if (!p || !bc) return fail(AK_EINVAL, "null argument");
   for (int f = 0; f < 6; f++) if (bc[f] < 0 || bc[f] > 2) return fail(AK_EINVAL, "unknown boundary condition");
@@ -226,18 +243,25 @@ extern "C" int ak_fill_ghosts(ak_pack* p) {
 
 extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
-  if (stage != 1 && stage != 2) return fail(AK_EINVAL, "stage must be 1 or 2");
+  if (stage < 1 || stage > p->integrator) return fail(AK_EINVAL, "stage must be 1 .. number of stages of the integrator");
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(AK_EINVAL, "dt must be positive and finite");
-  if (stage == 1 && p->cur != 0) return fail(AK_ESTATE, "stage 1 expects U^n in buffer A (call stage 2 first)");
-  if (stage == 2 && p->cur != 1) return fail(AK_ESTATE, "stage 2 expects U^(1) in buffer B (call stage 1 first)");
+  if (p->cur != stage - 1)
+    return fail(AK_ESTATE, stage == 1 ? "stage 1 expects U^n in buffer A (finish the previous step first)"
+                                      : "stages must be called in order (the previous stage's result is not current)");
   if (!p->ghosts_ok) return fail(AK_ESTATE, "ak_fill_ghosts must precede ak_hydro_stage");
   if (p->rsolver != AK_RSOLVER_HLLC && (p->variant != 0 || ((p->d.ng - (p->recon == 0 ? 2 : 3)) & 1)))
     return fail(AK_EUNSUPPORTED, "LLF / HLLE exist in the production kernel only (variant 0, ng - stencil radius even)");
-  // SSPRK(2,2) in two registers (Q1): (g0, g1, beta) = (0,1,1) then (1/2,1/2,1/2)
+  // Shu-Osher forms, every stage U_out = g0 U_in + g1 U^n + beta dt L(U_in) (Q1, Q27):
+  //   SSPRK(2,2): (0,1,1), (1/2,1/2,1/2);   SSPRK(3,3): (0,1,1), (1/4,3/4,1/4), (2/3,1/3,2/3)
+  static const double C2[2][3] = {{0.0, 1.0, 1.0}, {0.5, 0.5, 0.5}};
+  static const double C3[3][3] = {{0.0, 1.0, 1.0}, {0.25, 0.75, 0.25}, {2.0 / 3.0, 1.0 / 3.0, 2.0 / 3.0}};
+  const double* cf = (p->integrator == 2) ? C2[stage - 1] : C3[stage - 1];
   ak::StageCoef sc;
-  const double beta = (stage == 1) ? 1.0 : 0.5;
-  sc.g0 = (stage == 1) ? 0.0 : 0.5;
-  sc.g1 = (stage == 1) ? 1.0 : 0.5;
+  const double beta = cf[2];
+  sc.g0 = cf[0];
+  sc.g1 = cf[1];
+  // the last stage writes A in place (a cell's A value is read only by its own thread); the others the next buffer
+  const int out = (stage == p->integrator) ? 0 : stage;
   for (int lev = 0; lev < 2; lev++)
     for (int d = 0; d < 3; d++) {
       double dx = (p->xmax[d] - p->xmin[d]) / ((double)p->d.nrb[d] * p->d.nx[d] * (double)(1 << lev));
@@ -245,17 +269,20 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
     }
   // stage 2 of the production kernel also leaves the max signal speeds of U^{n+1} for the next ak_new_dt
   const bool v3 = p->variant == 0 && !((p->d.ng - (p->recon == 0 ? 2 : 3)) & 1);
+  if (p->integrator == 3 && !v3) return fail(AK_EUNSUPPORTED, "SSPRK(3,3) exists in the production kernel only");
+  const bool last = stage == p->integrator;
+  sc.take_dt = (last && stage >= 2) ? 1 : 0;
   p->dt_cached = false;
-  if (stage == 2 && v3) AK_CUDA(cudaMemsetAsync(p->d.smax_bits, 0, 48, p->stream), "reset signal speeds");
-  AK_CUDA(ak::launch_stage(*p, p->u[p->cur], p->u[0], p->u[1 - p->cur], sc), "ak_hydro_stage launch");
+  if (sc.take_dt && v3) AK_CUDA(cudaMemsetAsync(p->d.smax_bits, 0, 48, p->stream), "reset signal speeds");
+  AK_CUDA(ak::launch_stage(*p, p->u[p->cur], p->u[0], p->u[out], sc), "ak_hydro_stage launch");
   p->launches += ak::stage_launches_per_call(*p);
-  if (stage == 2 && v3) p->dt_cached = true;
+  if (last && v3) p->dt_cached = true;
   if (p->flux_correction && p->d.max_level > 0) {
-    AK_CUDA(ak::launch_flux_correction(*p, p->u[p->cur], p->u[1 - p->cur], sc), "flux correction launch");
+    AK_CUDA(ak::launch_flux_correction(*p, p->u[p->cur], p->u[out], sc), "flux correction launch");
     p->launches += 3;
     p->dt_cached = false;               // the correction changed cells after their signal speeds were taken
   }
-  p->cur = 1 - p->cur;
+  p->cur = out;
   p->ghosts_ok = false;
   return AK_OK;
 }
@@ -291,7 +318,7 @@ extern "C" int ak_new_dt(ak_pack* p, double cfl, double* dt_out) {
 extern "C" int ak_step(ak_pack* p, double cfl, double dt_fixed, double* dt_out) {
   double dt = dt_fixed;
   if (!(dt_fixed > 0.0)) { int rc = ak_new_dt(p, cfl, &dt); if (rc) return rc; }
-  for (int stage = 1; stage <= 2; stage++) {
+  for (int stage = 1; stage <= p->integrator; stage++) {
     int rc = ak_fill_ghosts(p); if (rc) return rc;
     rc = ak_hydro_stage(p, stage, dt); if (rc) return rc;
   }

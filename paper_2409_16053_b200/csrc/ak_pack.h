@@ -36,6 +36,7 @@ struct PackDev {
 struct StageCoef {
   double g0, g1;            // weights of U_in and U0
   double c[2][3];           // beta*dt/dx_d for level 0 and 1
+  int take_dt;              // last stage of a step: also reduce the signal speeds of the result
 };
 
 }  // namespace ak
@@ -48,7 +49,8 @@ struct ak_pack {
   bool dt_cached = false;         // smax_bits describe the current state (set by stage 2 of the production kernel)
   std::vector<int> level, lx;     // lx[3m+d]
   std::vector<char> blk_set;
-  double* u[2] = {nullptr, nullptr};
+  double* u[3] = {nullptr, nullptr, nullptr};   // A (U^n at the start of a step), B, C (third register, RK3 only)
+  int integrator = 2;                           // stages per step: 2 = SSPRK(2,2), 3 = SSPRK(3,3)
   void* scratch = nullptr;
   cudaStream_t stream = nullptr;
   int cur = 0;
@@ -59,10 +61,10 @@ struct ak_pack {
   long long launches = 0;
   int sm_count = 148;
   // tensor maps over u[0], u[1] for the TMA stage kernel, rebuilt when the staging box changes
-  mutable CUtensorMap tmap[2];
+  mutable CUtensorMap tmap[3];
   mutable int tmap_box[2] = {0, 0};
   // ... and the halo-free U0 boxes of the v3 kernel's stage 2
-  mutable CUtensorMap tmap0[2];
+  mutable CUtensorMap tmap0[3];
   mutable int tmap0_box[2] = {0, 0};
 };
 

@@ -267,7 +267,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
       double un[5];
 #pragma unroll
       for (int n = 0; n < 5; n++) { un[n] = fma(-c3, Gn[n] - G[n], Tc[n * NT]); o[n * nc] = un[n]; }
-      if constexpr (STAGE2) {
+      if (STAGE2 && sc.take_dt) {                  // (uniform over the grid)
         // S0 of the NEXT step (Eq.(3)) on U^{n+1} while it is in registers: the cell's signal speeds
         // |v_d| + c_s in the oracle's arithmetic (IEEE division and sqrt, no contraction: this translation unit
         // is compiled with -fmad=false), so that ak_new_dt need not read the state again
@@ -344,7 +344,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
     dslot = (dslot + 1 == NS) ? 0 : dslot + 1;
   }
   if (nfl) atomicAdd(P.floor_cnt, (unsigned long long)nfl);
-  if constexpr (STAGE2) {
+  if (STAGE2 && sc.take_dt) {
     // positive doubles order like their bit patterns: warp max by shuffles, one atomicMax per warp and direction
 #pragma unroll
     for (int d = 0; d < 3; d++) {
@@ -362,17 +362,17 @@ cudaError_t launch_v3(const ak_pack& p, const double* Uin, const double* U0, dou
   using S = V3Tile<RECON, TI, TJ>;
   const PackDev& P = p.d;
   if (p.tmap_box[0] != S::WI || p.tmap_box[1] != S::WJ) {
-    for (int b = 0; b < 2; b++)
-      if (!make_state_tmap(&p.tmap[b], p.u[b], P.nmb, P.nt, S::WI, S::WJ)) return cudaErrorNotSupported;
+    for (int b = 0; b < 3; b++)
+      if (p.u[b] && !make_state_tmap(&p.tmap[b], p.u[b], P.nmb, P.nt, S::WI, S::WJ)) return cudaErrorNotSupported;
     p.tmap_box[0] = S::WI; p.tmap_box[1] = S::WJ;
   }
   if (p.tmap0_box[0] != S::W0 || p.tmap0_box[1] != TJ) {
-    for (int b = 0; b < 2; b++)
-      if (!make_state_tmap(&p.tmap0[b], p.u[b], P.nmb, P.nt, S::W0, TJ)) return cudaErrorNotSupported;
+    for (int b = 0; b < 3; b++)
+      if (p.u[b] && !make_state_tmap(&p.tmap0[b], p.u[b], P.nmb, P.nt, S::W0, TJ)) return cudaErrorNotSupported;
     p.tmap0_box[0] = S::W0; p.tmap0_box[1] = TJ;
   }
-  const CUtensorMap& tm = (Uin == p.u[0]) ? p.tmap[0] : p.tmap[1];
-  const CUtensorMap& tm0 = (U0 == p.u[0]) ? p.tmap0[0] : p.tmap0[1];
+  const CUtensorMap& tm = (Uin == p.u[0]) ? p.tmap[0] : (Uin == p.u[1] ? p.tmap[1] : p.tmap[2]);
+  const CUtensorMap& tm0 = (U0 == p.u[0]) ? p.tmap0[0] : (U0 == p.u[1] ? p.tmap0[1] : p.tmap0[2]);
   const size_t smem = S::bytes;
   auto k1 = stage_v3_kernel<RECON, RS, TI, TJ, MINB, false>;
   auto k2 = stage_v3_kernel<RECON, RS, TI, TJ, MINB, true>;

@@ -524,3 +524,60 @@ def test_dt_from_stage2_is_bit_identical_to_the_reduction_over_the_state(orc, ak
         po.close()
         pg.upload(pg.current().cpu().contiguous())          # invalidates the cache: the reduction kernel runs
         assert pg.new_dt(w.cfl) == dt_fused and pg.launch_count() == l0 + 2
+
+
+# ------------------------------------------------------------ SSPRK(3,3) --------
+@pytest.mark.parametrize("which", ["cfg3", "cfg1", "smr_fc"])
+def test_rk3_matches_the_oracle(orc, ak, which):
+    """Three-stage integrator with the third register: the paper's showcased RK3 + PPM4 + HLLC combination on
+    the config-3 recipe, PLM on config 1, and the two-level mesh with flux correction; dt from the fused reduction
+    of the LAST stage is bit-identical to the oracle's reduction over the GPU state."""
+    w = {"cfg3": lambda: I.config3(nrb=2, nx=32), "cfg1": lambda: I.config1(nrb=2, nx=32), "smr_fc": lambda: I.smr_parity(nx=16)}[which]()
+    U0 = w.state()
+    po, pg = P.make_pair(orc, ak, w, U0)
+    po.set_integrator(3); pg.set_integrator(3)
+    if which == "smr_fc":
+        po.set_flux_correction(True); pg.set_flux_correction(True)
+    a = P.active(w.mesh)
+    for step in range(4):
+        dt = po.new_dt(w.cfl)
+        dt_g = pg.new_dt(w.cfl)
+        assert abs(dt_g - dt) <= 1e-13 * dt
+        for stage in (1, 2, 3):
+            po.fill_ghosts(); pg.fill_ghosts()
+            po.hydro_stage(stage, dt); pg.hydro_stage(stage, dt)
+            if step == 0:
+                e = P.q14(P.gpu_state(pg)[a], po.current()[a], w.gamma)
+                assert e <= TOL_STAGE * stage, f"stage {stage}: Q14 = {e:.3e}"
+        chk = orc.OrcPack(w.mesh, w.gamma, w.recon, threads=P.NTHREADS)
+        chk.load(P.gpu_state(pg))
+        l0 = pg.launch_count()
+        assert pg.new_dt(w.cfl) == chk.new_dt(w.cfl)
+        if which != "smr_fc":
+            assert pg.launch_count() == l0                  # taken from the last stage, no launch
+        chk.close()
+    assert P.q14(P.gpu_state(pg)[a], po.current()[a], w.gamma) <= TOL_RUN
+    check_totals(w, U0, po, pg)
+    assert pg.floor_count() == 0
+    with pytest.raises(ak.AkError):
+        pg.hydro_stage(2, 1e-3)                             # stage 1 first
+
+
+def test_rk3_through_ak_step_and_integrator_errors(orc, ak):
+    w = I.config1(nrb=2, nx=16)
+    U0 = w.state()
+    po, pg = P.make_pair(orc, ak, w, U0)
+    po.set_integrator(3); pg.set_integrator(3)
+    for _ in range(3):
+        dt = po.new_dt(w.cfl)
+        po.step(w.cfl, dt); pg.step(w.cfl, dt)
+    a = P.active(w.mesh)
+    assert P.q14(P.gpu_state(pg)[a], po.current()[a], w.gamma) <= TOL_RUN
+    pv = ak.Pack(w.mesh, w.gamma, w.recon, variant=1)
+    pv.set_integrator(3)
+    pv.load(U0)
+    pv.fill_ghosts()
+    with pytest.raises(ak.AkError):
+        pv.hydro_stage(1, 1e-3)                             # the cross-check kernels are two-stage only
+    L = ak.lib()
+    assert L.ak_pack_set_integrator(pg._h, 4, None) == -1 and L.ak_pack_set_integrator(pg._h, 3, None) == -1
