@@ -245,10 +245,25 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
     }
     // x3: plane c = s-(R-1) becomes reconstructible; its lower face flux completes plane c-1
     double qm3[5], qpn[5];
+    if constexpr (RECON == 0) {                    // the five reciprocal seeds in flight together (as in B)
+      double prod[5], r[5], den[5];
+#pragma unroll
+      for (int n = 0; n < 5; n++) {
+        const double dL = wk[1][n] - wk[0][n], dR = wp[n] - wk[1][n];
+        prod[n] = dL * dR; den[n] = dL + dR;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r[n]) : "d"(den[n]));
+      }
+#pragma unroll
+      for (int n = 0; n < 5; n++) {
+        const double e = fma(-den[n], r[n], 1.0);
+        const double q = prod[n] * fma(r[n], fma(e, e, e), r[n]);
+        const double h = pos(prod[n]) ? q : 0.0;
+        qm3[n] = wk[1][n] - h; qpn[n] = wk[1][n] + h;
+      }
+    }
 #pragma unroll
     for (int n = 0; n < 5; n++) {
       if constexpr (RECON == 0) {
-        plm_lean(wk[0][n], wk[1][n], wp[n], qm3[n], qpn[n]);
       } else {
         double hi = iface_lean(wk[0][n], wk[1][n], wk[2][n], wp[n]);
         double lo = qlow[n];
@@ -304,14 +319,40 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
     // ---- B(s) --------------------------------------------------------------------------------------
     double qm1[5], qm2[5];
     if (inplane && valid) {
+      if constexpr (RECON == 0) {
+        // PLM: the five variables of one direction in lock step, so that the five reciprocal seeds (MUFU, long
+        // latency) are in flight together instead of one per dependency chain
 #pragma unroll
-      for (int n = 0; n < 5; n++) {
-        const double* p = Ws + n * (WJ * WI) + oW;
-        double qp;
-        recon2<RECON>(p, 1, qm1[n], qp);
-        Q1[n * (TJ * (TI + 1)) + oQ1 + 1] = qp;
-        recon2<RECON>(p, WI, qm2[n], qp);
-        Q2[n * ((TJ + 1) * TI) + oQ2 + TI] = qp;
+        for (int d = 0; d < 2; d++) {
+          const int st = d ? WI : 1;
+          double c[5], prod[5], r[5], den[5];
+#pragma unroll
+          for (int n = 0; n < 5; n++) {
+            const double* p = Ws + n * (WJ * WI) + oW;
+            c[n] = p[0];
+            const double dL = c[n] - p[-st], dR = p[st] - c[n];
+            prod[n] = dL * dR; den[n] = dL + dR;
+            asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r[n]) : "d"(den[n]));
+          }
+#pragma unroll
+          for (int n = 0; n < 5; n++) {
+            const double e = fma(-den[n], r[n], 1.0);
+            const double q = prod[n] * fma(r[n], fma(e, e, e), r[n]);     // = div2(prod, den), same operations
+            const double h = pos(prod[n]) ? q : 0.0;
+            if (d == 0) { qm1[n] = c[n] - h; Q1[n * (TJ * (TI + 1)) + oQ1 + 1] = c[n] + h; }
+            else        { qm2[n] = c[n] - h; Q2[n * ((TJ + 1) * TI) + oQ2 + TI] = c[n] + h; }
+          }
+        }
+      } else {
+#pragma unroll
+        for (int n = 0; n < 5; n++) {
+          const double* p = Ws + n * (WJ * WI) + oW;
+          double qp;
+          recon2<RECON>(p, 1, qm1[n], qp);
+          Q1[n * (TJ * (TI + 1)) + oQ1 + 1] = qp;
+          recon2<RECON>(p, WI, qm2[n], qp);
+          Q2[n * ((TJ + 1) * TI) + oQ2 + TI] = qp;
+        }
       }
     }
     cta_sync(NTH);                                      // q+ visible; every read of W(s) is done
