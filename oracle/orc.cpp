@@ -161,6 +161,42 @@ extern "C" void orc_hlle(double gamma, int dir, const double WL[5], const double
   unrotate(dir, Fn, F);
 }
 
+// Roe's linearised solver ("as well as Roe's linearized solver"; Toro 2013 ch.11, restated): Roe averages as for
+// HLLE; eigenvalues l1 = u~ - c~, l2,3,4 = u~, l5 = u~ + c~; wave strengths from dU = U_R - U_L:
+//   a3 = dU3 - v~ dU1,  a4 = dU4 - w~ dU1,  dU5' = dU5 - a3 v~ - a4 w~,
+//   a2 = (gamma-1)/c~^2 [dU1 (H~ - u~^2) + u~ dU2 - dU5'],  a1 = [dU1 (u~ + c~) - dU2 - c~ a2] / (2 c~),  a5 = dU1 - (a1 + a2);
+// right eigenvectors K1 = (1, u~-c~, v~, w~, H~-u~c~), K2 = (1, u~, v~, w~, |v~|^2/2), K3 = (0,0,1,0,v~), K4 = (0,0,0,1,w~),
+// K5 = (1, u~+c~, v~, w~, H~+u~c~);  F = 1/2 (F_L + F_R) - 1/2 sum_k a_k |l_k| K_k.  No entropy fix, no fallback (Q28).
+extern "C" void orc_roe(double gamma, int dir, const double WL[5], const double WR[5], double F[5]) {
+  double UL[5], UR[5], FL[5], FR[5], cL, cR, Fn[5];
+  rotated_states(gamma, dir, WL, UL, FL, &cL);
+  rotated_states(gamma, dir, WR, UR, FR, &cR);
+  const double gm1 = gamma - 1.0;
+  const double sL = std::sqrt(WL[0]), sR = std::sqrt(WR[0]), isum = 1.0 / (sL + sR);
+  const double uL = UL[1] / UL[0], vL = UL[2] / UL[0], wL = UL[3] / UL[0];
+  const double uR = UR[1] / UR[0], vR = UR[2] / UR[0], wR = UR[3] / UR[0];
+  const double HL = (UL[4] + gm1 * WL[4]) / UL[0], HR = (UR[4] + gm1 * WR[4]) / UR[0];
+  const double ut = (sL * uL + sR * uR) * isum, vt = (sL * vL + sR * vR) * isum, wt = (sL * wL + sR * wR) * isum;
+  const double Ht = (sL * HL + sR * HR) * isum;
+  const double q2 = ut * ut + (vt * vt + wt * wt);
+  const double c2 = gm1 * (Ht - 0.5 * q2), ct = std::sqrt(c2);
+  double dU[5];
+  for (int n = 0; n < 5; n++) dU[n] = UR[n] - UL[n];
+  const double a3 = dU[2] - vt * dU[0], a4 = dU[3] - wt * dU[0];
+  const double dU5 = dU[4] - a3 * vt - a4 * wt;
+  const double a2 = gm1 / c2 * (dU[0] * (Ht - ut * ut) + ut * dU[1] - dU5);
+  const double a1 = (dU[0] * (ut + ct) - dU[1] - ct * a2) / (2.0 * ct);
+  const double a5 = dU[0] - (a1 + a2);
+  const double l1 = std::fabs(ut - ct), l2 = std::fabs(ut), l5 = std::fabs(ut + ct);
+  const double K1[5] = { 1.0, ut - ct, vt, wt, Ht - ut * ct }, K2[5] = { 1.0, ut, vt, wt, 0.5 * q2 };
+  const double K3[5] = { 0.0, 0.0, 1.0, 0.0, vt }, K4[5] = { 0.0, 0.0, 0.0, 1.0, wt }, K5[5] = { 1.0, ut + ct, vt, wt, Ht + ut * ct };
+  for (int n = 0; n < 5; n++) {
+    const double diss = (a1 * l1) * K1[n] + ((a2 * l2) * K2[n] + ((a3 * l2) * K3[n] + ((a4 * l2) * K4[n] + (a5 * l5) * K5[n])));
+    Fn[n] = 0.5 * ((FL[n] + FR[n]) - diss);
+  }
+  unrotate(dir, Fn, F);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Pack descriptor
 // ------------------------------------------------------------------------------------------------
@@ -201,7 +237,7 @@ extern "C" orc_pack* orc_pack_create(int nmb, int nx1, int nx2, int nx3, int ng,
   for (int d = 0; d < 3; d++) if (nx[d] < ng || (nx[d] & 1)) { fail("nx_d must be even and >= ng"); return nullptr; }
   if (!(gamma > 1.0)) { fail("gamma <= 1"); return nullptr; }
   if (recon != 0 && recon != 1) { fail("unknown recon"); return nullptr; }
-  if (rsolver < 0 || rsolver > 2) { fail("unknown rsolver"); return nullptr; }
+  if (rsolver < 0 || rsolver > 3) { fail("unknown rsolver"); return nullptr; }
   if ((recon == 0 && ng < 2) || (recon == 1 && ng < 3)) { fail("ng too small for the reconstruction"); return nullptr; }
   orc_pack* p = new orc_pack;
   p->nmb = nmb; p->ng = ng; p->gamma = gamma; p->recon = recon; p->rsolver = rsolver;
@@ -432,7 +468,8 @@ static long long block_fluxes(const orc_pack* p, const double* Uin, int m, FaceF
       }
       if (p->rsolver == 0) orc_hllc(p->gamma, d, WL, WR, Fl);
       else if (p->rsolver == 1) orc_llf(p->gamma, d, WL, WR, Fl);
-      else orc_hlle(p->gamma, d, WL, WR, Fl);
+      else if (p->rsolver == 2) orc_hlle(p->gamma, d, WL, WR, Fl);
+      else orc_roe(p->gamma, d, WL, WR, Fl);
       for (int n = 0; n < 5; n++) F[d][n * nc + c] = Fl[n];
     }
   }

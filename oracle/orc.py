@@ -61,7 +61,7 @@ def lib():
     L.orc_ppm4_iface.restype = None
     L.orc_hllc.argtypes = [C.c_double, C.c_int, dp, dp, dp]
     L.orc_hllc.restype = None
-    for f in (L.orc_llf, L.orc_hlle):
+    for f in (L.orc_llf, L.orc_hlle, L.orc_roe):
         f.argtypes = [C.c_double, C.c_int, dp, dp, dp]
         f.restype = None
     _lib = L
@@ -116,6 +116,12 @@ def hllc(gamma, direction, WL, WR):
 def llf(gamma, direction, WL, WR):
     F = (C.c_double * 5)()
     lib().orc_llf(gamma, direction, _arr5(WL), _arr5(WR), F)
+    return np.array(F[:])
+
+
+def roe(gamma, direction, WL, WR):
+    F = (C.c_double * 5)()
+    lib().orc_roe(gamma, direction, _arr5(WL), _arr5(WR), F)
     return np.array(F[:])
 
 
