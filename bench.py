@@ -163,7 +163,7 @@ def run_ours(args):
 
     w = workloads()[args.workload]()
     mesh = w.mesh
-    pack = ak.Pack(mesh, w.gamma, w.recon, rsolver={"hllc": 0, "llf": 1, "hlle": 2}[args.rsolver], device=dev,
+    pack = ak.Pack(mesh, w.gamma, w.recon, rsolver={"hllc": 0, "llf": 1, "hlle": 2, "roe": 3}[args.rsolver], device=dev,
                    variant=args.variant)
     if args.flux_correction:
         pack.set_flux_correction(True)
@@ -283,7 +283,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--rsolver", default="hllc", choices=["hllc", "llf", "hlle"],
+    ap.add_argument("--rsolver", default="hllc", choices=["hllc", "llf", "hlle", "roe"],
                     help="Riemann solver (headline metric: hllc; llf / hlle are the f2 variants on the same kernel)")
     ap.add_argument("--integrator", type=int, default=2, choices=[2, 3],
                     help="stages per step: 2 = SSPRK(2,2) (headline), 3 = SSPRK(3,3) (f2 variant, third state register)")

@@ -40,6 +40,7 @@ extern "C" {
 #define AK_RSOLVER_HLLC 0     /* P:103                                          */
 #define AK_RSOLVER_LLF  1     /* P:103 (SURVEY 8(f) f2): Rusanov, a = max(|u|+c) of the two states            */
 #define AK_RSOLVER_HLLE 2     /* P:103 (SURVEY 8(f) f2): Einfeldt speeds from the Roe averages                */
+#define AK_RSOLVER_ROE  3     /* P:103 (SURVEY 8(f) f2): Roe's linearised solver, no entropy fix               */
 
 typedef struct ak_pack ak_pack;          /* opaque host-side descriptor */
 

@@ -18,7 +18,7 @@ _lib = None
 
 AK_OK = 0
 RECON_PLM, RECON_PPM4 = 0, 1
-RSOLVER_HLLC, RSOLVER_LLF, RSOLVER_HLLE = 0, 1, 2
+RSOLVER_HLLC, RSOLVER_LLF, RSOLVER_HLLE, RSOLVER_ROE = 0, 1, 2, 3
 
 SYMBOLS = [
     "ak_last_error", "ak_pack_create", "ak_pack_set_mesh", "ak_pack_set_block", "ak_pack_state_bytes",

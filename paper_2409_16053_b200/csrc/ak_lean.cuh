@@ -262,12 +262,42 @@ __device__ __forceinline__ void hlle2(const GasConst& g, const double WL[5], con
   for (int n = 0; n < 5; n++) F[n] = (fma(bp, FL[n], -(bm * FR[n])) + bb * (UR[n] - UL[n])) * inv;
 }
 
-// solver chosen at compile time: RS = 0 HLLC, 1 LLF, 2 HLLE
+// Roe's linearised solver (Toro 2013 ch.11; Q28): Roe averages as in hlle2, wave strengths from dU,
+// F = 1/2 (F_L + F_R) - 1/2 sum_k a_k |l_k| K_k; no entropy fix
+__device__ __forceinline__ void roe2(const GasConst& g, const double WL[5], const double WR[5], double F[5]) {
+  double UL[5], UR[5], FL[5], FR[5], cL, cR, pL, pR;
+  state_flux(g, WL, UL, FL, cL, pL);
+  state_flux(g, WR, UR, FR, cR, pR);
+  const double sL = sqrt_ratio(WL[0], 1.0), sR = sqrt_ratio(WR[0], 1.0), isum = rcp2(sL + sR);
+  const double HL = (UL[4] + pL) * rcp2(WL[0]), HR = (UR[4] + pR) * rcp2(WR[0]);
+  const double ut = fma(sL, WL[1], sR * WR[1]) * isum, vt = fma(sL, WL[2], sR * WR[2]) * isum;
+  const double wt = fma(sL, WL[3], sR * WR[3]) * isum, Ht = fma(sL, HL, sR * HR) * isum;
+  const double q2 = fma(ut, ut, fma(vt, vt, wt * wt));
+  const double c2 = g.gm1 * fma(-0.5, q2, Ht), ct = sqrt_ratio(c2, 1.0), ic = rcp2(ct);
+  double dU[5];
+#pragma unroll
+  for (int n = 0; n < 5; n++) dU[n] = UR[n] - UL[n];
+  const double a3 = fma(-vt, dU[0], dU[2]), a4 = fma(-wt, dU[0], dU[3]);
+  const double dU5 = fma(-a4, wt, fma(-a3, vt, dU[4]));
+  const double a2 = (g.gm1 * (ic * ic)) * (fma(dU[0], fma(-ut, ut, Ht), ut * dU[1]) - dU5);
+  const double a1 = (fma(dU[0], ut + ct, -dU[1]) - ct * a2) * (0.5 * ic);
+  const double a5 = dU[0] - (a1 + a2);
+  const double w1 = a1 * fabs(ut - ct), l2 = fabs(ut), w2 = a2 * l2, w3 = a3 * l2, w4 = a4 * l2, w5 = a5 * fabs(ut + ct);
+  const double uc = ut * ct;
+  F[0] = 0.5 * ((FL[0] + FR[0]) - (w1 + (w2 + w5)));
+  F[1] = 0.5 * ((FL[1] + FR[1]) - fma(w1, ut - ct, fma(w2, ut, w5 * (ut + ct))));
+  F[2] = 0.5 * ((FL[2] + FR[2]) - fma(w1 + (w2 + w5), vt, w3));
+  F[3] = 0.5 * ((FL[3] + FR[3]) - fma(w1 + (w2 + w5), wt, w4));
+  F[4] = 0.5 * ((FL[4] + FR[4]) - fma(w1, Ht - uc, fma(w2, 0.5 * q2, fma(w3, vt, fma(w4, wt, w5 * (Ht + uc))))));
+}
+
+// solver chosen at compile time: RS = 0 HLLC, 1 LLF, 2 HLLE, 3 Roe
 template <int RS>
 __device__ __forceinline__ void riemann2(const GasConst& g, const double l[5], const double r[5], double f[5]) {
   if constexpr (RS == 0) hllc2(g, l, r, f);
   else if constexpr (RS == 1) llf2(g, l, r, f);
-  else hlle2(g, l, r, f);
+  else if constexpr (RS == 2) hlle2(g, l, r, f);
+  else roe2(g, l, r, f);
 }
 template <int RS, int D>
 __device__ __forceinline__ void flux3(const GasConst& g, const double L[5], const double Rr[5], double F[5]) {

@@ -61,6 +61,7 @@ static cudaError_t launch_stage_v3_rs(const ak_pack& p, const double* Uin, const
   switch (p.rsolver) {
     case 1:  return launch_stage_v3<RECON, 1>(p, Uin, U0, Uout, sc);
     case 2:  return launch_stage_v3<RECON, 2>(p, Uin, U0, Uout, sc);
+    case 3:  return launch_stage_v3<RECON, 3>(p, Uin, U0, Uout, sc);
     default: return launch_stage_v3<RECON, 0>(p, Uin, U0, Uout, sc);
   }
 }
@@ -80,6 +81,7 @@ cudaError_t launch_flux_correction(const ak_pack& p, const double* Uin, double* 
   switch (p.rsolver) {
     case 1:  return p.recon == 0 ? launch_flux_correction_t<0, 1>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 1>(p, Uin, Uout, sc);
     case 2:  return p.recon == 0 ? launch_flux_correction_t<0, 2>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 2>(p, Uin, Uout, sc);
+    case 3:  return p.recon == 0 ? launch_flux_correction_t<0, 3>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 3>(p, Uin, Uout, sc);
     default: return p.recon == 0 ? launch_flux_correction_t<0, 0>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 0>(p, Uin, Uout, sc);
   }
 }

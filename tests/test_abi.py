@@ -44,7 +44,7 @@ def test_create_rejects_bad_arguments(L):
         (1, 8, 8, 8, 2, 5 / 3, 1, 0),      # ng too small for PPM4
         (1, 8, 8, 8, 2, 1.0, 0, 0),        # gamma <= 1
         (1, 8, 8, 8, 2, 5 / 3, 7, 0),      # unknown recon
-        (1, 8, 8, 8, 2, 5 / 3, 0, 3),      # unknown rsolver
+        (1, 8, 8, 8, 2, 5 / 3, 0, 4),      # unknown rsolver
         (1, 2, 8, 8, 3, 5 / 3, 1, 0),      # nx < ng
     ]
     for args in bad:

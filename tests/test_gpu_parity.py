@@ -413,7 +413,7 @@ def test_flux_correction_keeps_uniform_state_bit_exact_on_gpu(ak):
 
 
 # ------------------------------------------------------------ LLF / HLLE --------
-@pytest.mark.parametrize("rsolver", [1, 2])
+@pytest.mark.parametrize("rsolver", [1, 2, 3])
 def test_llf_and_hlle_match_the_oracle(orc, ak, rsolver):
     """Same kernel skeleton, other two-state solver: PLM on the config-1 recipe and on ragged blocks, PPM4 on the
     config-3 recipe, the SMR mesh with structure on the level boundaries and flux correction on."""
