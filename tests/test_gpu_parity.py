@@ -186,7 +186,8 @@ def test_smr_with_structure_on_level_boundaries(orc, ak):
     ((1, 2, 1), (6, 2, 4), 2, I.RECON_PLM),
     ((3, 1, 2), (34, 10, 6), 2, I.RECON_PLM),      # ragged: not a multiple of any tile size
     ((1, 1, 1), (130, 18, 10), 3, I.RECON_PPM4),   # longer than one 128-wide tile row
-    ((1, 1, 1), (16, 16, 16), 4, I.RECON_PPM4),    # more ghosts than the stencil needs
+    ((1, 1, 1), (16, 16, 16), 4, I.RECON_PPM4),    # more ghosts than the stencil needs (odd surplus: LDG-staged kernel)
+    ((1, 1, 2), (16, 12, 8), 4, I.RECON_PLM),      # more ghosts than the stencil needs (even surplus: TMA-staged kernel)
 ])
 @pytest.mark.parametrize("variant", [0, 1])
 def test_ragged_and_degenerate_blocks(orc, ak, nrb, nx, ng, recon, variant):
