@@ -84,21 +84,27 @@ int ak_pack_bind(ak_pack*, void* u_a, void* u_b, void* scratch, void* cuda_strea
  * writes ghost cells only; bit-exact against the oracle.  Asynchronous on the stream. */
 int ak_fill_ghosts(ak_pack*);
 
-/* One Runge-Kutta stage of SSP-RK2 in two registers:
+/* One Runge-Kutta stage.  Default integrator, SSP-RK2 in two registers:
  *   stage 1:  B = A - dt L(A)-terms            (reads A, writes B, B becomes current)
  *   stage 2:  A = 1/2 A + 1/2 (B + dt L(B))    (reads B and A, writes A, A becomes current)
- * with L = -sum_d (F_d(i+1/2) - F_d(i-1/2))/dx_d, F from conserved->primitive, PLM/PPM4
+ * (SSPRK(3,3) after ak_pack_set_integrator: stages 1..3, A -> B -> C -> A.)  Stages are called in order, starting
+ * with U^n in buffer A (AK_ESTATE otherwise; AK_EINVAL for a stage number the integrator does not have).
+ * With L = -sum_d (F_d(i+1/2) - F_d(i-1/2))/dx_d, F from conserved->primitive, PLM/PPM4
  * reconstruction of the primitives and the HLLC flux in x1, x2, x3, fused in one
- * launch; face fluxes never reach device memory.  Requires ak_fill_ghosts on the current buffer
- * since the last change (else AK_ESTATE).  Asynchronous on the stream. */
+ * launch; face fluxes never reach device memory.  The Riemann solver is the one given to ak_pack_create (HLLC, LLF,
+ * HLLE or Roe).  The last stage of a step also reduces the signal speeds of its result for the next ak_new_dt.
+ * Requires ak_fill_ghosts on the current buffer since the last change (else AK_ESTATE).  Asynchronous on the
+ * stream. */
 int ak_hydro_stage(ak_pack*, int stage, double dt);
 
 /* CFL time step, Eq.(3): cfl * min over active cells of all blocks and over d of
  * dx_d(level) / (|v_d| + c_s), one dt for all levels.  dt_out is a HOST pointer.
- * Synchronises the stream. */
+ * Synchronises the stream.  After a complete step the answer comes from the maxima the last stage left behind
+ * (48 bytes copied, no launch); otherwise a reduction kernel reads the state.  Both give the same bits. */
 int ak_new_dt(ak_pack*, double cfl, double* dt_out);
 
-/* Convenience: ak_new_dt, then 2 x (ak_fill_ghosts, ak_hydro_stage).  dt_out (HOST, may be NULL)
+/* Convenience: ak_new_dt, then (ak_fill_ghosts, ak_hydro_stage) for every stage of the integrator (2 by default,
+ * 3 after ak_pack_set_integrator(p, 3, u_c)).  dt_out (HOST, may be NULL)
  * receives the step taken.  If dt_fixed > 0 it is used instead of the CFL value (lock-step parity
  * runs) and no reduction is launched. */
 int ak_step(ak_pack*, double cfl, double dt_fixed, double* dt_out);
