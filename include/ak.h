@@ -135,7 +135,9 @@ int ak_pack_set_variant(ak_pack*, int variant);
  * SSPRK(2,2) (default, two registers), nstages = 3 SSPRK(3,3), which needs a third caller-owned device buffer u_c
  * of ak_pack_state_bytes() (256-byte aligned; ignored for nstages = 2).  Stages are then ak_hydro_stage(p, 1..3, dt):
  * stage 1 A -> B, stage 2 B (and U^n in A) -> C, stage 3 C (and A) -> A.  Call on a bound pack between steps
- * (AK_ESTATE otherwise).  SSPRK(3,3) runs in the production kernel only (AK_EUNSUPPORTED with other variants). */
+ * (AK_ESTATE otherwise).  nstages = 1 is forward Euler ("RK1"): every ak_hydro_stage(p, 1, dt) is a whole step from
+ * the current buffer into the other one (A and B alternate; u_c ignored).  Integrators other than the default run in
+ * the production kernel only (AK_EUNSUPPORTED with other variants). */
 int ak_pack_set_integrator(ak_pack*, int nstages, void* u_c);
 
 /* Boundary condition per domain face, in the order x1min, x1max, x2min, x2max, x3min, x3max (paper P:67; SURVEY

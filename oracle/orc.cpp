@@ -306,9 +306,10 @@ extern "C" int orc_pack_set_boundaries(orc_pack* p, const int bc[6]) {
 }
 extern "C" int orc_set_integrator(orc_pack* p, int nstages, double* u_c) {
   if (!p) return fail("null pack");
-  if (nstages != 2 && nstages != 3) return fail("integrator must be 2 (SSPRK(2,2)) or 3 (SSPRK(3,3))");
+  if (nstages < 1 || nstages > 3) return fail("integrator must be 1 (forward Euler), 2 (SSPRK(2,2)) or 3 (SSPRK(3,3))");
   if (nstages == 3 && !u_c) return fail("SSPRK(3,3) needs a third state buffer");
-  if (p->bound && p->cur != 0) return fail("change the integrator between steps");
+  if (p->bound && p->cur != 0 && !(p->integrator == 1 && p->cur == 1)) return fail("change the integrator between steps");
+  if (p->bound && p->cur == 1 && nstages != 1) return fail("after an odd number of forward-Euler steps U^n is in buffer B: take one more or reload");
   p->integrator = nstages; p->u[2] = u_c;
   return 0;
 }
@@ -544,7 +545,10 @@ static void correct_coarse_fluxes(const orc_pack* p, std::vector<FaceFlux>& F) {
 extern "C" int orc_hydro_stage(orc_pack* p, int stage, double dt) {
   if (!p || !p->bound) return fail("pack not bound");
   if (stage < 1 || stage > p->integrator) return fail("stage out of range for the integrator");
-  if (p->cur != stage - 1) return fail("stages must be called in order, starting from U^n in buffer A");
+  if (p->integrator == 1) {
+    // RK1 (forward Euler, "RK1 through RK4"): U^{n+1} = U^n + dt L(U^n); the two registers alternate
+    if (p->cur > 1) return fail("forward Euler alternates between buffers A and B");
+  } else if (p->cur != stage - 1) return fail("stages must be called in order, starting from U^n in buffer A");
   // Shu-Osher forms (P:105 names the family; coefficients: SURVEY Q1 and, for three stages, Q27), every
   // stage  U_out = g0 U_in + g1 U^n + beta dt L(U_in):
   //   SSPRK(2,2): U1 = U^n + dt L(U^n);  U^{n+1} = 1/2 U^n + 1/2 [U1 + dt L(U1)]
@@ -554,9 +558,10 @@ extern "C" int orc_hydro_stage(orc_pack* p, int stage, double dt) {
   const double* cf = (p->integrator == 2) ? C2[stage - 1] : C3[stage - 1];
   const double g0 = cf[0], g1 = cf[1], beta = cf[2];
   const double* Uin = p->u[p->cur];
-  const double* U0 = p->u[0];
-  // the last stage writes A in place (each cell's A value is read only for itself); the others write the next buffer
-  const int out = (stage == p->integrator) ? 0 : stage;
+  const double* U0 = (p->integrator == 1) ? Uin : p->u[0];
+  // the last stage writes A in place (each cell's A value is read only for itself); the others write the next buffer;
+  // forward Euler has no second register to combine with and writes the other buffer
+  const int out = (p->integrator == 1) ? 1 - p->cur : ((stage == p->integrator) ? 0 : stage);
   double* Uout = p->u[out];
   long long nfl = 0;
   if (p->flux_correction && p->max_level > 0) {

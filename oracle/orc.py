@@ -155,10 +155,10 @@ class OrcPack:
             _chk(L.orc_set_threads(self._h, threads))
 
     def set_integrator(self, nstages):
-        """2 = SSPRK(2,2) (default), 3 = SSPRK(3,3) (allocates the third register)."""
-        self.nstages = nstages
-        self.uc = np.zeros(self.mesh.state_shape(), dtype=np.float64) if nstages == 3 else None
-        _chk(lib().orc_set_integrator(self._h, nstages, self.uc.ctypes.data if nstages == 3 else None))
+        """1 = forward Euler, 2 = SSPRK(2,2) (default), 3 = SSPRK(3,3) (allocates the third register)."""
+        uc = np.zeros(self.mesh.state_shape(), dtype=np.float64) if nstages == 3 else None
+        _chk(lib().orc_set_integrator(self._h, nstages, uc.ctypes.data if nstages == 3 else None))
+        self.nstages, self.uc = nstages, uc
 
     def set_flux_correction(self, on=True):
         """f1 of SURVEY 8(f): coarse fluxes at level-boundary faces <- mean of the four fine fluxes (off by default)."""

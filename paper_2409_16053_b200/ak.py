@@ -125,11 +125,11 @@ class Pack:
         return self.ua if p == self.ua.data_ptr() else self.ub
 
     def set_integrator(self, nstages):
-        """2 = SSPRK(2,2) (default), 3 = SSPRK(3,3): allocates the third state register."""
+        """1 = forward Euler, 2 = SSPRK(2,2) (default), 3 = SSPRK(3,3): allocates the third state register."""
         with torch.cuda.device(self.device):
-            self.uc = torch.zeros(self.mesh.state_shape(), dtype=torch.float64, device=self.device) if nstages == 3 else None
-        _chk(lib().ak_pack_set_integrator(self._h, nstages, self.uc.data_ptr() if nstages == 3 else None))
-        self.nstages = nstages
+            uc = torch.zeros(self.mesh.state_shape(), dtype=torch.float64, device=self.device) if nstages == 3 else None
+        _chk(lib().ak_pack_set_integrator(self._h, nstages, uc.data_ptr() if nstages == 3 else None))
+        self.nstages, self.uc = nstages, uc
 
     def upload(self, host_tensor):
         """ak_pack_upload: HOST (ideally pinned) tensor -> buffer A through the C-ABI."""

@@ -195,14 +195,16 @@ extern "C" int ak_pack_set_variant(ak_pack* p, int variant) {
 
 extern "C" int ak_pack_set_integrator(ak_pack* p, int nstages, void* u_c) {
   if (!p) return fail(AK_EINVAL, "null pack");
-  if (nstages != 2 && nstages != 3) return fail(AK_EINVAL, "integrator must be 2 (SSPRK(2,2)) or 3 (SSPRK(3,3))");
+  if (nstages < 1 || nstages > 3) return fail(AK_EINVAL, "integrator must be 1 (forward Euler), 2 (SSPRK(2,2)) or 3 (SSPRK(3,3))");
   if (nstages == 3) {
     if (!u_c) return fail(AK_EINVAL, "SSPRK(3,3) needs a third state buffer");
     if ((uintptr_t)u_c & 255) return fail(AK_EINVAL, "buffers must be 256-byte aligned");
     if (!p->bound) return fail(AK_ESTATE, "bind the pack first");
     if (u_c == (void*)p->u[0] || u_c == (void*)p->u[1]) return fail(AK_EINVAL, "device buffers overlap");
   }
-  if (p->bound && p->cur != 0) return fail(AK_ESTATE, "change the integrator between steps");
+  if (p->bound && p->cur != 0 && !(p->integrator == 1 && p->cur == 1)) return fail(AK_ESTATE, "change the integrator between steps");
+  if (p->bound && p->cur == 1 && nstages != 1)
+    return fail(AK_ESTATE, "after an odd number of forward-Euler steps U^n is in buffer B: take one more or reload");
   p->integrator = nstages;
   p->u[2] = (nstages == 3) ? (double*)u_c : nullptr;
   p->tmap_box[0] = p->tmap_box[1] = 0;          // tensor maps are rebuilt over all bound buffers
@@ -245,7 +247,7 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
   if (stage < 1 || stage > p->integrator) return fail(AK_EINVAL, "stage must be 1 .. number of stages of the integrator");
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(AK_EINVAL, "dt must be positive and finite");
-  if (p->cur != stage - 1)
+  if (p->integrator == 1 ? p->cur > 1 : p->cur != stage - 1)
     return fail(AK_ESTATE, stage == 1 ? "stage 1 expects U^n in buffer A (finish the previous step first)"
                                       : "stages must be called in order (the previous stage's result is not current)");
   if (!p->ghosts_ok) return fail(AK_ESTATE, "ak_fill_ghosts must precede ak_hydro_stage");
@@ -261,7 +263,9 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
   sc.g0 = cf[0];
   sc.g1 = cf[1];
   // the last stage writes A in place (a cell's A value is read only by its own thread); the others the next buffer
-  const int out = (stage == p->integrator) ? 0 : stage;
+  // (forward Euler has no second register to combine with: it writes the other buffer, A and B alternate)
+  const int out = (p->integrator == 1) ? 1 - p->cur : ((stage == p->integrator) ? 0 : stage);
+  const double* u0 = (p->integrator == 1) ? p->u[p->cur] : p->u[0];
   for (int lev = 0; lev < 2; lev++)
     for (int d = 0; d < 3; d++) {
       double dx = (p->xmax[d] - p->xmin[d]) / ((double)p->d.nrb[d] * p->d.nx[d] * (double)(1 << lev));
@@ -269,14 +273,14 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
     }
   // stage 2 of the production kernel also leaves the max signal speeds of U^{n+1} for the next ak_new_dt
   const bool v3 = p->variant == 0 && !((p->d.ng - (p->recon == 0 ? 2 : 3)) & 1);
-  if (p->integrator == 3 && !v3) return fail(AK_EUNSUPPORTED, "SSPRK(3,3) exists in the production kernel only");
+  if (p->integrator != 2 && !v3) return fail(AK_EUNSUPPORTED, "forward Euler and SSPRK(3,3) exist in the production kernel only");
   const bool last = stage == p->integrator;
   sc.take_dt = (last && stage >= 2) ? 1 : 0;
   p->dt_cached = false;
   if (sc.take_dt && v3) AK_CUDA(cudaMemsetAsync(p->d.smax_bits, 0, 48, p->stream), "reset signal speeds");
-  AK_CUDA(ak::launch_stage(*p, p->u[p->cur], p->u[0], p->u[out], sc), "ak_hydro_stage launch");
+  AK_CUDA(ak::launch_stage(*p, p->u[p->cur], u0, p->u[out], sc), "ak_hydro_stage launch");
   p->launches += ak::stage_launches_per_call(*p);
-  if (last && v3) p->dt_cached = true;
+  if (sc.take_dt && v3) p->dt_cached = true;
   if (p->flux_correction && p->d.max_level > 0) {
     AK_CUDA(ak::launch_flux_correction(*p, p->u[p->cur], p->u[out], sc), "flux correction launch");
     p->launches += 3;

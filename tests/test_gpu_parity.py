@@ -582,3 +582,19 @@ def test_rk3_through_ak_step_and_integrator_errors(orc, ak):
         pv.hydro_stage(1, 1e-3)                             # the cross-check kernels are two-stage only
     L = ak.lib()
     assert L.ak_pack_set_integrator(pg._h, 4, None) == -1 and L.ak_pack_set_integrator(pg._h, 3, None) == -1
+
+
+def test_forward_euler_matches_the_oracle(orc, ak):
+    w = I.config1(nrb=2, nx=16)
+    U0 = w.state()
+    po, pg = P.make_pair(orc, ak, w, U0)
+    po.set_integrator(1); pg.set_integrator(1)
+    a = P.active(w.mesh)
+    for step in range(5):
+        dt = 0.5 * po.new_dt(w.cfl)
+        assert abs(0.5 * pg.new_dt(w.cfl) - dt) <= 1e-13 * dt
+        po.step(w.cfl, dt); pg.step(w.cfl, dt)
+        assert P.q14(P.gpu_state(pg)[a], po.current()[a], w.gamma) <= TOL_STAGE * (step + 1)
+    assert pg.current().data_ptr() == pg.ub.data_ptr()          # five steps: the registers alternate
+    with pytest.raises(ak.AkError):
+        pg.set_integrator(2)

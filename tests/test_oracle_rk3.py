@@ -26,8 +26,8 @@ def _setup():
 def _run(orc, mesh, U0, nstages, nsteps, T=0.05):
     p = orc.OrcPack(mesh, I.GAMMA, I.RECON_PLM)
     p.load(U0)
-    if nstages == 3:
-        p.set_integrator(3)
+    if nstages != 2:
+        p.set_integrator(nstages)
     for _ in range(nsteps):
         p.step(0.3, T / nsteps)
     return p.current()[P.active(mesh)].copy()
@@ -40,6 +40,27 @@ def test_temporal_order_on_a_fixed_grid(orc):
     assert 3.7 <= err[2][8] / err[2][16] <= 4.3 and 3.7 <= err[2][16] / err[2][32] <= 4.3, err
     assert 6.5 <= err[3][8] / err[3][16] <= 8.5 and 5.5 <= err[3][16] / err[3][32] <= 8.5, err
     assert err[3][8] < err[2][8] / 5 and err[3][32] < err[2][32] / 15, err
+
+
+def test_forward_euler_is_first_order_and_alternates_the_registers(orc):
+    """RK1 of the paper's list: error to the tiny-dt reference halves with dt; A and B alternate."""
+    mesh, U0 = _setup()
+    ref = _run(orc, mesh, U0, 3, 1024)
+    e = {k: np.abs(_run(orc, mesh, U0, 1, k) - ref).max() for k in (16, 32, 64)}
+    assert 1.9 <= e[16] / e[32] <= 2.2 and 1.9 <= e[32] / e[64] <= 2.2, e
+    p = orc.OrcPack(mesh, I.GAMMA, I.RECON_PLM)
+    p.load(U0)
+    p.set_integrator(1)
+    p.step(0.3, 1e-3)
+    assert p.current() is p.ub
+    t0, t1 = P.totals(mesh, U0), P.totals(mesh, p.current())
+    assert abs(t1[0] - t0[0]) <= 1e-14 * t0[0] and abs(t1[4] - t0[4]) <= 1e-14 * t0[4]
+    import pytest
+    with pytest.raises(orc.OrcError):
+        p.set_integrator(2)                 # U^n sits in B after an odd number of Euler steps
+    p.step(0.3, 1e-3)
+    assert p.current() is p.ua
+    p.set_integrator(2)
 
 
 def test_rk3_conserves_and_keeps_a_uniform_state_to_round_off(orc):
