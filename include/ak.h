@@ -118,6 +118,10 @@ void* ak_pack_current(const ak_pack*);
  * download: current buffer -> HOST, synchronises the stream. */
 int ak_pack_upload(ak_pack*, const void* host_u);
 int ak_pack_download(ak_pack*, void* host_u);
+/* As ak_pack_download without the synchronisation: the copy is only enqueued on the pack's stream (pinned host
+ * memory makes it asynchronous); the caller synchronises the stream before reading host_u.  Lets two packs on two
+ * streams overlap one pack's download with the other's upload and compute (bench.py e2e_pipelined). */
+int ak_pack_download_async(ak_pack*, void* host_u);
 
 /* Number of density / internal-energy floor activations in conserved->primitive since bind
  * (diagnostic; 0 on all BASELINE configs).  Synchronises the stream.  Negative on error. */

@@ -23,7 +23,7 @@ RSOLVER_HLLC, RSOLVER_LLF, RSOLVER_HLLE, RSOLVER_ROE = 0, 1, 2, 3
 SYMBOLS = [
     "ak_last_error", "ak_pack_create", "ak_pack_set_mesh", "ak_pack_set_block", "ak_pack_state_bytes",
     "ak_pack_scratch_bytes", "ak_pack_bind", "ak_fill_ghosts", "ak_hydro_stage", "ak_new_dt", "ak_step",
-    "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_floor_count", "ak_pack_set_variant", "ak_pack_set_tile", "ak_pack_set_flux_correction", "ak_pack_set_boundaries", "ak_pack_set_integrator",
+    "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_download_async", "ak_pack_floor_count", "ak_pack_set_variant", "ak_pack_set_tile", "ak_pack_set_flux_correction", "ak_pack_set_boundaries", "ak_pack_set_integrator",
     "ak_pack_launch_count", "ak_pack_destroy",
 ]
 
@@ -56,6 +56,7 @@ def lib():
         "ak_pack_current": (vp, [vp]),
         "ak_pack_upload": (i, [vp, vp]),
         "ak_pack_download": (i, [vp, vp]),
+        "ak_pack_download_async": (i, [vp, vp]),
         "ak_pack_floor_count": (ll, [vp]),
         "ak_pack_set_variant": (i, [vp, i]),
         "ak_pack_set_tile": (i, [vp, i]),
@@ -135,6 +136,10 @@ class Pack:
         """ak_pack_upload: HOST (ideally pinned) tensor -> buffer A through the C-ABI."""
         assert host_tensor.device.type == "cpu" and host_tensor.is_contiguous() and host_tensor.dtype == torch.float64
         _chk(lib().ak_pack_upload(self._h, host_tensor.data_ptr()))
+
+    def download_async(self, host_tensor):
+        assert host_tensor.device.type == "cpu" and host_tensor.is_contiguous() and host_tensor.dtype == torch.float64
+        _chk(lib().ak_pack_download_async(self._h, host_tensor.data_ptr()))
 
     def download(self, host_tensor):
         assert host_tensor.device.type == "cpu" and host_tensor.is_contiguous() and host_tensor.dtype == torch.float64

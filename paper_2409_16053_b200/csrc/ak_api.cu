@@ -340,6 +340,13 @@ extern "C" int ak_pack_upload(ak_pack* p, const void* host_u) {
   return AK_OK;
 }
 
+extern "C" int ak_pack_download_async(ak_pack* p, void* host_u) {
+  if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  if (!host_u) return fail(AK_EINVAL, "null host buffer");
+  AK_CUDA(cudaMemcpyAsync(host_u, p->u[p->cur], ak_pack_state_bytes(p), cudaMemcpyDeviceToHost, p->stream), "ak_pack_download_async");
+  return AK_OK;
+}
+
 extern "C" int ak_pack_download(ak_pack* p, void* host_u) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
   if (!host_u) return fail(AK_EINVAL, "null host buffer");
