@@ -598,3 +598,47 @@ def test_forward_euler_matches_the_oracle(orc, ak):
     assert pg.current().data_ptr() == pg.ub.data_ptr()          # five steps: the registers alternate
     with pytest.raises(ak.AkError):
         pg.set_integrator(2)
+
+
+@pytest.mark.parametrize("nx", [16, 128])
+def test_config2_full_size_sampled(orc, ak, nx):
+    """BASELINE config 2 at its full 256^3, at the two ends of the block-size sweep (4096 blocks of 16^3: every
+    sampled box spans 8-27 MeshBlocks; 8 blocks of 128^3), as bench.py runs it: two RK2 steps on the GPU against the
+    oracle on 32^3 sub-boxes (PLM: a step reaches 2 x 2 cells, two steps 8 = the margin dropped on each side).  The
+    boxes sit on the blast (centre, edge of the hot sphere), on a block corner and on the periodic wrap."""
+    w = I.config2(nx)
+    dev = torch.device("cuda", 0)
+    pg = ak.Pack(w.mesh, w.gamma, w.recon, device=dev)
+    U0 = w.state(device=dev)
+    pg.load(U0)
+    G0 = _assemble(w.mesh, U0)
+    del U0
+    n, pad = 32, 8
+    origins = [(112, 112, 112), (100, 118, 120), (240, 240, 240), (112, 112, 121), (0, 64, 200)]
+    subs0 = [_subbox(G0, o, n) for o in origins]
+    tot0 = G0.sum(dim=(1, 2, 3)).cpu().numpy()
+    del G0
+    dts = []
+    for _ in range(2):
+        dts.append(pg.new_dt(w.cfl))
+        pg.step(w.cfl, dts[-1])
+    assert pg.floor_count() == 0
+    G1 = _assemble(w.mesh, pg.current())
+    tot1 = G1.sum(dim=(1, 2, 3)).cpu().numpy()
+    assert abs(tot1[0] - tot0[0]) <= TOL_TOTALS * tot0[0] and abs(tot1[4] - tot0[4]) <= TOL_TOTALS * tot0[4]
+    dx = w.mesh.dx(0)
+    sub_mesh = I.Mesh((1, 1, 1), (n, n, n), w.mesh.ng, [(0, 0, 0, 0)], xmax=(n * dx[0], n * dx[1], n * dx[2]))
+    assert sub_mesh.dx(0) == dx
+    g = w.mesh.ng
+    for o, s0 in zip(origins, subs0):
+        po = orc.OrcPack(sub_mesh, w.gamma, w.recon, threads=1)
+        u = np.zeros(sub_mesh.state_shape())
+        u[0][:, g:-g, g:-g, g:-g] = s0
+        po.load(u)
+        for dt in dts:
+            po.step(w.cfl, dt)
+        ref = po.current()[0][:, g + pad:-g - pad, g + pad:-g - pad, g + pad:-g - pad]
+        got = _subbox(G1, o, n)[:, pad:-pad, pad:-pad, pad:-pad]
+        e = P.q14(got[None], ref[None], w.gamma)
+        assert e <= 4 * TOL_STAGE, (nx, o, e)
+        po.close()
