@@ -130,8 +130,9 @@ long long ak_pack_floor_count(ak_pack*);
 /* Selects the implementation of ak_hydro_stage (all of them CUDA kernels of this library; they give the
  * same results to rounding and exist as independent cross-checks for the tests):
  *   0 = production kernel: TMA-staged plane marching, worker threads + edge warp (default)
- *   1 = one thread per cell, recomputes everything        2 = tiled plane marching, LDG staging
- *   3 = first TMA-staged kernel                            4 = second generation (edge faces on warp 0)
+ *   1 = one thread per cell, recomputes everything (independent cross-check)
+ *   2 = tiled plane marching with LDG staging (also taken automatically when ng - stencil radius is odd, where
+ *       the TMA box origin would not be 16-byte aligned)
  * AK_EINVAL for any other value. */
 int ak_pack_set_variant(ak_pack*, int variant);
 

@@ -77,7 +77,13 @@ extern "C" void orc_ppm4(const double q[5], double* q_minus, double* q_plus) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// S3  HLLC flux at one face (Toro 2013 ch.10 restated in SURVEY 8(c) S3)
+// S3  HLLC flux at one face (P:103 names the solver; formulas: Toro 2013 ch.10, restated)
+// Wave speeds (Q2, round-2 reading): Davis's direct estimates, Toro Eq.(10.48),
+//   S_L = min(u_L - c_L, u_R - c_R),   S_R = max(u_L + c_L, u_R + c_R).
+// They bound the speeds of an isolated shock (Lax condition) and of both rarefaction heads, satisfy
+// S_L <= u_L - c_L and S_R >= u_R + c_R (Batten et al.'s condition for a positively conservative HLLC), and give
+// S_L < S* < S_R for every pair of states with positive pressure, so the star flux is finite for head-on
+// collisions at any Mach number (the pressure-based estimate of round 1 gave S_L > 0 > S_R and 0/0 there, Q26).
 // ------------------------------------------------------------------------------------------------
 extern "C" void orc_hllc(double gamma, int dir, const double WL[5], const double WR[5], double F[5]) {
   const int iu = 1 + dir, iv = 1 + (dir + 1) % 3, iw = 1 + (dir + 2) % 3;   // normal, transverse pair (cyclic)
@@ -86,12 +92,7 @@ extern "C" void orc_hllc(double gamma, int dir, const double WL[5], const double
   double rR = WR[0], uR = WR[iu], vR = WR[iv], wR = WR[iw], eR = WR[4];
   double pL = gm1 * eL, pR = gm1 * eR;
   double cL = std::sqrt(gamma * pL / rL), cR = std::sqrt(gamma * pR / rR);
-  double rbar = 0.5 * (rL + rR), cbar = 0.5 * (cL + cR);
-  double ppv = 0.5 * ((pL + pR) + (uL - uR) * rbar * cbar);                  // PVRS pressure estimate
-  const double gq = (gamma + 1.0) / (2.0 * gamma);
-  double qL = (ppv <= pL) ? 1.0 : std::sqrt(1.0 + gq * (ppv / pL - 1.0));
-  double qR = (ppv <= pR) ? 1.0 : std::sqrt(1.0 + gq * (ppv / pR - 1.0));
-  double SL = uL - cL * qL, SR = uR + cR * qR;
+  double SL = std::fmin(uL - cL, uR - cR), SR = std::fmax(uL + cL, uR + cR);
   double bm = std::fmin(SL, 0.0), bp = std::fmax(SR, 0.0);
   double mL = rL * (uL - SL), mR = rR * (SR - uR);
   double Ss = ((pL - pR) + (mL * uL + mR * uR)) / (mL + mR);                  // contact speed
@@ -593,7 +594,8 @@ extern "C" int orc_new_dt(orc_pack* p, double cfl, double* dt_out) {
   const double* U = p->u[p->cur];
   const int ng = p->ng;
   double dtmin = HUGE_VAL;
-#pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) reduction(min : dtmin) if (p->nthreads > 1)
+  long long bad = 0;      // cells whose signal speed is not a finite positive number (NaN / inf state): reported, not skipped
+#pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) reduction(min : dtmin) reduction(+ : bad) if (p->nthreads > 1)
   for (int m = 0; m < p->nmb; m++) {
     const int lev = p->level[m];
     for (int k = ng; k < p->nx[2] + ng; k++) for (int j = ng; j < p->nx[1] + ng; j++) for (int i = ng; i < p->nx[0] + ng; i++) {
@@ -603,11 +605,14 @@ extern "C" int orc_new_dt(orc_pack* p, double cfl, double* dt_out) {
       double pr = (p->gamma - 1.0) * w[4];
       double cs = std::sqrt(p->gamma * pr / w[0]);
       for (int d = 0; d < 3; d++) {
-        double cand = p->dx(lev, d) / (std::fabs(w[1 + d]) + cs);
+        double s = std::fabs(w[1 + d]) + cs;
+        if (!(s > 0.0 && s < HUGE_VAL)) { bad++; continue; }
+        double cand = p->dx(lev, d) / s;
         if (cand < dtmin) dtmin = cand;
       }
     }
   }
+  if (bad) return fail("non-finite signal speed in the state (NaN or inf)");
   *dt_out = cfl * dtmin;
   return 0;
 }

@@ -188,7 +188,7 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
 
 extern "C" int ak_pack_set_variant(ak_pack* p, int variant) {
   if (!p) return fail(AK_EINVAL, "null pack");
-  if (variant < 0 || variant > 4) return fail(AK_EINVAL, "unknown variant");
+  if (variant < 0 || variant > 2) return fail(AK_EINVAL, "unknown variant");
   p->variant = variant;
   return AK_OK;
 }

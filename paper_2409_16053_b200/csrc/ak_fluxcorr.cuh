@@ -12,8 +12,7 @@
 // launches in sequence keep its corrections in a fixed order, no atomics).
 #pragma once
 #include "ak_pack.h"
-#include "ak_lean.cuh"
-#include "ak_stage_v2.cuh"     // recon2<>
+#include "ak_lean.cuh"          // recon2<>, flux3<>
 
 namespace ak {
 
@@ -60,7 +59,7 @@ __global__ void __launch_bounds__(128) flux_correct_kernel(PackDev P, const doub
   const long long nc = P.ncell;
   const long long str[3] = {1, P.nt[0], (long long)P.nt[0] * P.nt[1]};
   GasConst g;
-  g.gamma = P.gamma; g.gm1 = P.gamma - 1.0; g.gq = (P.gamma + 1.0) / (2.0 * P.gamma);
+  g.gamma = P.gamma; g.gm1 = P.gamma - 1.0;
   g.ug_floor = P_FLOOR / (P.gamma - 1.0);
 
   const long long c = cc[2] * str[2] + cc[1] * str[1] + cc[0];

@@ -1,5 +1,5 @@
 // ak_lean.cuh -- branch-free, instruction-lean forms of the per-cell / per-face arithmetic for the
-// production stage kernel (ak_stage_v2.cuh).  Same formulas as ak_physics.cuh (DESIGN.md section 2
+// production stage kernel (ak_stage_v3.cuh).  Same formulas as ak_physics.cuh (DESIGN.md section 2
 // readings Q1-Q7; paper P:101 reconstruction on primitives, P:103 HLLC, P:122-126 gamma-law gas); they
 // differ from it by rounding only (a few ulp) and are written against what profiles/r01_v1_stage_cfg3.md
 // showed to be expensive on sm_100a:
@@ -80,6 +80,20 @@ __device__ __forceinline__ void limit_lean(double a, double& aL, double& aR) {
   aR = flat ? a : (cR ? nR : aR);
 }
 
+// q-/q+ of the cell at p[0] from the stencil along stride st: RECON 0 = PLM, 1 = PPM4
+template <int RECON>
+__device__ __forceinline__ void recon2(const double* p, int st, double& qm, double& qp) {
+  if constexpr (RECON == 0) {
+    plm_lean(p[-st], p[0], p[st], qm, qp);
+  } else {
+    const double m2 = p[-2 * st], m1 = p[-st], a = p[0], p1 = p[st], p2 = p[2 * st];
+    double lo = iface_lean(m2, m1, a, p1);
+    double hi = iface_lean(m1, a, p1, p2);
+    limit_lean(a, lo, hi);
+    qm = lo; qp = hi;
+  }
+}
+
 // sqrt(a / b) = a (a b)^(-1/2) for a, b > 0 without a division: MUFU seed r of t^(-1/2) (error e = 1 - t r^2
 // <= 2^-19) + ONE cubic (Halley) step r (1 + e/2 + 3 e^2/8), truncation 5/16 e^3 < 2^-58    7 FP64 + 1 MUFU
 __device__ __forceinline__ double sqrt_ratio(double a, double b) {
@@ -92,23 +106,18 @@ __device__ __forceinline__ double sqrt_ratio(double a, double b) {
 }
 
 // ---- S3  HLLC, rotated states (rho, u_normal, v, w, u_g) -------------------------------------------
-// Straight-line: the shock branch of the pressure-based wave speeds is folded into
-//   c_K q_K = sqrt(gamma (p_K + gq max(p_pvrs - p_K, 0)) / rho_K)
-// (equal to c_K where p_pvrs <= p_K), u_K - S_K is taken as c_K q_K, and the upwind side is chosen by the
-// sign of S*.  ~100 FP64-pipe instructions + 6 MUFU.
+// Wave speeds: Davis's direct estimates S_L = min(u_L - c_L, u_R - c_R), S_R = max(u_L + c_L, u_R + c_R) (Q2,
+// round-2 reading): always S_L < S* < S_R, so the star flux is finite for head-on collisions at any Mach number.
+// Straight-line; the upwind side is chosen by the sign of S*.  ~70 FP64-pipe instructions + 4 MUFU.
 __device__ __forceinline__ void hllc2(const GasConst& g, const double WL[5], const double WR[5], double F[5]) {
   const double rL = WL[0], uL = WL[1], eL = WL[4];
   const double rR = WR[0], uR = WR[1], eR = WR[4];
   const double pL = g.gm1 * eL, pR = g.gm1 * eR;
   const double ggm1 = g.gamma * g.gm1;
-  const double gpL = ggm1 * eL, gpR = ggm1 * eR;
-  const double cL = sqrt_ratio(gpL, rL), cR = sqrt_ratio(gpR, rR);
-  const double ppv = fma(0.125, ((uL - uR) * (rL + rR)) * (cL + cR), 0.5 * (pL + pR));
-  const double ggq = g.gamma * g.gq;
-  const double cqL = sqrt_ratio(fma(ggq, max0(ppv - pL), gpL), rL);
-  const double cqR = sqrt_ratio(fma(ggq, max0(ppv - pR), gpR), rR);
-  const double SL = uL - cqL, SR = uR + cqR;
-  const double mL = rL * cqL, mR = rR * cqR;
+  const double cL = sqrt_ratio(ggm1 * eL, rL), cR = sqrt_ratio(ggm1 * eR, rR);
+  const double sl1 = uL - cL, sl2 = uR - cR, sr1 = uL + cL, sr2 = uR + cR;
+  const double SL = sl1 < sl2 ? sl1 : sl2, SR = sr1 > sr2 ? sr1 : sr2;
+  const double mL = rL * (uL - SL), mR = rR * (SR - uR);
   const double Ss = div2((pL - pR) + fma(mL, uL, mR * uR), mL + mR);
   const double psL = fma(-mL, Ss - uL, pL);
   const double psR = fma(mR, Ss - uR, pR);
@@ -157,26 +166,17 @@ __device__ __forceinline__ void flux2_12(const GasConst& g, bool d2, const doubl
 // the instruction stream and ptxas can interleave them.  Same arithmetic per face as hllc2, bit for bit.
 template <int N>
 __device__ __forceinline__ void hllc2n(const GasConst& g, const double WL[N][5], const double WR[N][5], double F[N][5]) {
-  const double ggm1 = g.gamma * g.gm1, ggq = g.gamma * g.gq;
-  double pL[N], pR[N], gpL[N], gpR[N], cL[N], cR[N], ppv[N], cqL[N], cqR[N], SL[N], SR[N], mL[N], mR[N], Ss[N];
+  const double ggm1 = g.gamma * g.gm1;
+  double pL[N], pR[N], cL[N], cR[N], SL[N], SR[N], mL[N], mR[N], Ss[N];
 #pragma unroll
   for (int f = 0; f < N; f++) { pL[f] = g.gm1 * WL[f][4]; pR[f] = g.gm1 * WR[f][4]; }
 #pragma unroll
-  for (int f = 0; f < N; f++) { gpL[f] = ggm1 * WL[f][4]; gpR[f] = ggm1 * WR[f][4]; }
-#pragma unroll
-  for (int f = 0; f < N; f++) { cL[f] = sqrt_ratio(gpL[f], WL[f][0]); cR[f] = sqrt_ratio(gpR[f], WR[f][0]); }
-#pragma unroll
-  for (int f = 0; f < N; f++)
-    ppv[f] = fma(0.125, ((WL[f][1] - WR[f][1]) * (WL[f][0] + WR[f][0])) * (cL[f] + cR[f]), 0.5 * (pL[f] + pR[f]));
+  for (int f = 0; f < N; f++) { cL[f] = sqrt_ratio(ggm1 * WL[f][4], WL[f][0]); cR[f] = sqrt_ratio(ggm1 * WR[f][4], WR[f][0]); }
 #pragma unroll
   for (int f = 0; f < N; f++) {
-    cqL[f] = sqrt_ratio(fma(ggq, max0(ppv[f] - pL[f]), gpL[f]), WL[f][0]);
-    cqR[f] = sqrt_ratio(fma(ggq, max0(ppv[f] - pR[f]), gpR[f]), WR[f][0]);
-  }
-#pragma unroll
-  for (int f = 0; f < N; f++) {
-    SL[f] = WL[f][1] - cqL[f]; SR[f] = WR[f][1] + cqR[f];
-    mL[f] = WL[f][0] * cqL[f]; mR[f] = WR[f][0] * cqR[f];
+    const double sl1 = WL[f][1] - cL[f], sl2 = WR[f][1] - cR[f], sr1 = WL[f][1] + cL[f], sr2 = WR[f][1] + cR[f];
+    SL[f] = sl1 < sl2 ? sl1 : sl2; SR[f] = sr1 > sr2 ? sr1 : sr2;
+    mL[f] = WL[f][0] * (WL[f][1] - SL[f]); mR[f] = WR[f][0] * (SR[f] - WR[f][1]);
   }
 #pragma unroll
   for (int f = 0; f < N; f++)

@@ -53,38 +53,6 @@ __device__ __forceinline__ double sqrt_fast(double x) {
 }
 
 
-// ---- leaner forms for the stage kernel --------------------------
-// The MUFU seed carries ~20+ bits; ONE Newton step (~40 bits) followed by a residual correction of the
-// final product reaches <= ~1 ulp with fewer FP64-pipe instructions than refining the reciprocal fully.
-__device__ __forceinline__ double div_lean(double a, double b) {      // 5 FP64 + 1 MUFU
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
-  double e = fma(-b, r, 1.0);
-  r = fma(r, e, r);
-  double q = a * r;
-  double res = fma(-b, q, a);
-  return fma(res, r, q);
-}
-// c = sqrt(gp / rho) without a division: r ~ (gp*rho)^(-1/2), s = gp*r, one residual step on c^2*rho = gp.
-__device__ __forceinline__ double sound_speed_lean(double gp, double rho) {   // 10 FP64 + 1 MUFU
-  double t = gp * rho, r;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(t));
-  double e = fma(-(0.5 * t) * r, r, 0.5);
-  r = fma(r, e, r);
-  double s = gp * r;
-  double res = fma(-(s * rho), s, gp);
-  return fma(res, 0.5 * r, s);
-}
-__device__ __forceinline__ double sqrt_lean(double x) {               // 8 FP64 + 1 MUFU
-  double r;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-(0.5 * x) * r, r, 0.5);
-  r = fma(r, e, r);
-  double s = x * r;
-  double res = fma(-s, s, x);
-  return fma(res, 0.5 * r, s);
-}
-
 #ifdef AK_EXACT_MATH
 __device__ __forceinline__ double rcp_(double x)  { return 1.0 / x; }
 __device__ __forceinline__ double div_(double a, double b) { return a / b; }
@@ -140,7 +108,7 @@ __device__ __forceinline__ void ppm4_limit(double a, double& aL, double& aR) {
 // the cyclic transverse pair; F is returned in the same rotated order (mass, normal momentum,
 // transverse momenta, energy).
 struct GasConst {
-  double gamma, gm1, gq, ug_floor;   // gq = (gamma+1)/(2 gamma)
+  double gamma, gm1, ug_floor;
 };
 
 __device__ __forceinline__ void hllc(const GasConst& g, const double WL[5], const double WR[5], double F[5]) {
@@ -149,12 +117,8 @@ __device__ __forceinline__ void hllc(const GasConst& g, const double WL[5], cons
   const double pL = g.gm1 * eL, pR = g.gm1 * eR;
   const double rLinv = rcp_(rL), rRinv = rcp_(rR);
   const double cL = sqrt_(g.gamma * pL * rLinv), cR = sqrt_(g.gamma * pR * rRinv);
-  const double rbar = 0.5 * (rL + rR), cbar = 0.5 * (cL + cR);
-  const double ppv = 0.5 * ((pL + pR) + (uL - uR) * rbar * cbar);
-  double qL = 1.0, qR = 1.0;
-  if (ppv > pL) qL = sqrt_(1.0 + g.gq * (ppv * rcp_(pL) - 1.0));
-  if (ppv > pR) qR = sqrt_(1.0 + g.gq * (ppv * rcp_(pR) - 1.0));
-  const double SL = uL - cL * qL, SR = uR + cR * qR;
+  // Davis's direct wave-speed estimates (Q2, round-2 reading; Toro Eq.(10.48))
+  const double SL = fmin(uL - cL, uR - cR), SR = fmax(uL + cL, uR + cR);
   const double bm = fmin(SL, 0.0), bp = fmax(SR, 0.0);
   const double mL = rL * (uL - SL), mR = rR * (SR - uR);
   const double Ss = ((pL - pR) + (mL * uL + mR * uR)) * rcp_(mL + mR);
@@ -174,42 +138,6 @@ __device__ __forceinline__ void hllc(const GasConst& g, const double WL[5], cons
   F[2] = Ss * (mom * vK - b * (rK * vK)) * inv;
   F[3] = Ss * (mom * wK - b * (rK * wK)) * inv;
   F[4] = (Ss * ((EK + pK) * uK - b * EK) - bps * Ss) * inv;
-}
-
-// Same flux as hllc() with fewer FP64-pipe instructions: division-free sound speeds, one-Newton
-// quotients, transverse momentum fluxes as (mass flux) x (upwind transverse velocity), and the common
-// factor S*/(S* - b) formed once.  Differs from hllc() by rounding only (a few ulp).
-__device__ __forceinline__ void hllc_lean(const GasConst& g, const double WL[5], const double WR[5], double F[5]) {
-  const double rL = WL[0], uL = WL[1], eL = WL[4];
-  const double rR = WR[0], uR = WR[1], eR = WR[4];
-  const double pL = g.gm1 * eL, pR = g.gm1 * eR;
-  const double cL = sound_speed_lean(g.gamma * pL, rL), cR = sound_speed_lean(g.gamma * pR, rR);
-  const double ppv = 0.5 * ((pL + pR) + (uL - uR) * (0.5 * (rL + rR)) * (0.5 * (cL + cR)));
-  double qL = 1.0, qR = 1.0;
-  if (ppv > pL) qL = sqrt_lean(fma(g.gq, div_lean(ppv, pL) - 1.0, 1.0));
-  if (ppv > pR) qR = sqrt_lean(fma(g.gq, div_lean(ppv, pR) - 1.0, 1.0));
-  const double SL = fma(-cL, qL, uL), SR = fma(cR, qR, uR);
-  const double bm = fmin(SL, 0.0), bp = fmax(SR, 0.0);
-  const double dL = uL - SL, dR = SR - uR;
-  const double mL = rL * dL, mR = rR * dR;
-  const double Ss = div_lean((pL - pR) + fma(mL, uL, mR * uR), mL + mR);
-  const double psL = fma(-mL, Ss - uL, pL);
-  const double psR = fma(mR, Ss - uR, pR);
-  const double ps = fmax(0.5 * (psL + psR), 0.0);
-  const bool left = (Ss >= 0.0);
-  const double rK = left ? rL : rR, uK = left ? uL : uR, vK = left ? WL[2] : WR[2], wK = left ? WL[3] : WR[3];
-  const double eK = left ? eL : eR, pK = left ? pL : pR, b = left ? bm : bp;
-  const double EK = fma(0.5 * rK, fma(uK, uK, fma(vK, vK, wK * wK)), eK);
-  const double mom = rK * uK;
-  const double inv = rcp_fast(Ss - b);
-  const double w = Ss * inv;                       // S*/(S* - b)
-  const double bps = b * ps;
-  const double f0 = fma(-b, rK, mom) * w;
-  F[0] = f0;
-  F[1] = fma(Ss, fma(mom, uK, pK) - b * mom, -bps) * inv;
-  F[2] = f0 * vK;
-  F[3] = f0 * wK;
-  F[4] = (fma(EK + pK, uK, -b * EK) - bps) * w;
 }
 
 }  // namespace ak

@@ -6,30 +6,12 @@
 #include "ak_physics.cuh"
 #include "ak_stage_simple.cuh"
 #include "ak_stage_tiled.cuh"
-#include "ak_stage_tma.cuh"
-#include "ak_stage_v2.cuh"
 #include "ak_stage_v3.cuh"
 #include "ak_fluxcorr.cuh"
 
 #include <cstdlib>
 
 namespace ak {
-
-// tile shape of the production kernel: 0 = 16x12 (2 CTAs/SM), 1 = 16x8 (3 CTAs/SM), 2 = 32x6 (2 CTAs/SM)
-static int pick_tile(const ak_pack& p) {
-  return (p.d.nx[1] % 12 == 0 || p.d.nx[1] >= 48) ? 0 : 1;
-}
-
-template <int RECON>
-static cudaError_t launch_stage_v2(const ak_pack& p, const double* Uin, const double* U0, double* Uout,
-                                   const StageCoef& sc) {
-  const bool stage2 = (Uin != U0);
-  switch (pick_tile(p)) {
-    case 1:  return launch_v2<RECON, 16, 8, 3>(p, Uin, U0, Uout, sc, stage2);
-    case 2:  return launch_v2<RECON, 32, 6, 2>(p, Uin, U0, Uout, sc, stage2);
-    default: return launch_v2<RECON, 16, 12, 2>(p, Uin, U0, Uout, sc, stage2);
-  }
-}
 
 // tile shape of the v3 kernel (workers + one edge warp): the one that wastes the fewest lanes on the ragged
 // last tile row and on the edge warp.  0 = 16x10 (6 warps), 1 = 16x8 (5 warps)
@@ -72,8 +54,6 @@ cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, 
   // an odd surplus of ghost layers (ng = 4 with PPM4, ng = 3 with PLM) takes the LDG-staged tiled kernel.
   const int R = (p.recon == 0) ? 2 : 3;
   if (p.variant == 2 || ((p.d.ng - R) & 1)) return launch_stage_tiled(p, Uin, U0, Uout, sc);
-  if (p.variant == 3) return launch_stage_tma(p, Uin, U0, Uout, sc);
-  if (p.variant == 4) return p.recon == 0 ? launch_stage_v2<0>(p, Uin, U0, Uout, sc) : launch_stage_v2<1>(p, Uin, U0, Uout, sc);
   return p.recon == 0 ? launch_stage_v3_rs<0>(p, Uin, U0, Uout, sc) : launch_stage_v3_rs<1>(p, Uin, U0, Uout, sc);
 }
 

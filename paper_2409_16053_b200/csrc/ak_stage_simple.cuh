@@ -17,7 +17,7 @@ __global__ void __launch_bounds__(128) stage_simple_kernel(PackDev P, const doub
   if (i >= P.nx[0]) return;
   const int j = blockIdx.y % P.nx[1], k = blockIdx.y / P.nx[1], m = blockIdx.z;
   GasConst g;
-  g.gamma = P.gamma; g.gm1 = P.gamma - 1.0; g.gq = (P.gamma + 1.0) / (2.0 * P.gamma);
+  g.gamma = P.gamma; g.gm1 = P.gamma - 1.0;
   g.ug_floor = P_FLOOR / (P.gamma - 1.0);
   const long long nc = P.ncell;
   const long long base = (long long)m * 5 * nc + ((long long)(k + P.ng) * P.nt[1] + (j + P.ng)) * P.nt[0] + (i + P.ng);

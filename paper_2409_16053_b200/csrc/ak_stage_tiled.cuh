@@ -86,7 +86,7 @@ stage_tiled_kernel(PackDev P, const double* __restrict__ Uin, const double* U0, 
   const double c1 = sc.c[lev][0], c2 = sc.c[lev][1], c3 = sc.c[lev][2];
 
   GasConst g;
-  g.gamma = P.gamma; g.gm1 = P.gamma - 1.0; g.gq = (P.gamma + 1.0) / (2.0 * P.gamma);
+  g.gamma = P.gamma; g.gm1 = P.gamma - 1.0;
   g.ug_floor = P_FLOOR / (P.gamma - 1.0);
 
   const int nextra = wI + wJ;           // threads that also handle halo cells / upper-edge faces

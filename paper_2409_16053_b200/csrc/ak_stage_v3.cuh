@@ -1,15 +1,12 @@
-// ak_stage_v3.cuh -- production ak_hydro_stage kernel: TMA-staged 2.5-D plane marching, third
-// generation.  Same scheme and data flow as v2 (ak_stage_v2.cuh, kept as variant 4), changed where
-// profiles/r01_v2_stage_cfg3.md showed the time going:
-//   * v2 let the first TI+TJ threads of a CTA also solve the tile-edge faces; that warp ran 41 % longer per
-//     plane than the others, which waited for it at both barriers (20 % of all stall samples).  Here the
-//     CTA is NT = TI x TJ WORKER threads (one per (i, j) column) plus ONE EDGE WARP whose lanes own the
-//     TI + TJ tile-edge faces (reconstruct the two halo cells, solve the upper-edge face) and whose lane 0
-//     issues the TMA copies.  The edge warp has less work per plane than a worker warp, so it is never
-//     the one the barrier waits for, and the workers' instruction stream contains no edge code.
-//   * stage 2 needs U0 = U^n pointwise; v2 loaded it with LDG inside the plane loop and stalled on it (three
-//     warps per scheduler cannot hide an HBM round trip).  Here it arrives by a second TMA box into a
-//     two-slot ring on the same mbarrier as the plane that needs it.
+// ak_stage_v3.cuh -- production ak_hydro_stage kernel: TMA-staged 2.5-D plane marching.
+// A CTA owns a TI x TJ tile of (i, j) columns of one MeshBlock and marches along k:
+//   * each k-plane of the tile WITH its R halo layers, all 5 variables, arrives by ONE 5-D cp.async.bulk.tensor
+//     (TMA) into a two-slot shared-memory ring, armed on an mbarrier two planes ahead; in stage 2 a second box
+//     brings U0 = U^n of the tile's columns on the same mbarrier;
+//   * the CTA is NT = TI x TJ WORKER threads (one per column) plus ONE EDGE WARP whose lanes own the TI + TJ
+//     tile-edge faces (reconstruct the two halo cells, solve the upper-edge face) and whose lane 0 issues the
+//     TMA copies.  The edge warp has less work per plane than a worker warp, so it is never the one the
+//     barrier waits for, and the workers' instruction stream contains no edge code.
 // Per iteration s (plane s already converted to primitives in slot b = it & 1):
 //       B(s)    workers: reconstruct own cell in x1, x2: q+ -> Q[b], q- in registers
 //               edge:    reconstruct halo cells -1 and wI (wJ): q+ of -1 -> Q[b], q- of wI in registers
@@ -26,7 +23,6 @@
 #include "ak_pack.h"
 #include "ak_lean.cuh"
 #include "ak_tma.cuh"
-#include "ak_stage_v2.cuh"     // recon2<>
 
 namespace ak {
 
@@ -79,7 +75,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
   const int send = k1 + R;                              // planes k0-R .. send-1 are staged
 
   GasConst g;
-  g.gamma = P.gamma; g.gm1 = P.gamma - 1.0; g.gq = (P.gamma + 1.0) / (2.0 * P.gamma);
+  g.gamma = P.gamma; g.gm1 = P.gamma - 1.0;
   g.ug_floor = P_FLOOR / (P.gamma - 1.0);
 
   // plane p (absolute active index, may lie in the ghost layers) -> ring slot `slot`, armed on bars[slot]

@@ -63,7 +63,7 @@ def test_create_rejects_bad_arguments(L):
     assert L.ak_fill_ghosts(h) == -2 and L.ak_hydro_stage(h, 1, 1e-3) == -2      # not bound
     assert L.ak_pack_bind(h, 0, 0, 0, 0) == -1
     assert L.ak_pack_bind(h, 0x1000080, 0x2000000, 0x3000000, 0) == -1           # misaligned
-    assert L.ak_pack_set_variant(h, 5) == -1 and L.ak_pack_set_variant(h, 4) == 0 and L.ak_pack_set_variant(h, 0) == 0
+    assert L.ak_pack_set_variant(h, 3) == -1 and L.ak_pack_set_variant(h, 2) == 0 and L.ak_pack_set_variant(h, 0) == 0
     assert L.ak_pack_set_tile(h, 4) == -1 and L.ak_pack_set_tile(h, -2) == -1
     assert L.ak_pack_set_tile(h, 3) == 0 and L.ak_pack_set_tile(h, -1) == 0
     assert L.ak_pack_destroy(h) == 0

@@ -271,9 +271,9 @@ def test_tile_shapes_give_bit_identical_results(ak, recon):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("variant", [2, 3, 4])
-def test_older_kernel_generations_still_match_the_oracle(orc, ak, variant):
-    """Variants 2-4 (include/ak.h) stay in the library as independent cross-checks of the production kernel."""
+@pytest.mark.parametrize("variant", [2])
+def test_ldg_staged_fallback_kernel_matches_the_oracle(orc, ak, variant):
+    """Variant 2 (include/ak.h) is the kernel taken automatically when the TMA box origin would be misaligned."""
     for w in (I.config3(nrb=2, nx=32), I.config1(nrb=2, nx=32)):
         errs, *_ = run_lockstep(orc, ak, w, 2, variant, check_ghosts=False)
         assert max(errs) <= TOL_RUN, (variant, w.name, errs)

@@ -170,17 +170,20 @@ def wave_error(orc, N, recon, ng, cfl, direction=0):
 
 def test_sound_wave_second_order_plm(orc):
     e = {N: wave_error(orc, N, I.RECON_PLM, 2, 0.3) for N in (32, 64, 128, 256)}
-    for N, ref in GOLD_C["plm_cfl0.3"].items():
+    for N, ref in GOLD_C["plm_cfl0.3"].items():              # written by tests/golden/make_appendix_c.py (stand-alone 1-D numpy)
         if int(N) in e:
-            assert e[int(N)] == pytest.approx(ref, rel=2e-4)
+            assert e[int(N)] == pytest.approx(ref, rel=1e-6)
     for N in (64, 128):
         assert 3.5 <= e[N] / e[2 * N] <= 4.2, e
 
 
 def test_sound_wave_second_order_ppm4(orc):
     e = {N: wave_error(orc, N, I.RECON_PPM4, 3, 0.1) for N in (32, 64, 128)}
+    # PPM4 + SSPRK(2,2) amplifies round-off differences on this 1e-6-amplitude wave (limiter decisions flip at the
+    # grid scale: two implementations that agree to 1e-16 after one step differ by 3e-10 after the 320 steps of a
+    # period, measured), so the stand-alone script's errors are reproduced to a fraction of a per cent only
     for N, ref in GOLD_C["ppm4_cfl0.1"].items():
-        assert e[int(N)] == pytest.approx(ref, rel=2e-4)
+        assert e[int(N)] == pytest.approx(ref, rel=1e-2)
     for N in (32, 64):
         assert 3.6 <= e[N] / e[2 * N] <= 4.3, e
 
@@ -245,6 +248,114 @@ def test_dt_uses_each_directions_own_dx_and_is_a_min(orc):
     U0[0, 4, 5, 7, 3] *= 50.0
     p.load(U0)
     assert p.new_dt(0.3) < expect
+
+
+def test_dt_on_a_two_level_mesh_uses_each_levels_own_dx(orc):
+    """Eq.(3), P:107-110 with 'uniform time stepping' over all levels; reading Q9: every leaf block enters with
+    its OWN level's dx.  (the level-dependent dx of orc_new_dt had no CPU pin.)
+    A 'level-0 dx everywhere' oracle fails case 1 (dt twice too large), a 'finest dx everywhere' oracle fails case 2."""
+    nx, ng = 8, 2
+    mesh = I.smr_mesh((2, 2, 2), (nx, nx, nx), ng, (0, 0, 0), (1, 1, 1))     # one root block refined: 7 + 8 blocks
+    assert sorted(set(b[0] for b in mesh.blocks)) == [0, 1]
+    rho, v, P = 1.3, (0.4, -0.7, 0.2), 0.9
+    prim = lambda X1, X2, X3: (rho + 0 * X1, v[0] + 0 * X1, v[1] + 0 * X1, v[2] + 0 * X1, P + 0 * X1)
+    U0 = I.make_state(mesh, prim).numpy()
+    p = orc.OrcPack(mesh, I.GAMMA, I.RECON_PLM)
+    p.load(U0)
+    cs = math.sqrt(I.GAMMA * P / rho)
+    dx0 = 1.0 / (2 * nx)
+    # case 1: uniform state -> the fine level decides: CFL (dx0/2) / (max_d |v_d| + c_s)
+    assert p.new_dt(0.3) == pytest.approx(0.3 * (dx0 / 2) / (0.7 + cs), rel=1e-14)
+    # case 2: one fast cell that sits in a level-0 block only: the answer is the COARSE candidate dx0/(|v1| + c_s)
+    m0 = [m for m, b in enumerate(mesh.blocks) if b[0] == 0][3]
+    vfast = 40.0
+    U1 = U0.copy()
+    k, j, i = ng + 3, ng + 1, ng + 5
+    U1[m0, 1, k, j, i] = rho * vfast
+    U1[m0, 4, k, j, i] = P / (I.GAMMA - 1) + 0.5 * rho * (vfast ** 2 + v[1] ** 2 + v[2] ** 2)
+    p.load(U1)
+    assert p.new_dt(0.3) == pytest.approx(0.3 * dx0 / (vfast + cs), rel=1e-13)
+    # case 3: the same fast cell in a level-1 block: the fine candidate, half of case 2
+    m1 = [m for m, b in enumerate(mesh.blocks) if b[0] == 1][5]
+    U2 = U0.copy()
+    U2[m1, 1, k, j, i] = rho * vfast
+    U2[m1, 4, k, j, i] = P / (I.GAMMA - 1) + 0.5 * rho * (vfast ** 2 + v[1] ** 2 + v[2] ** 2)
+    p.load(U2)
+    assert p.new_dt(0.3) == pytest.approx(0.3 * (dx0 / 2) / (vfast + cs), rel=1e-13)
+    # a NaN momentum anywhere in the active cells is reported, not skipped (ADVICE r1; a NaN density or energy is
+    # caught by the floors of reading Q7, which are written as !(x >= floor))
+    U3 = U0.copy()
+    U3[m0, 2, k, j, i] = float("nan")
+    p.load(U3)
+    with pytest.raises(orc.OrcError):
+        p.new_dt(0.3)
+    p.close()
+
+
+# ------------------------------------------------------------------ strong shocks (VERDICT r1 item 1b) -------------
+def two_shock_sample(g, L, R, ps, us, xi):
+    """rho, u, p of a two-shock Riemann solution at xi = x/t (both outer waves shocks: ps > pL, pR)."""
+    (rL, uL, pL), (rR, uR, pR) = L, R
+    cL, cR = math.sqrt(g * pL / rL), math.sqrt(g * pR / rR)
+    mu = (g - 1) / (g + 1)
+    rsL = rL * (ps / pL + mu) / (mu * ps / pL + 1)
+    rsR = rR * (ps / pR + mu) / (mu * ps / pR + 1)
+    SL = uL - cL * math.sqrt((g + 1) / (2 * g) * ps / pL + (g - 1) / (2 * g))
+    SR = uR + cR * math.sqrt((g + 1) / (2 * g) * ps / pR + (g - 1) / (2 * g))
+    rho = np.where(xi < SL, rL, np.where(xi < us, rsL, np.where(xi < SR, rsR, rR)))
+    u = np.where(xi < SL, uL, np.where(xi < SR, us, uR))
+    pr = np.where(xi < SL, pL, np.where(xi < SR, ps, pR))
+    return rho, u, pr, dict(SL=SL, SR=SR, rsL=rsL, rsR=rsR)
+
+
+@pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3)])
+def test_colliding_supersonic_streams_converge_to_the_exact_two_shock_solution(orc, recon, ng):
+    """Two Mach-3 / Mach-2.5 streams colliding head-on (the regime of the paper's supersonic-turbulence and blast runs,
+    P:142): with the round-1 pressure-based HLLC speeds the first face flux was 0/0.  The run must stay finite,
+    floor-free, and converge in L1 to the exact solution (two shocks, a contact), with the star pressure and
+    velocity on the plateaus between the shocks within 3 % (post-shock oscillations behind slowly moving strong shocks are a known feature of Godunov-type schemes)."""
+    g = 1.4
+    L = (1.0, 3.0 * math.sqrt(g * 1.0 / 1.0), 1.0)
+    R = (2.0, -2.5 * math.sqrt(g * 0.5 / 2.0), 0.5)
+    ps, us = exact_riemann(g, L[0], L[1], L[2], R[0], R[1], R[2])
+    assert ps > 10 * L[2]                                  # strong shocks on both sides
+    tend = 0.05
+    errs = {}
+    for N in (128, 256, 512):
+        mesh = I.uniform_mesh((1, 1, 1), (N, 4, 4), ng)
+        mesh = __import__("dataclasses").replace(mesh, bc=(1, 1, 0, 0, 0, 0))       # outflow ends along x1
+
+        def prim(X1, X2, X3):
+            left = X1 < 0.5
+            f = lambda a, b: torch.where(left, a, b).to(torch.float64)
+            z = torch.zeros_like(X1)
+            return (f(L[0], R[0]), f(L[1], R[1]), z, z, f(L[2], R[2]))
+
+        U0 = I.make_state(mesh, prim, gamma=g).numpy()
+        U = run(orc, mesh, U0, recon, gamma=g, cfl=0.3, tend=tend)     # asserts floor_count == 0
+        prof = U[0, :, ng, ng, ng:-ng]
+        assert np.all(np.isfinite(prof))
+        x = (np.arange(N) + 0.5) / N
+        xi = (x - 0.5) / tend
+        rho_ex, u_ex, p_ex, d = two_shock_sample(g, L, R, ps, us, xi)
+        assert -0.5 / tend < d["SL"] and d["SR"] < 0.5 / tend          # both shocks still inside the tube
+        errs[N] = np.abs(prof[0] - rho_ex).mean()
+        if N == 512:
+            rho, u = prof[0], prof[1] / prof[0]
+            pr = (g - 1) * (prof[4] - 0.5 * rho * u * u)
+            width = d["SR"] - d["SL"]
+            plateau = (xi > d["SL"] + 0.15 * width) & (xi < d["SR"] - 0.15 * width)
+            assert plateau.sum() >= 20
+            assert np.abs(pr[plateau] / ps - 1).max() < 3e-2
+            assert np.abs(u[plateau] - us).max() < 3e-2 * abs(L[1])
+            # densities away from the contact (start-up 'wall heating' leaves a dip AT the contact in every
+            # shock-capturing scheme): the outer third of each post-shock region
+            left_third = (xi > d["SL"] + 0.1 * width) & (xi < d["SL"] + 0.3 * width) & (xi < us - 0.1 * width)
+            right_third = (xi < d["SR"] - 0.1 * width) & (xi > d["SR"] - 0.3 * width) & (xi > us + 0.1 * width)
+            assert left_third.sum() >= 5 and right_third.sum() >= 5
+            assert np.abs(rho[left_third] / d["rsL"] - 1).max() < 3e-2
+            assert np.abs(rho[right_third] / d["rsR"] - 1).max() < 3e-2
+    assert errs[256] < 0.75 * errs[128] and errs[512] < 0.75 * errs[256], errs
 
 
 @pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3)])
