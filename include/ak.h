@@ -34,6 +34,7 @@ extern "C" {
 #define AK_ESTATE      (-2)   /* call order violated (e.g. stage before fill)   */
 #define AK_EUNSUPPORTED (-3)  /* valid request outside the implemented scope    */
 #define AK_ECUDA       (-4)   /* CUDA runtime error, message in ak_last_error() */
+#define AK_ENONFINITE  (-5)   /* the state holds a NaN / inf: ak_new_dt found a non-finite signal speed */
 
 #define AK_RECON_PLM   0      /* piecewise linear, van Leer limiter     */
 #define AK_RECON_PPM4  1      /* piecewise parabolic, Colella-Woodward limiters */

@@ -18,6 +18,13 @@ static int cuda_fail(cudaError_t e, const char* where) {
 
 extern "C" const char* ak_last_error(void) { return g_err.c_str(); }
 
+// every launching entry point runs on the device that owns the pack's buffers, whatever the caller's current device
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(int dev) { if (dev >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != dev) cudaSetDevice(dev); else prev = -1; }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 static size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
 
 // scratch layout: [0,256) reduction cells | block table int4[nmb] | leaf0 | leaf1 | same-level neighbours int[nmb][27]
@@ -160,6 +167,14 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
       nbc[k] = code;
     }
   }
+  {
+    // the device that owns u_a runs every kernel of this pack (not whatever device is current at call time)
+    cudaPointerAttributes pa;
+    AK_CUDA(cudaPointerGetAttributes(&pa, u_a), "cudaPointerGetAttributes");
+    if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) return fail(AK_EINVAL, "u_a is not a device pointer");
+    p->device = pa.device;
+  }
+  DeviceGuard guard(p->device);
   char* s = (char*)scratch;
   AK_CUDA(cudaMemsetAsync(s, 0, 256, st), "memset scratch");
   AK_CUDA(cudaMemcpyAsync(s + sl.nbr, nbr.data(), sizeof(int) * nbr.size(), cudaMemcpyHostToDevice, st), "upload neighbour table");
@@ -170,16 +185,19 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
   AK_CUDA(cudaStreamSynchronize(st), "bind sync");
   d.dtmin_bits = (unsigned long long*)s;
   d.floor_cnt = (unsigned long long*)(s + 8);
+  d.nonfinite = (unsigned long long*)(s + 16);
   d.smax_bits = (unsigned long long*)(s + 64);
   d.blk = (const int4*)(s + sl.blk);
   d.leaf0 = (const int*)(s + sl.leaf0);
   d.leaf1 = (const int*)(s + sl.leaf1);
   d.nbr = (const int*)(s + sl.nbr);
   d.nbc = (const int*)(s + sl.nbc);
-  int dev = 0;
-  AK_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
-  AK_CUDA(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev), "query SM count");
+  AK_CUDA(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device), "query SM count");
   p->u[0] = (double*)u_a; p->u[1] = (double*)u_b; p->scratch = scratch; p->stream = st;
+  // a third register bound earlier (SSPRK(3,3)) stays valid only if it is still disjoint from the new buffers
+  if (p->u[2] && (overlap(p->u[2], sb, u_a, sb) || overlap(p->u[2], sb, u_b, sb) || overlap(p->u[2], sb, scratch, sl.total))) {
+    p->u[2] = nullptr; p->integrator = 2;
+  }
   p->cur = 0; p->ghosts_ok = false; p->bound = true; p->launches = 0; p->dt_cached = false;
   p->tmap_box[0] = p->tmap_box[1] = 0;
   p->tmap0_box[0] = p->tmap0_box[1] = 0;
@@ -200,7 +218,12 @@ extern "C" int ak_pack_set_integrator(ak_pack* p, int nstages, void* u_c) {
     if (!u_c) return fail(AK_EINVAL, "SSPRK(3,3) needs a third state buffer");
     if ((uintptr_t)u_c & 255) return fail(AK_EINVAL, "buffers must be 256-byte aligned");
     if (!p->bound) return fail(AK_ESTATE, "bind the pack first");
-    if (u_c == (void*)p->u[0] || u_c == (void*)p->u[1]) return fail(AK_EINVAL, "device buffers overlap");
+    const size_t sb = ak_pack_state_bytes(p), ss = scratch_layout(p).total;
+    auto overlap = [](const void* a, size_t na, const void* b, size_t nb) {
+      return (uintptr_t)a < (uintptr_t)b + nb && (uintptr_t)b < (uintptr_t)a + na;
+    };
+    if (overlap(u_c, sb, p->u[0], sb) || overlap(u_c, sb, p->u[1], sb) || overlap(u_c, sb, p->scratch, ss))
+      return fail(AK_EINVAL, "device buffers overlap");
   }
   if (p->bound && p->cur != 0 && !(p->integrator == 1 && p->cur == 1)) return fail(AK_ESTATE, "change the integrator between steps");
   if (p->bound && p->cur == 1 && nstages != 1)
@@ -237,6 +260,7 @@ extern "C" int ak_pack_set_tile(ak_pack* p, int tile) {
 
 extern "C" int ak_fill_ghosts(ak_pack* p) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  DeviceGuard guard(p->device);
   AK_CUDA(ak::launch_fill_ghosts(*p, p->u[p->cur]), "ak_fill_ghosts launch");
   p->launches += 1;
   p->ghosts_ok = true;
@@ -245,6 +269,7 @@ extern "C" int ak_fill_ghosts(ak_pack* p) {
 
 extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  DeviceGuard guard(p->device);
   if (stage < 1 || stage > p->integrator) return fail(AK_EINVAL, "stage must be 1 .. number of stages of the integrator");
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(AK_EINVAL, "dt must be positive and finite");
   if (p->integrator == 1 ? p->cur > 1 : p->cur != stage - 1)
@@ -293,6 +318,7 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
 
 extern "C" int ak_new_dt(ak_pack* p, double cfl, double* dt_out) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  DeviceGuard guard(p->device);
   if (!dt_out) return fail(AK_EINVAL, "null dt_out");
   if (!(cfl > 0.0)) return fail(AK_EINVAL, "cfl must be positive");
   double dtmin = 0.0;
@@ -306,15 +332,23 @@ extern "C" int ak_new_dt(ak_pack* p, double cfl, double* dt_out) {
     for (int lev = 0; lev < 2; lev++)
       for (int d = 0; d < 3; d++) {
         const double dx = (lev ? 0.5 : 1.0) * p->d.dx0[d];
-        if (s[3 * lev + d] > 0.0) dtmin = std::fmin(dtmin, dx / s[3 * lev + d]);
+        // the maxima were taken on the bit patterns, where every NaN and +inf orders above all finite speeds, so a
+        // single corrupted cell survives the reduction; an all-zero pattern means the level holds no block
+        const double sv = s[3 * lev + d];
+        if (sv != sv || sv == HUGE_VAL) return fail(AK_ENONFINITE, "non-finite signal speed in the state (NaN or inf in an active cell)");
+        if (sv > 0.0) dtmin = std::fmin(dtmin, dx / sv);
       }
   } else {
     AK_CUDA(ak::launch_new_dt(*p, p->u[p->cur]), "ak_new_dt launch");
     p->launches += 2;
-    AK_CUDA(cudaMemcpyAsync(&dtmin, p->d.dtmin_bits, 8, cudaMemcpyDeviceToHost, p->stream), "ak_new_dt copy");
+    unsigned long long cells[3];    // dtmin bits, floor counter, non-finite rows
+    AK_CUDA(cudaMemcpyAsync(cells, p->d.dtmin_bits, 24, cudaMemcpyDeviceToHost, p->stream), "ak_new_dt copy");
     AK_CUDA(cudaStreamSynchronize(p->stream), "ak_new_dt sync");
+    if (cells[2]) return fail(AK_ENONFINITE, "non-finite signal speed in the state (NaN or inf in an active cell)");
+    std::memcpy(&dtmin, &cells[0], 8);
   }
-  if (!(dtmin > 0.0) || !std::isfinite(dtmin)) return fail(AK_ECUDA, "non-finite time step (state corrupted?)");
+  if (!(dtmin > 0.0) || !std::isfinite(dtmin))
+    return fail(AK_ENONFINITE, "non-finite signal speed in the state (NaN or inf in an active cell)");
   *dt_out = cfl * dtmin;
   return AK_OK;
 }
@@ -334,6 +368,7 @@ extern "C" void* ak_pack_current(const ak_pack* p) { return (p && p->bound) ? (v
 
 extern "C" int ak_pack_upload(ak_pack* p, const void* host_u) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  DeviceGuard guard(p->device);
   if (!host_u) return fail(AK_EINVAL, "null host buffer");
   AK_CUDA(cudaMemcpyAsync(p->u[0], host_u, ak_pack_state_bytes(p), cudaMemcpyHostToDevice, p->stream), "ak_pack_upload");
   p->cur = 0; p->ghosts_ok = false; p->dt_cached = false;
@@ -342,6 +377,7 @@ extern "C" int ak_pack_upload(ak_pack* p, const void* host_u) {
 
 extern "C" int ak_pack_download_async(ak_pack* p, void* host_u) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  DeviceGuard guard(p->device);
   if (!host_u) return fail(AK_EINVAL, "null host buffer");
   AK_CUDA(cudaMemcpyAsync(host_u, p->u[p->cur], ak_pack_state_bytes(p), cudaMemcpyDeviceToHost, p->stream), "ak_pack_download_async");
   return AK_OK;
@@ -349,6 +385,7 @@ extern "C" int ak_pack_download_async(ak_pack* p, void* host_u) {
 
 extern "C" int ak_pack_download(ak_pack* p, void* host_u) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  DeviceGuard guard(p->device);
   if (!host_u) return fail(AK_EINVAL, "null host buffer");
   AK_CUDA(cudaMemcpyAsync(host_u, p->u[p->cur], ak_pack_state_bytes(p), cudaMemcpyDeviceToHost, p->stream), "ak_pack_download");
   AK_CUDA(cudaStreamSynchronize(p->stream), "ak_pack_download sync");
@@ -357,6 +394,7 @@ extern "C" int ak_pack_download(ak_pack* p, void* host_u) {
 
 extern "C" long long ak_pack_floor_count(ak_pack* p) {
   if (!p || !p->bound) { fail(AK_ESTATE, "pack not bound"); return -1; }
+  DeviceGuard guard(p->device);
   unsigned long long n = 0;
   if (cudaMemcpyAsync(&n, p->d.floor_cnt, 8, cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
       cudaStreamSynchronize(p->stream) != cudaSuccess) { fail(AK_ECUDA, "ak_pack_floor_count copy failed"); return -1; }

@@ -213,7 +213,7 @@ cudaError_t launch_fill_ghosts(const ak_pack& p, double* U) {
 // ---- S0: CFL time step ---------------------------------------------------------------------------
 // Every candidate dx_d/(|v_d|+c_s) is positive, so its IEEE bit pattern orders like an unsigned
 // integer and the global min is one atomicMin per CTA after a shuffle + shared-memory reduction.
-__global__ void dt_init_kernel(PackDev P) { *P.dtmin_bits = 0x7FF0000000000000ull; }
+__global__ void dt_init_kernel(PackDev P) { *P.dtmin_bits = 0x7FF0000000000000ull; *P.nonfinite = 0ull; }
 
 __global__ void __launch_bounds__(256) new_dt_kernel(PackDev P, const double* __restrict__ U, long long nrows) {
   const double ug_floor = P_FLOOR / (P.gamma - 1.0);
@@ -237,6 +237,7 @@ __global__ void __launch_bounds__(256) new_dt_kernel(PackDev P, const double* __
     // dx_d / s is monotone in s > 0 (IEEE division rounds monotonically), so the row's min over cells of
     // dx_d / (|v_d| + c_s) is dx_d / max(|v_d| + c_s), bit for bit: three divisions per row instead of per cell
     double s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    bool bad = false;                 // a NaN / inf signal speed must not be skipped by fmax (it is reported, ak.h)
 #pragma unroll 2
     for (int i = li; rowok && i < P.nx[0]; i += 32) {
       double u[5], w[5];
@@ -244,10 +245,13 @@ __global__ void __launch_bounds__(256) new_dt_kernel(PackDev P, const double* __
       c2p(u, w, ug_floor);
       double pr = (P.gamma - 1.0) * w[4];
       double cs = sqrt(P.gamma * pr / w[0]);
-      s1 = fmax(s1, fabs(w[1]) + cs);
-      s2 = fmax(s2, fabs(w[2]) + cs);
-      s3 = fmax(s3, fabs(w[3]) + cs);
+      const double a1 = fabs(w[1]) + cs, a2 = fabs(w[2]) + cs, a3 = fabs(w[3]) + cs;
+      bad = bad || !((a1 + a2) + a3 < __longlong_as_double(0x7FF0000000000000ll));
+      s1 = fmax(s1, a1);
+      s2 = fmax(s2, a2);
+      s3 = fmax(s3, a3);
     }
+    if (bad) atomicAdd(P.nonfinite, 1ull);
     if (s1 > 0.0) best = fmin(best, fmin(dx1 / s1, fmin(dx2 / s2, dx3 / s3)));
   }
   for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));

@@ -30,6 +30,7 @@ struct PackDev {
   double gamma;
   unsigned long long* dtmin_bits;   // scratch cell: min candidate dt as ordered bits
   unsigned long long* floor_cnt;    // scratch cell: floor activations
+  unsigned long long* nonfinite;    // scratch cell: rows with a NaN / inf signal speed seen by new_dt_kernel
   unsigned long long* smax_bits;    // 6 scratch cells [level][d]: max |v_d| + c_s of U^{n+1} as ordered bits (stage 2)
 };
 
@@ -60,6 +61,7 @@ struct ak_pack {
   int tile = -1;                  // -1 = automatic (ak_pack_set_tile)
   long long launches = 0;
   int sm_count = 148;
+  int device = -1;                // ordinal of the device that owns the buffers (set at bind)
   // tensor maps over u[0], u[1] for the TMA stage kernel, rebuilt when the staging box changes
   mutable CUtensorMap tmap[3];
   mutable int tmap_box[2] = {0, 0};

@@ -282,7 +282,8 @@ cudaError_t launch_tiled(const ak_pack& p, const double* Uin, const double* U0, 
   using S = TileSmem<RECON, TI, TJ>;
   const PackDev& P = p.d;
   auto kern = stage_tiled_kernel<RECON, TI, TJ>;
-  static bool attr_set = false;
+  static bool attr_set_dev[64] = {};   // the opt-in to > 48 KB of dynamic shared memory is per device
+  bool& attr_set = attr_set_dev[p.device & 63];
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes);
     if (e != cudaSuccess) return e;

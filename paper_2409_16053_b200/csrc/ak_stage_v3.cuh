@@ -191,7 +191,9 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
   }
 
   double wk[R][5], qlow[5], qp3[5], G[5];
-  double smax[3] = {0.0, 0.0, 0.0};                     // stage 2: max signal speed per direction over this thread's cells
+  // stage 2: max signal speed per direction over this thread's cells, kept as BIT PATTERNS: for x >= 0 they order
+  // like the doubles, and every NaN / +inf orders above all finite values, so a corrupted cell is not skipped
+  unsigned long long smax[3] = {0ull, 0ull, 0ull};
   int nfl = 0;
 #pragma unroll
   for (int a = 0; a < R; a++)
@@ -288,9 +290,11 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
         double ug = un[4] - 0.5 * rinv * (un[1] * un[1] + (un[2] * un[2] + un[3] * un[3]));
         if (!(ug >= g.ug_floor)) ug = g.ug_floor;
         const double cs = sqrt(g.gamma * (g.gm1 * ug) / rho);
-        smax[0] = fmax(smax[0], fabs(un[1] * rinv) + cs);
-        smax[1] = fmax(smax[1], fabs(un[2] * rinv) + cs);
-        smax[2] = fmax(smax[2], fabs(un[3] * rinv) + cs);
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+          const unsigned long long b = (unsigned long long)__double_as_longlong(fabs(un[1 + d] * rinv) + cs);
+          smax[d] = b > smax[d] ? b : smax[d];
+        }
       }
     }
 #pragma unroll
@@ -385,10 +389,10 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
     // positive doubles order like their bit patterns: warp max by shuffles, one atomicMax per warp and direction
 #pragma unroll
     for (int d = 0; d < 3; d++) {
-      double v = smax[d];
+      unsigned long long v = smax[d];
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-      if ((tid & 31) == 0 && v > 0.0) atomicMax(P.smax_bits + 3 * lev + d, (unsigned long long)__double_as_longlong(v));
+      for (int o = 16; o > 0; o >>= 1) { const unsigned long long t = __shfl_xor_sync(0xffffffffu, v, o); v = t > v ? t : v; }
+      if ((tid & 31) == 0 && v) atomicMax(P.smax_bits + 3 * lev + d, v);
     }
   }
 }
@@ -413,7 +417,8 @@ cudaError_t launch_v3(const ak_pack& p, const double* Uin, const double* U0, dou
   const size_t smem = S::bytes;
   auto k1 = stage_v3_kernel<RECON, RS, TI, TJ, MINB, false>;
   auto k2 = stage_v3_kernel<RECON, RS, TI, TJ, MINB, true>;
-  static bool attr_set = false;
+  static bool attr_set_dev[64] = {};   // the opt-in to > 48 KB of dynamic shared memory is per device
+  bool& attr_set = attr_set_dev[p.device & 63];
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -17,3 +17,12 @@ def orc():
     from oracle import orc as _orc
     _orc.build()
     return _orc
+
+
+def pytest_terminal_summary(terminalreporter):
+    """Margins of the parity runs (worst Q14 against the bar), so that a `-q` log shows more than dots."""
+    from tests import parity
+    if parity.MARGINS:
+        terminalreporter.write_sep("-", "parity margins (CUDA path vs oracle)")
+        for line in parity.MARGINS:
+            terminalreporter.write_line(line)

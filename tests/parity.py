@@ -12,6 +12,14 @@ from paper_2409_16053_b200 import inputs as I
 
 NTHREADS = max(1, os.cpu_count() or 1)     # oracle OpenMP threads: bit-identical to 1 thread (orc.h)
 
+MARGINS = []                               # one line per parity run; tests/conftest.py prints them in the summary
+
+
+def report(line: str) -> None:
+    """Record how far inside its bar a parity run ended (shown after the dots of `pytest -q`)."""
+    MARGINS.append(line)
+    print(line)
+
 
 def active(mesh):
     g = mesh.ng

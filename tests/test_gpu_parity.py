@@ -50,6 +50,9 @@ def run_lockstep(orc, ak, w, nsteps, variant=0, check_ghosts=True, rsolver=0):
                 assert e <= TOL_STAGE * stage, f"stage {stage}: Q14 = {e:.3e}"
         errs.append(P.q14(P.gpu_state(pg)[a], po.current()[a], w.gamma))
     assert po.floor_count() == 0 and pg.floor_count() == 0
+    # one line per parity run in the test log (pytest -s / the driver's captured tail): how far inside the bars
+    P.report(f"[parity] {w.name} nmb={w.mesh.nmb} nx={tuple(w.mesh.nx)} recon={w.recon} rsolver={rsolver} variant={variant} "
+          f"steps={nsteps}: worst Q14 per step {max(errs):.3e} (bar {TOL_RUN:.0e}), first step {errs[0]:.3e}")
     return errs, po, pg, U0
 
 
@@ -296,13 +299,24 @@ def _subbox(G, origin, n):
     return G.index_select(1, idx[2]).index_select(2, idx[1]).index_select(3, idx[0]).cpu().numpy()
 
 
+def _dt_reference(G, gamma, dx, cfl):
+    """Eq.(3) on the assembled global state with torch ops on the device (not the library's kernels)."""
+    rho, mom, E = G[0], G[1:4], G[4]
+    p = (gamma - 1.0) * (E - 0.5 * (mom ** 2).sum(0) / rho)
+    cs = torch.sqrt(gamma * p / rho)
+    return cfl * min(float((dx[d] / (mom[d].abs() / rho + cs)).min()) for d in range(3))
+
+
 def test_config3_full_size_sampled(orc, ak):
-    """BASELINE config 3 at its full size (64 MeshBlocks of 128^3, the launch configuration bench.py times):
-    one RK2 step on the GPU, checked on sampled 32^3 sub-boxes that the oracle advances one by one.  A cell's RK2
+    """BASELINE config 3 at its full size (64 MeshBlocks of 128^3, the launch configuration bench.py times: 16 x 10
+    tiles, one k-chunk, the dt of steps 2 and 3 taken from the reduction fused into stage 2 of the step before):
+    THREE RK2 steps on the GPU, checked on sampled 64^3 sub-boxes that the oracle advances one by one.  A cell's RK2
     update depends on cells within 2 x 3 of it (two PPM4 stages), so the oracle, run on a sub-box as its own small
-    periodic block with the same dx and dt, is exact on the cells >= 6 away from the sub-box faces.  The boxes
-    sit on a corner where 8 blocks meet, on the periodic wrap of the domain, on the shear layers and inside a
-    block (every box spans several 16 x 10 tiles).  Plus what holds at any size: conservation and no floors."""
+    periodic block with the same dx and the same dt sequence, is exact on the cells >= 18 away from the sub-box
+    faces after three steps (pad 20 -> 24^3 cells compared per box).  The boxes sit on a corner where 8 blocks
+    meet, on the periodic wrap of the domain, on the shear layers and inside a block (every box spans several
+    tiles).  Plus what holds at any size: conservation, no floors, and each step's dt against Eq.(3) evaluated with
+    torch on the assembled state."""
     w = I.config3()
     dev = torch.device("cuda", 0)
     pg = ak.Pack(w.mesh, w.gamma, w.recon, device=dev)
@@ -310,22 +324,27 @@ def test_config3_full_size_sampled(orc, ak):
     pg.load(U0)
     G0 = _assemble(w.mesh, U0)
     del U0
-    n, pad = 32, 8
-    origins = [(112, 112, 112), (496, 496, 496), (300, 112, 200), (40, 368, 500), (200, 50, 60), (240, 250, 260)]
+    nsteps, n, pad = 3, 64, 20
+    origins = [(96, 96, 96), (480, 480, 480), (300, 96, 200), (40, 352, 500), (200, 50, 60), (240, 250, 260)]
     subs0 = [_subbox(G0, o, n) for o in origins]
     tot0 = G0.sum(dim=(1, 2, 3)).cpu().numpy()
     rho, mom, E = G0[0], G0[1:4], G0[4]
     p = (w.gamma - 1.0) * (E - 0.5 * (mom ** 2).sum(0) / rho)
-    cs = torch.sqrt(w.gamma * p / rho)
+    mnorm = float((mom.norm(dim=0) + rho * torch.sqrt(w.gamma * p / rho)).sum())
     dx = w.mesh.dx(0)
-    dt_ref = w.cfl * min(float((dx[d] / (mom[d].abs() / rho + cs)).min()) for d in range(3))
-    mnorm = float((mom.norm(dim=0) + rho * cs).sum())
-    del G0, rho, mom, E, p, cs
-    dt = pg.new_dt(w.cfl)
-    assert abs(dt - dt_ref) <= 1e-13 * dt_ref
-    pg.step(w.cfl, dt)
+    dt_ref = _dt_reference(G0, w.gamma, dx, w.cfl)
+    del G0, rho, mom, E, p
+    dts = []
+    for step in range(nsteps):
+        dt = pg.new_dt(w.cfl)                    # step 0: stand-alone reduction; later: from stage 2 of the step before
+        assert abs(dt - dt_ref) <= 1e-13 * dt_ref, (step, dt, dt_ref)
+        pg.step(w.cfl, dt)
+        dts.append(dt)
+        G1 = _assemble(w.mesh, pg.current())
+        dt_ref = _dt_reference(G1, w.gamma, dx, w.cfl)
+        if step + 1 < nsteps:
+            del G1
     assert pg.floor_count() == 0
-    G1 = _assemble(w.mesh, pg.current())
     tot1 = G1.sum(dim=(1, 2, 3)).cpu().numpy()
     scale = np.array([tot0[0], mnorm, mnorm, mnorm, tot0[4]])
     assert (np.abs(tot1 - tot0) / scale).max() <= TOL_TOTALS
@@ -334,18 +353,19 @@ def test_config3_full_size_sampled(orc, ak):
     g = w.mesh.ng
     worst = 0.0
     for o, s0 in zip(origins, subs0):
-        po = orc.OrcPack(sub_mesh, w.gamma, w.recon, threads=1)
+        po = orc.OrcPack(sub_mesh, w.gamma, w.recon, threads=P.NTHREADS)
         u = np.zeros(sub_mesh.state_shape())
         u[0][:, g:-g, g:-g, g:-g] = s0
         po.load(u)
-        po.step(w.cfl, dt)
+        for dt in dts:
+            po.step(w.cfl, dt)
         ref = po.current()[0][:, g + pad:-g - pad, g + pad:-g - pad, g + pad:-g - pad]
         got = _subbox(G1, o, n)[:, pad:-pad, pad:-pad, pad:-pad]
         e = P.q14(got[None], ref[None], w.gamma)
         worst = max(worst, e)
-        assert e <= 2 * TOL_STAGE, (o, e)
+        assert e <= 2 * nsteps * TOL_STAGE, (o, e)
         po.close()
-    print(f"cfg3 full size: worst sampled Q14 after one RK2 step = {worst:.2e}")
+    P.report(f"[parity] cfg3 full size (64 x 128^3, bench launch configuration): worst sampled Q14 after {nsteps} RK2 steps = {worst:.2e}")
 
 
 # ------------------------------------------------------------ flux correction --------
@@ -446,6 +466,61 @@ def test_llf_hlle_only_in_the_production_kernel(ak):
         pg.hydro_stage(1, 1e-3)
 
 
+# ------------------------------------------------------------ strong collisions / non-finite states ----
+@pytest.mark.parametrize("recon,ng", [(0, 2), (1, 3)])
+def test_supersonic_inflow_into_a_wall_matches_the_oracle(orc, ak, recon, ng):
+    """Mach-5 stream running into a reflecting wall (the mirror state makes the face a symmetric head-on collision):
+    finite, floor-free, within the bar of the oracle, and the wall carries no mass flux (mass is conserved)."""
+    import dataclasses
+    g = 5.0 / 3.0
+    mesh = dataclasses.replace(I.uniform_mesh((2, 1, 1), (16, 8, 8), ng), bc=(1, 2, 0, 0, 0, 0))   # outflow left, wall right
+    c = (g * 1.0 / 1.0) ** 0.5
+    prim = lambda X1, X2, X3: (1.0 + 0.1 * torch.sin(6.283185307179586 * X2), 5.0 * c + 0 * X1, 0.2 + 0 * X1, 0 * X1, 1.0 + 0 * X1)
+    U0 = I.make_state(mesh, prim, gamma=g)
+    po = orc.OrcPack(mesh, g, recon, threads=P.NTHREADS)
+    pg = ak.Pack(mesh, g, recon)
+    po.load(U0.numpy()); pg.load(U0)
+    a = P.active(mesh)
+    worst = 0.0
+    for _ in range(8):
+        dt = po.new_dt(0.3)
+        assert abs(pg.new_dt(0.3) - dt) <= 1e-13 * dt              # (states differ by rounding after the first step)
+        po.step(0.3, dt); pg.step(0.3, dt)
+        ug = P.gpu_state(pg)[a]
+        assert np.all(np.isfinite(ug))
+        worst = max(worst, P.q14(ug, po.current()[a], g))
+    P.report(f"[parity] wall inflow Mach 5 recon={recon}: worst Q14 {worst:.3e}")
+    assert worst <= TOL_RUN
+    assert po.floor_count() == 0 and pg.floor_count() == 0
+    assert po.current()[a][:, 0].max() > 2.0               # the reflected shock has formed (density jump towards 4)
+
+
+def test_non_finite_state_is_reported_by_new_dt(orc, ak):
+    """a NaN in one active cell must not be skipped by the max / min reductions -- both the stand-alone
+    reduction and the one fused into the last stage return AK_ENONFINITE (-5), as the oracle reports it."""
+    w = I.config1(nrb=2, nx=16)
+    U0 = w.state()
+    po, pg = P.make_pair(orc, ak, w, U0)
+    dt = pg.new_dt(w.cfl)
+    assert dt == po.new_dt(w.cfl)
+    ng = w.mesh.ng
+    bad = U0.clone()
+    bad[3, 2, ng + 5, ng + 7, ng + 1] = float("nan")        # one momentum component of one cell
+    pg.load(bad); po.load(bad.numpy())
+    with pytest.raises(orc.OrcError):
+        po.new_dt(w.cfl)
+    with pytest.raises(ak.AkError) as ei:
+        pg.new_dt(w.cfl)                                    # stand-alone kernel
+    assert "non-finite" in str(ei.value)
+    pg.step(w.cfl, dt)                                      # the NaN spreads; stage 2 reduces the speeds of its result
+    with pytest.raises(ak.AkError) as ei:
+        pg.new_dt(w.cfl)                                    # fused path
+    assert "non-finite" in str(ei.value)
+    # a healthy state afterwards works again
+    pg.load(U0)
+    assert pg.new_dt(w.cfl) == dt
+
+
 # ------------------------------------------------------------ outflow / reflecting boundaries (SURVEY 8(f) f3) --------
 @pytest.mark.parametrize("bc", [(1, 1, 0, 0, 2, 2), (2, 2, 2, 2, 2, 2), (0, 0, 1, 1, 0, 0), (2, 1, 1, 2, 1, 1)])
 @pytest.mark.parametrize("recon,ng", [(0, 2), (1, 3)])
@@ -453,14 +528,15 @@ def test_physical_boundaries_match_the_oracle(orc, ak, bc, recon, ng):
     """Ghost cells bit-exact after every fill (run_lockstep checks them at step 0 against the oracle's fill of the
     GPU's own active cells), states within the run tolerance."""
     import dataclasses
-    # the Mach-0.3 field of config 1 for both reconstructions: at rms Mach 1 (config 3) patches of the flow run into a
-    # wall at Mach > 1.9, where the PVRS wave-speed estimate of the HLLC reading (DESIGN.md Q2) gives S_L > 0 > S_R
-    # and the star-state flux is 0/0 -- in the oracle as on the GPU; that is a property of the reading, not of the walls
-    w = I.config1(nrb=2, nx=16)
-    w.recon = recon
-    w.mesh = dataclasses.replace(I.uniform_mesh((2, 2, 1), (16, 12, 8), ng), bc=bc)
-    errs, po, pg, U0 = run_lockstep(orc, ak, w, 3)
-    assert max(errs) <= TOL_RUN, (bc, errs)
+    # the Mach-0.3 field of config 1 and the Mach-1 field of config 3, where patches of the flow run into a wall at
+    # Mach > 1.9: with the round-1 pressure-based HLLC speeds that gave 0/0 on both sides (DESIGN.md Q26); with
+    # Davis's speeds (Q2, round 2) the run is finite, floor-free and within the bar
+    for w in (I.config1(nrb=2, nx=16), I.config3(nrb=2, nx=16)):
+        w.recon = recon
+        w.mesh = dataclasses.replace(I.uniform_mesh((2, 2, 1), (16, 12, 8), ng), bc=bc)
+        errs, po, pg, U0 = run_lockstep(orc, ak, w, 3)
+        assert max(errs) <= TOL_RUN, (bc, errs)
+        assert np.all(np.isfinite(P.gpu_state(pg)[P.active(w.mesh)]))
     po.fill_ghosts(); pg.fill_ghosts()
     chk = orc.OrcPack(w.mesh, w.gamma, w.recon)
     chk.load(P.gpu_state(pg)); chk.fill_ghosts()
@@ -600,10 +676,11 @@ def test_forward_euler_matches_the_oracle(orc, ak):
         pg.set_integrator(2)
 
 
-@pytest.mark.parametrize("nx", [16, 128])
+@pytest.mark.parametrize("nx", [16, 32, 64, 128])
 def test_config2_full_size_sampled(orc, ak, nx):
-    """BASELINE config 2 at its full 256^3, at the two ends of the block-size sweep (4096 blocks of 16^3: every
-    sampled box spans 8-27 MeshBlocks; 8 blocks of 128^3), as bench.py runs it: two RK2 steps on the GPU against the
+    """BASELINE config 2 at its full 256^3, at every block size of the sweep (4096 blocks of 16^3: every sampled box
+    spans 8-27 MeshBlocks; 512 of 32^3 -- the variant BASELINE.json names for parity; 64 of 64^3; 8 blocks of 128^3),
+    as bench.py runs it: two RK2 steps on the GPU against the
     oracle on 32^3 sub-boxes (PLM: a step reaches 2 x 2 cells, two steps 8 = the margin dropped on each side).  The
     boxes sit on the blast (centre, edge of the hot sphere), on a block corner and on the periodic wrap."""
     w = I.config2(nx)
@@ -630,6 +707,7 @@ def test_config2_full_size_sampled(orc, ak, nx):
     sub_mesh = I.Mesh((1, 1, 1), (n, n, n), w.mesh.ng, [(0, 0, 0, 0)], xmax=(n * dx[0], n * dx[1], n * dx[2]))
     assert sub_mesh.dx(0) == dx
     g = w.mesh.ng
+    worst = 0.0
     for o, s0 in zip(origins, subs0):
         po = orc.OrcPack(sub_mesh, w.gamma, w.recon, threads=1)
         u = np.zeros(sub_mesh.state_shape())
@@ -640,5 +718,7 @@ def test_config2_full_size_sampled(orc, ak, nx):
         ref = po.current()[0][:, g + pad:-g - pad, g + pad:-g - pad, g + pad:-g - pad]
         got = _subbox(G1, o, n)[:, pad:-pad, pad:-pad, pad:-pad]
         e = P.q14(got[None], ref[None], w.gamma)
+        worst = max(worst, e)
         assert e <= 4 * TOL_STAGE, (nx, o, e)
         po.close()
+    P.report(f"[parity] cfg2 full size 256^3 in {nx}^3 blocks: worst sampled Q14 after 2 RK2 steps = {worst:.2e}")
