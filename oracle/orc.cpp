@@ -77,6 +77,83 @@ extern "C" void orc_ppm4(const double q[5], double* q_minus, double* q_plus) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// S2'  the higher-order reconstructions of the paper's option list ("PPM ... using extremum-preserving limiters
+// (McCorquodale et al. 2015, hereafter PPMX), and the improved WENOZ scheme"; both converge at fourth order on
+// the 1-D linear wave).  The paper defers the formulas; the readings are DESIGN.md Q29 (WENOZ) and Q30 (PPMX).
+// Both take the five values q[i-2..i+2] of one primitive along one direction and return q- (at i-1/2) and q+ (at i+1/2).
+// ------------------------------------------------------------------------------------------------
+// WENO-Z (Borges et al. 2008) fifth-order value at the UPPER face of the middle cell from the stencil (a,b,c,d,e) =
+// q[i-2..i+2]: candidate parabolas p_k, Jiang-Shu smoothness indicators beta_k, global indicator tau5 = |beta0 - beta2|,
+// weights alpha_k = d_k (1 + (tau5 / (beta_k + eps))^2) with d = (1/10, 6/10, 3/10), eps = 1e-40.
+static double wenoz_upper(double a, double b, double c, double d, double e) {
+  // written in the differences of neighbouring cells, so that constant data are reproduced exactly (uniform states
+  // must be preserved bit for bit): p_k = c + P_k / 6
+  const double d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
+  const double P0 = 5.0 * d2 - 2.0 * d1;          // (2a - 7b + 11c)/6 = c + P0/6
+  const double P1 = 2.0 * d3 + d2;                // (-b + 5c + 2d)/6  = c + P1/6
+  const double P2 = 4.0 * d3 - d4;                // (2c + 5d - e)/6   = c + P2/6
+  const double s0 = d2 - d1, t0 = 3.0 * d2 - d1;  // a - 2b + c,  a - 4b + 3c
+  const double s1 = d3 - d2, t1 = d2 + d3;        // b - 2c + d,  d - b
+  const double s2 = d4 - d3, t2 = d4 - 3.0 * d3;  // c - 2d + e,  3c - 4d + e
+  const double b0 = 13.0 / 12.0 * (s0 * s0) + 0.25 * (t0 * t0);
+  const double b1 = 13.0 / 12.0 * (s1 * s1) + 0.25 * (t1 * t1);
+  const double b2 = 13.0 / 12.0 * (s2 * s2) + 0.25 * (t2 * t2);
+  const double eps = 1e-40;
+  const double tau = std::fabs(b0 - b2);
+  const double r0 = tau / (b0 + eps), r1 = tau / (b1 + eps), r2 = tau / (b2 + eps);
+  const double a0 = 0.1 * (1.0 + r0 * r0), a1 = 0.6 * (1.0 + r1 * r1), a2 = 0.3 * (1.0 + r2 * r2);
+  return c + (a0 * P0 + (a1 * P1 + a2 * P2)) / (6.0 * (a0 + (a1 + a2)));
+}
+extern "C" void orc_wenoz(const double q[5], double* q_minus, double* q_plus) {
+  *q_plus  = wenoz_upper(q[0], q[1], q[2], q[3], q[4]);
+  *q_minus = wenoz_upper(q[4], q[3], q[2], q[1], q[0]);    // the mirrored stencil: exact mirror symmetry
+}
+
+// PPMX: fourth-order interface values, the Colella-Sekora (2008) / McCorquodale-Colella (2011) limiters.
+// (i) interface value between q0 and q1 from (qm1, q0, q1, q2): the fourth-order value; where it is not between q0 and
+// q1 it is replaced by (q0 + q1)/2 - D/6 with D the second difference limited among the face-centred one
+// 3 (q0 - 2 v + q1) and C times the two cell-centred ones (C = 5/4), zero unless all three share a sign.
+static double ppmx_iface(double qm1, double q0, double q1, double q2) {
+  const double C = 1.25;
+  double v = (7.0 * (q0 + q1) - (qm1 + q2)) / 12.0;
+  if ((v - q0) * (q1 - v) < 0.0) {
+    const double dc = 3.0 * ((q0 + q1) - 2.0 * v);               // (groupings symmetric under mirroring)
+    const double dl = (qm1 + q1) - 2.0 * q0, dr = (q0 + q2) - 2.0 * q1;
+    double D = 0.0;
+    if (dc > 0.0 && dl > 0.0 && dr > 0.0) D = std::fmin(dc, C * std::fmin(dl, dr));
+    else if (dc < 0.0 && dl < 0.0 && dr < 0.0) D = -std::fmin(-dc, C * std::fmin(-dl, -dr));
+    v = 0.5 * (q0 + q1) - D / 6.0;
+  }
+  return v;
+}
+// (ii) the parabola of cell i with edge values (aL, aR): at an extremum (of the parabola or of the cell averages) the
+// parabola's second derivative 6 (aL + aR - 2a) is limited among itself and C times the three cell-centred second
+// differences (zero unless all four share a sign) and both edge increments are scaled by the ratio -- a smooth
+// extremum keeps its parabola, which is what PPM4's "flatten at every extremum" cannot do; elsewhere CW84's monotonicity
+// constraint in the two-sided form (an edge increment at most twice the other).
+extern "C" void orc_ppmx(const double q[5], double* q_minus, double* q_plus) {
+  const double C = 1.25;
+  const double a = q[2];
+  double aL = ppmx_iface(q[0], q[1], q[2], q[3]);
+  double aR = ppmx_iface(q[1], q[2], q[3], q[4]);
+  const double dm = a - aL, dp = aR - a;
+  if (dm * dp <= 0.0 || (q[3] - a) * (a - q[1]) <= 0.0) {
+    const double df = 6.0 * ((aL + aR) - 2.0 * a);
+    const double d1 = (q[0] + q[2]) - 2.0 * q[1], d2 = (q[1] + q[3]) - 2.0 * q[2], d3 = (q[2] + q[4]) - 2.0 * q[3];
+    double D = 0.0;
+    if (df > 0.0 && d1 > 0.0 && d2 > 0.0 && d3 > 0.0) D = std::fmin(df, C * std::fmin(d1, std::fmin(d2, d3)));
+    else if (df < 0.0 && d1 < 0.0 && d2 < 0.0 && d3 < 0.0) D = -std::fmin(-df, C * std::fmin(-d1, std::fmin(-d2, -d3)));
+    const double rho = (df != 0.0) ? D / df : 0.0;
+    if (rho <= 1.0 - 1e-12) { aL = a - rho * dm; aR = a + rho * dp; }
+  } else {
+    if (std::fabs(dm) >= 2.0 * std::fabs(dp)) aL = a - 2.0 * dp;
+    if (std::fabs(dp) >= 2.0 * std::fabs(dm)) aR = a + 2.0 * dm;
+  }
+  *q_minus = aL;
+  *q_plus  = aR;
+}
+
+// ------------------------------------------------------------------------------------------------
 // S3  HLLC flux at one face (P:103 names the solver; formulas: Toro 2013 ch.10, restated)
 // Wave speeds (Q2, round-2 reading): Davis's direct estimates, Toro Eq.(10.48),
 //   S_L = min(u_L - c_L, u_R - c_R),   S_R = max(u_L + c_L, u_R + c_R).
@@ -237,9 +314,9 @@ extern "C" orc_pack* orc_pack_create(int nmb, int nx1, int nx2, int nx3, int ng,
   if (nmb < 1) { fail("nmb < 1"); return nullptr; }
   for (int d = 0; d < 3; d++) if (nx[d] < ng || (nx[d] & 1)) { fail("nx_d must be even and >= ng"); return nullptr; }
   if (!(gamma > 1.0)) { fail("gamma <= 1"); return nullptr; }
-  if (recon != 0 && recon != 1) { fail("unknown recon"); return nullptr; }
+  if (recon < 0 || recon > 3) { fail("unknown recon"); return nullptr; }
   if (rsolver < 0 || rsolver > 3) { fail("unknown rsolver"); return nullptr; }
-  if ((recon == 0 && ng < 2) || (recon == 1 && ng < 3)) { fail("ng too small for the reconstruction"); return nullptr; }
+  if ((recon == 0 && ng < 2) || (recon >= 1 && ng < 3)) { fail("ng too small for the reconstruction"); return nullptr; }
   orc_pack* p = new orc_pack;
   p->nmb = nmb; p->ng = ng; p->gamma = gamma; p->recon = recon; p->rsolver = rsolver;
   for (int d = 0; d < 3; d++) { p->nx[d] = nx[d]; p->nt[d] = nx[d] + 2 * ng; }
@@ -464,8 +541,9 @@ static long long block_fluxes(const orc_pack* p, const double* Uin, int m, FaceF
         } else {
           double sL[5] = { q[cm - 2 * str[d]], q[cm - str[d]], q[cm], q[cm + str[d]], q[cm + 2 * str[d]] };
           double sR[5] = { q[c - 2 * str[d]],  q[c - str[d]],  q[c],  q[c + str[d]],  q[c + 2 * str[d]] };
-          orc_ppm4(sL, &qm, &qp);                                             WL[n] = qp;
-          orc_ppm4(sR, &qm, &qp);                                             WR[n] = qm;
+          if (p->recon == 1)      { orc_ppm4(sL, &qm, &qp);  WL[n] = qp;  orc_ppm4(sR, &qm, &qp);  WR[n] = qm; }
+          else if (p->recon == 2) { orc_ppmx(sL, &qm, &qp);  WL[n] = qp;  orc_ppmx(sR, &qm, &qp);  WR[n] = qm; }
+          else                    { orc_wenoz(sL, &qm, &qp); WL[n] = qp;  orc_wenoz(sR, &qm, &qp); WR[n] = qm; }
         }
       }
       if (p->rsolver == 0) orc_hllc(p->gamma, d, WL, WR, Fl);

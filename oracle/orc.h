@@ -33,7 +33,7 @@ extern "C" {
 
 typedef struct orc_pack orc_pack;
 
-/* recon: 0 = PLM (van Leer), 1 = PPM4; rsolver: 0 = HLLC, 1 = LLF, 2 = HLLE, 3 = Roe.  NULL on invalid arguments. */
+/* recon: 0 = PLM (van Leer), 1 = PPM4, 2 = PPMX, 3 = WENOZ (ng >= 3 for 1-3); rsolver: 0 = HLLC, 1 = LLF, 2 = HLLE, 3 = Roe.  NULL on invalid arguments. */
 orc_pack* orc_pack_create(int nmb, int nx1, int nx2, int nx3, int ng, double gamma, int recon, int rsolver);
 int orc_pack_set_mesh(orc_pack*, int nrb1, int nrb2, int nrb3,
                       double x1min, double x1max, double x2min, double x2max, double x3min, double x3max);
@@ -61,6 +61,8 @@ void orc_c2p(double gamma, const double U[5], double W[5], int* floored);       
 void orc_plm(double qm1, double q0, double qp1, double* q_minus, double* q_plus);       /* S2 */
 void orc_ppm4(const double q[5] /* i-2..i+2 */, double* q_minus, double* q_plus);      /* S2 */
 void orc_ppm4_iface(double qm1, double q0, double qp1, double qp2, double* q_half);    /* S2 (i),(ii) */
+void orc_ppmx(const double q[5] /* i-2..i+2 */, double* q_minus, double* q_plus);      /* S2', f2: DESIGN.md Q30 */
+void orc_wenoz(const double q[5] /* i-2..i+2 */, double* q_minus, double* q_plus);     /* S2', f2: DESIGN.md Q29 */
 void orc_hllc(double gamma, int dir /*0,1,2*/, const double WL[5], const double WR[5], double F[5]); /* S3 */
 void orc_llf (double gamma, int dir, const double WL[5], const double WR[5], double F[5]);             /* S3', f2 */
 void orc_hlle(double gamma, int dir, const double WL[5], const double WR[5], double F[5]);             /* S3', f2 */

@@ -55,8 +55,9 @@ def lib():
     L.orc_c2p.restype = None
     L.orc_plm.argtypes = [C.c_double] * 3 + [dp, dp]
     L.orc_plm.restype = None
-    L.orc_ppm4.argtypes = [dp, dp, dp]
-    L.orc_ppm4.restype = None
+    for f in (L.orc_ppm4, L.orc_ppmx, L.orc_wenoz):
+        f.argtypes = [dp, dp, dp]
+        f.restype = None
     L.orc_ppm4_iface.argtypes = [C.c_double] * 4 + [dp]
     L.orc_ppm4_iface.restype = None
     L.orc_hllc.argtypes = [C.c_double, C.c_int, dp, dp, dp]
@@ -98,6 +99,18 @@ def plm(qm1, q0, qp1):
 def ppm4(q5):
     a, b = C.c_double(), C.c_double()
     lib().orc_ppm4(_arr5(q5), C.byref(a), C.byref(b))
+    return a.value, b.value
+
+
+def ppmx(q5):
+    a, b = C.c_double(), C.c_double()
+    lib().orc_ppmx(_arr5(q5), C.byref(a), C.byref(b))
+    return a.value, b.value
+
+
+def wenoz(q5):
+    a, b = C.c_double(), C.c_double()
+    lib().orc_wenoz(_arr5(q5), C.byref(a), C.byref(b))
     return a.value, b.value
 
 

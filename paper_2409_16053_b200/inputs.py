@@ -19,7 +19,7 @@ import torch
 
 GAMMA = 5.0 / 3.0          # BASELINE.json: all configs
 CFL = 0.3                  # BASELINE.json: all configs
-RECON_PLM, RECON_PPM4 = 0, 1
+RECON_PLM, RECON_PPM4, RECON_PPMX, RECON_WENOZ = 0, 1, 2, 3
 RSOLVER_HLLC = 0
 
 

@@ -38,6 +38,47 @@ def ppm4(q):
     nR = np.where(~c1 & c2, 3.0 * q - 2.0 * aL, aR)
     return np.where(flat, q, nL), np.where(flat, q, nR)
 
+def wenoz(q):
+    """WENO-Z, Q29: (q-, q+) of every cell from q[i-2..i+2] (periodic)."""
+    def upper(a, b, c, d, e):
+        d1, d2, d3, d4 = b - a, c - b, d - c, e - d
+        P0, P1, P2 = 5 * d2 - 2 * d1, 2 * d3 + d2, 4 * d3 - d4
+        b0 = 13 / 12 * (d2 - d1) ** 2 + 0.25 * (3 * d2 - d1) ** 2
+        b1 = 13 / 12 * (d3 - d2) ** 2 + 0.25 * (d2 + d3) ** 2
+        b2 = 13 / 12 * (d4 - d3) ** 2 + 0.25 * (d4 - 3 * d3) ** 2
+        tau = np.abs(b0 - b2)
+        a0, a1, a2 = (w * (1 + (tau / (b + 1e-40)) ** 2) for w, b in ((0.1, b0), (0.6, b1), (0.3, b2)))
+        return c + (a0 * P0 + (a1 * P1 + a2 * P2)) / (6 * (a0 + (a1 + a2)))
+    m2, m1, p1, p2 = np.roll(q, 2), np.roll(q, 1), np.roll(q, -1), np.roll(q, -2)
+    return upper(p2, p1, q, m1, m2), upper(m2, m1, q, p1, p2)
+
+def ppmx(q):
+    """PPMX, Q30: fourth-order interfaces + Colella-Sekora / McCorquodale-Colella limiters (C = 5/4)."""
+    C = 1.25
+    m2, m1, p1, p2 = np.roll(q, 2), np.roll(q, 1), np.roll(q, -1), np.roll(q, -2)
+    def lim3(dc, dl, dr):
+        pos = (dc > 0) & (dl > 0) & (dr > 0); neg = (dc < 0) & (dl < 0) & (dr < 0)
+        return np.where(pos, np.minimum(dc, C * np.minimum(dl, dr)), np.where(neg, -np.minimum(-dc, C * np.minimum(-dl, -dr)), 0.0))
+    v = (7.0 * (q + p1) - (m1 + p2)) / 12.0                        # interface i+1/2
+    bad = (v - q) * (p1 - v) < 0.0
+    D = lim3(3.0 * ((q + p1) - 2.0 * v), (m1 + p1) - 2.0 * q, (q + p2) - 2.0 * p1)
+    v = np.where(bad, 0.5 * (q + p1) - D / 6.0, v)
+    aR, aL = v, np.roll(v, 1)
+    dm, dp = q - aL, aR - q
+    ext = (dm * dp <= 0.0) | ((p1 - q) * (q - m1) <= 0.0)
+    df = 6.0 * ((aL + aR) - 2.0 * q)
+    d1, d2, d3 = (m2 + q) - 2.0 * m1, (m1 + p1) - 2.0 * q, (q + p2) - 2.0 * p1
+    pos = (df > 0) & (d1 > 0) & (d2 > 0) & (d3 > 0); neg = (df < 0) & (d1 < 0) & (d2 < 0) & (d3 < 0)
+    Dl = np.where(pos, np.minimum(df, C * np.minimum(d1, np.minimum(d2, d3))),
+                  np.where(neg, -np.minimum(-df, C * np.minimum(-d1, np.minimum(-d2, -d3))), 0.0))
+    with np.errstate(divide="ignore", invalid="ignore"):
+        rho = np.where(df != 0.0, Dl / df, 0.0)
+    use = rho <= 1.0 - 1e-12
+    eL = np.where(use, q - rho * dm, aL); eR = np.where(use, q + rho * dp, aR)
+    mL = np.where(np.abs(dm) >= 2.0 * np.abs(dp), q - 2.0 * dp, aL)
+    mR = np.where(np.abs(dp) >= 2.0 * np.abs(dm), q + 2.0 * dm, aR)
+    return np.where(ext, eL, mL), np.where(ext, eR, mR)
+
 def hllc(WL, WR):
     rL, uL, eL = WL; rR, uR, eR = WR
     pL, pR = (G - 1) * eL, (G - 1) * eR
@@ -62,7 +103,7 @@ def rhs(U, recon):
     F = hllc(WL, WR)                                             # flux at the lower face of cell i
     return -(np.roll(F, -1, axis=1) - F)
 
-def run(N, recon, cfl, amp=1e-6):
+def run(N, recon, cfl, amp=1e-6, rk3=False):
     x = (np.arange(N) + 0.5) / N
     s = np.sin(2 * math.pi * x)
     rho, v, P = 1.0 + amp * s, amp * s, 1.0 / G + amp * s
@@ -73,7 +114,11 @@ def run(N, recon, cfl, amp=1e-6):
         dt = cfl * np.min(dx / (np.abs(W[1]) + np.sqrt(G * ((G - 1) * W[2]) / W[0])))
         if t + dt > 1.0: dt = 1.0 - t
         U1 = U + dt / dx * rhs(U, recon)
-        U = 0.5 * U + 0.5 * (U1 + dt / dx * rhs(U1, recon))
+        if rk3:                                                  # SSPRK(3,3), Q27
+            U2 = 0.75 * U + 0.25 * (U1 + dt / dx * rhs(U1, recon))
+            U = (1.0 / 3.0) * U + (2.0 / 3.0) * (U2 + dt / dx * rhs(U2, recon))
+        else:
+            U = 0.5 * U + 0.5 * (U1 + dt / dx * rhs(U1, recon))
         t += dt
     return math.sqrt(sum(np.abs(U[n] - U0[n]).mean() ** 2 for n in range(3)))
 
@@ -81,7 +126,11 @@ if __name__ == "__main__":
     out = {"source": "tests/golden/make_appendix_c.py (stand-alone 1-D numpy scheme; Davis wave speeds, DESIGN.md Q2); "
                      "sound wave A=1e-6, gamma=5/3, one period",
            "plm_cfl0.3": {str(N): run(N, plm, 0.3) for N in (16, 32, 64, 128, 256)},
-           "ppm4_cfl0.1": {str(N): run(N, ppm4, 0.1) for N in (32, 64, 128)}}
+           "ppm4_cfl0.1": {str(N): run(N, ppm4, 0.1) for N in (32, 64, 128)},
+           # P:130 "fourth-order convergence ... for PPMX and WENOZ": SSPRK(3,3), CFL = 0.4 (16/N)^(1/3) so that the
+           # time error falls at fourth order too
+           "wenoz_rk3": {str(N): run(N, wenoz, 0.4 * (16.0 / N) ** (1.0 / 3.0), rk3=True) for N in (16, 32, 64, 128)},
+           "ppmx_rk3": {str(N): run(N, ppmx, 0.4 * (16.0 / N) ** (1.0 / 3.0), rk3=True) for N in (16, 32, 64, 128)}}
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "appendix_c.json")
     with open(path, "w") as f:
         json.dump(out, f, indent=1)

@@ -188,7 +188,7 @@ def test_sound_wave_second_order_ppm4(orc):
         assert 3.6 <= e[N] / e[2 * N] <= 4.3, e
 
 
-@pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3)])
+@pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3), (I.RECON_PPMX, 3), (I.RECON_WENOZ, 3)])
 def test_sound_wave_along_x2_x3_matches_x1(orc, recon, ng):
     e1 = wave_error(orc, 32, recon, ng, 0.3, 0)
     assert wave_error(orc, 32, recon, ng, 0.3, 1) == e1
@@ -201,7 +201,7 @@ def totals(mesh, U):
     return np.array([math.fsum(U[a][:, n].ravel()) for n in range(5)])
 
 
-@pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3)])
+@pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3), (I.RECON_PPMX, 3), (I.RECON_WENOZ, 3)])
 def test_conservation_on_periodic_multiblock_mesh(orc, recon, ng):
     mesh = I.uniform_mesh((2, 2, 2), (16, 16, 16), ng)
     U0 = I.make_state(mesh, I.modes_prim(0.5, shear=False, rho_pert=True)).numpy()
@@ -216,7 +216,7 @@ def test_conservation_on_periodic_multiblock_mesh(orc, recon, ng):
     assert np.abs(U[a] - U0[a]).max() > 1e-3               # the state did evolve
 
 
-@pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3)])
+@pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3), (I.RECON_PPMX, 3), (I.RECON_WENOZ, 3)])
 def test_uniform_state_is_preserved_bit_exactly(orc, recon, ng):
     mesh = I.uniform_mesh((2, 1, 1), (8, 8, 8), ng)
     prim = lambda X1, X2, X3: (1.3 + 0 * X1, 0.4 + 0 * X1, -0.7 + 0 * X1, 0.2 + 0 * X1, 0.9 + 0 * X1)
@@ -358,7 +358,7 @@ def test_colliding_supersonic_streams_converge_to_the_exact_two_shock_solution(o
     assert errs[256] < 0.75 * errs[128] and errs[512] < 0.75 * errs[256], errs
 
 
-@pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3)])
+@pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3), (I.RECON_PPMX, 3), (I.RECON_WENOZ, 3)])
 def test_decomposition_invariance_bit_exact(orc, recon, ng):
     """Same global field cut into 1x32^3, 8x16^3 and 64x8^3 blocks gives identical active cells."""
     results = []
@@ -374,7 +374,7 @@ def test_decomposition_invariance_bit_exact(orc, recon, ng):
     assert np.array_equal(results[0], results[2])
 
 
-@pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3)])
+@pytest.mark.parametrize("recon,ng", [(I.RECON_PLM, 2), (I.RECON_PPM4, 3), (I.RECON_PPMX, 3), (I.RECON_WENOZ, 3)])
 def test_mirror_symmetry_bit_exact_and_axis_permutation(orc, recon, ng):
     mesh = I.uniform_mesh((1, 1, 1), (16, 16, 16), ng)
     U0 = I.make_state(mesh, I.modes_prim(0.8, shear=False, rho_pert=True)).numpy()
