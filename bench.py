@@ -27,12 +27,9 @@ METRIC = "3D hydro cell-updates/sec (fp64)"
 UNIT = "cell-updates/s"
 BYTES_PER_CELL_UPDATE = 200.0      # 5 streams x 5 vars x 8 B per RK2 cell-update
 BYTES_STAGE = {1: 80.0, 2: 120.0}  # per active cell: stage 1 reads U^n writes U^(1); stage 2 reads U^(1),U^n writes
-# FP64-pipe thread instructions per active cell per stage launch of the PPM4+HLLC kernel, counted by ncu on
-# cfg3 (profiles/r01_v3_stage_cfg3.md: 656 in stage 1, 708 in stage 2, which also takes the next step's CFL
-# reduction), and the same capture's DRAM bytes per stage launch (12.29 GB and 17.69 GB); both are properties of
-# the committed kernel, not of this run
-FP64_INSTR_PER_CELL_STAGE_PPM = 682.0
-NCU_DRAM_BYTES_PER_STAGE_LAUNCH_CFG3 = 14.99e9
+# ncu's DRAM bytes and FP64-pipe instructions per stage launch come from profiles/r02_stage_counters_<workload>.json
+# (written by paper_2409_16053_b200/counters.py from an ncu pass of THIS command); they are printed only while the hash
+# of the kernel sources stored there equals the hash of the tree this runs from
 FP64_LANES_PER_SM = 64             # DESIGN.md 6.1 (ncu peak_sustained of the dfma counter / SM count)
 
 
@@ -162,6 +159,8 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
 
     w = workloads()[args.workload]()
+    if args.recon is not None:
+        w.recon = {"plm": 0, "ppm4": 1, "ppmx": 2, "wenoz": 3}[args.recon]
     mesh = w.mesh
     pack = ak.Pack(mesh, w.gamma, w.recon, rsolver={"hllc": 0, "llf": 1, "hlle": 2, "roe": 3}[args.rsolver], device=dev,
                    variant=args.variant)
@@ -214,9 +213,13 @@ def run_ours(args):
     alg_bytes = (BYTES_STAGE[1] + (nst - 1) * BYTES_STAGE[2]) / nst * ncell
     peaks, which = measured_peaks()
     achieved = alg_bytes / (stage_ms * 1e-3) / 1e9
+    from paper_2409_16053_b200 import counters
+    ctr = counters.load(args.workload) if (args.variant == 0 and args.rsolver == "hllc" and args.integrator == 2
+                                            and args.recon is None and not args.flux_correction) else None
     traffic = args.traffic
-    if traffic is None and args.workload == "cfg3" and args.variant == 0:
-        traffic = NCU_DRAM_BYTES_PER_STAGE_LAUNCH_CFG3
+    if traffic is None and ctr:
+        L = ctr["launches"]
+        traffic = sum(L[k]["dram__bytes_read.sum"] + L[k]["dram__bytes_write.sum"] for k in ("stage1", "stage2")) / 2.0
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "peak_source": which + " (MEASURED_PEAKS.json hbm_gbs)",
                 "kernel": "ak_hydro_stage", "kernel_ms": stage_ms, "kernel_share_of_step": nst * stage_ms * args.steps / elapsed_ms,
@@ -226,13 +229,24 @@ def run_ours(args):
 
     # the unit that actually binds the stage kernel is the FP64 pipe (plain ALU work)
     roofline_alu = None
-    if w.recon == 1:
+    if ctr:
+        L = ctr["launches"]
         sms = torch.cuda.get_device_properties(dev).multi_processor_count
         peak_alu = sms * FP64_LANES_PER_SM * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
-        ach_alu = FP64_INSTR_PER_CELL_STAGE_PPM * ncell / (stage_ms * 1e-3) / 1e12
+        # warp instructions on the FP64 pipe x 32 lanes, per stage launch (mean of the two stages)
+        fp64_thread_instr = 32.0 * sum(L[k]["sm__inst_executed_pipe_fp64.sum"] for k in ("stage1", "stage2")) / 2.0
+        alu_thread_instr = 32.0 * sum(L[k]["sm__inst_executed_pipe_alu.sum"] for k in ("stage1", "stage2")) / 2.0
+        ach_alu = fp64_thread_instr / (stage_ms * 1e-3) / 1e12
         roofline_alu = {"bound": "alu", "achieved": ach_alu, "peak": peak_alu, "unit": "T FP64-pipe thread-instr/s",
                         "frac": ach_alu / peak_alu, "kernel": "ak_hydro_stage",
-                        "instr_per_cell_launch": FP64_INSTR_PER_CELL_STAGE_PPM,
+                        "instr_per_cell_launch": fp64_thread_instr / ncell,
+                        "alu_pipe_instr_per_cell_launch": alu_thread_instr / ncell,
+                        # on this part FP64-pipe and ALU-pipe warp instructions issue at 2 cycles each and
+                        # overlap only partly; the fraction below is of the limit the probe measured for an ideally
+                        # interleaved stream, 0.78 x 2 cycles x (FP64 + ALU instructions)
+                        "frac_of_dispatch_limit": 0.78 * 2.0 * (fp64_thread_instr + alu_thread_instr) / 32.0
+                                                  / (sms * 4 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 * stage_ms * 1e-3),
+                        "counters": f"profiles/r02_stage_counters_{args.workload}.json (csrc hash {ctr['csrc_sha']})",
                         "peak_source": f"{sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x sm_max_mhz (DESIGN.md 6.1)"}
 
     # ---- end to end through the C-ABI with HOST buffers ------------------------------------------
@@ -286,7 +300,7 @@ def run_ours(args):
             "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{args.workload}: {w.name}", "nmb": mesh.nmb, "nx": list(mesh.nx), "ng": mesh.ng,
-                       "recon": "PPM4" if w.recon else "PLM", "rsolver": args.rsolver.upper(), "integrator": "SSPRK2" if args.integrator == 2 else "SSPRK3", "cfl": w.cfl,
+                       "recon": ["PLM", "PPM4", "PPMX", "WENOZ"][w.recon], "rsolver": args.rsolver.upper(), "integrator": "SSPRK2" if args.integrator == 2 else "SSPRK3", "cfl": w.cfl,
                        "cells": ncell, "state_bytes": state_bytes, "l2_policy": "inputs larger than L2 (no flush needed)"
                        if state_bytes > 4e8 else "state fits L2: numbers are L2-resident", "variant": args.variant, "flux_correction": bool(args.flux_correction),
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
@@ -307,8 +321,10 @@ def main():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--e2e-pipelined", action="store_true",
-                    help="also time the end-to-end path with two packs on two streams (upload and download overlapped)")
+    ap.add_argument("--no-e2e-pipelined", dest="e2e_pipelined", action="store_false",
+                    help="skip the second end-to-end figure (two packs on two streams, upload and download overlapped)")
+    ap.add_argument("--recon", default=None, choices=["plm", "ppm4", "ppmx", "wenoz"],
+                    help="override the workload's reconstruction (ppmx / wenoz: SURVEY 8(f) f2, need a workload with ng = 3)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--rsolver", default="hllc", choices=["hllc", "llf", "hlle", "roe"],
                     help="Riemann solver (headline metric: hllc; llf / hlle are the f2 variants on the same kernel)")

@@ -38,6 +38,8 @@ extern "C" {
 
 #define AK_RECON_PLM   0      /* piecewise linear, van Leer limiter     */
 #define AK_RECON_PPM4  1      /* piecewise parabolic, Colella-Woodward limiters */
+#define AK_RECON_PPMX  2      /* PPM with extremum-preserving limiters; ng >= 3; HLLC, production kernel only */
+#define AK_RECON_WENOZ 3      /* fifth-order WENO-Z; ng >= 3; HLLC, production kernel only */
 #define AK_RSOLVER_HLLC 0
 #define AK_RSOLVER_LLF  1     /* Rusanov, a = max(|u|+c) of the two states            */
 #define AK_RSOLVER_HLLE 2     /* Einfeldt speeds from the Roe averages                */

@@ -49,9 +49,9 @@ extern "C" ak_pack* ak_pack_create(int nmb, int nx1, int nx2, int nx3, int ng, d
   for (int d = 0; d < 3; d++)
     if (nx[d] < ng || (nx[d] & 1) || nx[d] < 2) { fail(AK_EINVAL, "nx_d must be even and >= ng"); return nullptr; }
   if (!(gamma > 1.0)) { fail(AK_EINVAL, "gamma <= 1"); return nullptr; }
-  if (recon != AK_RECON_PLM && recon != AK_RECON_PPM4) { fail(AK_EINVAL, "unknown recon"); return nullptr; }
+  if (recon < AK_RECON_PLM || recon > AK_RECON_WENOZ) { fail(AK_EINVAL, "unknown recon"); return nullptr; }
   if (rsolver < AK_RSOLVER_HLLC || rsolver > AK_RSOLVER_ROE) { fail(AK_EINVAL, "unknown rsolver"); return nullptr; }
-  if ((recon == AK_RECON_PLM && ng < 2) || (recon == AK_RECON_PPM4 && ng < 3)) {
+  if ((recon == AK_RECON_PLM && ng < 2) || (recon >= AK_RECON_PPM4 && ng < 3)) {
     fail(AK_EINVAL, "ng too small for the reconstruction stencil"); return nullptr;
   }
   long long ncell = (long long)(nx1 + 2 * ng) * (nx2 + 2 * ng) * (nx3 + 2 * ng);
@@ -278,6 +278,8 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
   if (!p->ghosts_ok) return fail(AK_ESTATE, "ak_fill_ghosts must precede ak_hydro_stage");
   if (p->rsolver != AK_RSOLVER_HLLC && (p->variant != 0 || ((p->d.ng - (p->recon == 0 ? 2 : 3)) & 1)))
     return fail(AK_EUNSUPPORTED, "LLF / HLLE / Roe exist in the production kernel only (variant 0, ng - stencil radius even)");
+  if (p->recon >= AK_RECON_PPMX && (p->variant != 0 || ((p->d.ng - 3) & 1) || p->rsolver != AK_RSOLVER_HLLC))
+    return fail(AK_EUNSUPPORTED, "PPMX / WENOZ exist in the production kernel with HLLC only (variant 0, ng - 3 even)");
   // Shu-Osher forms, every stage U_out = g0 U_in + g1 U^n + beta dt L(U_in) (Q1, Q27):
   //   SSPRK(2,2): (0,1,1), (1/2,1/2,1/2);   SSPRK(3,3): (0,1,1), (1/4,3/4,1/4), (2/3,1/3,2/3)
   static const double C2[2][3] = {{0.0, 1.0, 1.0}, {0.5, 0.5, 0.5}};

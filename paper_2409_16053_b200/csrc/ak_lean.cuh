@@ -80,11 +80,78 @@ __device__ __forceinline__ void limit_lean(double a, double& aL, double& aR) {
   aR = flat ? a : (cR ? nR : aR);
 }
 
-// q-/q+ of the cell at p[0] from the stencil along stride st: RECON 0 = PLM, 1 = PPM4
+// ---- S2'  PPMX and WENOZ (paper P:101; Q29, Q30), straight-line -----------------------------
+// select-min on doubles without the NaN handling of fmin (operands are finite here)
+__device__ __forceinline__ double dmin2(double a, double b) { return a < b ? a : b; }
+
+// WENO-Z value at the UPPER face of the middle cell of (a, b, c, d, e), in the differences of neighbouring cells
+// (constants are reproduced exactly); same operation order as the oracle, reciprocals by rcp2
+__device__ __forceinline__ double wenoz_upper(double a, double b, double c, double d, double e) {
+  const double d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
+  const double P0 = 5.0 * d2 - 2.0 * d1, P1 = 2.0 * d3 + d2, P2 = 4.0 * d3 - d4;
+  const double s0 = d2 - d1, t0 = 3.0 * d2 - d1;
+  const double s1 = d3 - d2, t1 = d2 + d3;
+  const double s2 = d4 - d3, t2 = d4 - 3.0 * d3;
+  const double b0 = (13.0 / 12.0) * (s0 * s0) + 0.25 * (t0 * t0);
+  const double b1 = (13.0 / 12.0) * (s1 * s1) + 0.25 * (t1 * t1);
+  const double b2 = (13.0 / 12.0) * (s2 * s2) + 0.25 * (t2 * t2);
+  const double eps = 1e-40;
+  const double tau = fabs(b0 - b2);
+  const double r0 = tau * rcp2(b0 + eps), r1 = tau * rcp2(b1 + eps), r2 = tau * rcp2(b2 + eps);
+  const double a0 = 0.1 * (1.0 + r0 * r0), a1 = 0.6 * (1.0 + r1 * r1), a2 = 0.3 * (1.0 + r2 * r2);
+  return c + (a0 * P0 + (a1 * P1 + a2 * P2)) * rcp2(6.0 * (a0 + (a1 + a2)));
+}
+__device__ __forceinline__ void wenoz_lean(const double q[5], double& qm, double& qp) {
+  qp = wenoz_upper(q[0], q[1], q[2], q[3], q[4]);
+  qm = wenoz_upper(q[4], q[3], q[2], q[1], q[0]);
+}
+
+// PPMX (i): fourth-order interface value between q0 and q1, limited where it is not between them
+__device__ __forceinline__ double ppmx_iface(double qm1, double q0, double q1, double q2) {
+  const double v = (7.0 * (q0 + q1) - (qm1 + q2)) * (1.0 / 12.0);
+  const double dc = 3.0 * ((q0 + q1) - 2.0 * v);
+  const double dl = (qm1 + q1) - 2.0 * q0, dr = (q0 + q2) - 2.0 * q1;
+  const bool same = (dc > 0.0 && dl > 0.0 && dr > 0.0) || (dc < 0.0 && dl < 0.0 && dr < 0.0);
+  const double m = dmin2(fabs(dc), 1.25 * dmin2(fabs(dl), fabs(dr)));
+  const double D = same ? copysign(m, dc) : 0.0;
+  const double lim = 0.5 * (q0 + q1) - D * (1.0 / 6.0);
+  return ((v - q0) * (q1 - v) < 0.0) ? lim : v;
+}
+// PPMX (ii): limited parabola of the middle cell of q[i-2..i+2]
+__device__ __forceinline__ void ppmx_lean(const double q[5], double& qm, double& qp) {
+  const double a = q[2];
+  const double aL = ppmx_iface(q[0], q[1], q[2], q[3]);
+  const double aR = ppmx_iface(q[1], q[2], q[3], q[4]);
+  const double dm = a - aL, dp = aR - a;
+  const bool ext = (dm * dp <= 0.0) || ((q[3] - a) * (a - q[1]) <= 0.0);
+  const double df = 6.0 * ((aL + aR) - 2.0 * a);
+  const double d1 = (q[0] + q[2]) - 2.0 * q[1], d2 = (q[1] + q[3]) - 2.0 * q[2], d3 = (q[2] + q[4]) - 2.0 * q[3];
+  const bool same = (df > 0.0 && d1 > 0.0 && d2 > 0.0 && d3 > 0.0) || (df < 0.0 && d1 < 0.0 && d2 < 0.0 && d3 < 0.0);
+  const double m = dmin2(fabs(df), 1.25 * dmin2(fabs(d1), dmin2(fabs(d2), fabs(d3))));
+  const double D = same ? copysign(m, df) : 0.0;
+  const double rho = (df != 0.0) ? div2(D, df) : 0.0;
+  const bool use = rho <= 1.0 - 1e-12;
+  const double eL = use ? a - rho * dm : aL, eR = use ? a + rho * dp : aR;
+  const double mL = (fabs(dm) >= 2.0 * fabs(dp)) ? a - 2.0 * dp : aL;
+  const double mR = (fabs(dp) >= 2.0 * fabs(dm)) ? a + 2.0 * dm : aR;
+  qm = ext ? eL : mL;
+  qp = ext ? eR : mR;
+}
+// q-/q+ of the middle cell of five values: RECON 2 = PPMX, 3 = WENOZ
+template <int RECON>
+__device__ __forceinline__ void recon5(const double q[5], double& qm, double& qp) {
+  if constexpr (RECON == 2) ppmx_lean(q, qm, qp);
+  else wenoz_lean(q, qm, qp);
+}
+
+// q-/q+ of the cell at p[0] from the stencil along stride st: RECON 0 = PLM, 1 = PPM4, 2 = PPMX, 3 = WENOZ
 template <int RECON>
 __device__ __forceinline__ void recon2(const double* p, int st, double& qm, double& qp) {
   if constexpr (RECON == 0) {
     plm_lean(p[-st], p[0], p[st], qm, qp);
+  } else if constexpr (RECON >= 2) {
+    const double q[5] = {p[-2 * st], p[-st], p[0], p[st], p[2 * st]};
+    recon5<RECON>(q, qm, qp);
   } else {
     const double m2 = p[-2 * st], m1 = p[-st], a = p[0], p1 = p[st], p2 = p[2 * st];
     double lo = iface_lean(m2, m1, a, p1);

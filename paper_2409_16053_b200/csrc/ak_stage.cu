@@ -54,10 +54,19 @@ cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, 
   // an odd surplus of ghost layers (ng = 4 with PPM4, ng = 3 with PLM) takes the LDG-staged tiled kernel.
   const int R = (p.recon == 0) ? 2 : 3;
   if (p.variant == 2 || ((p.d.ng - R) & 1)) return launch_stage_tiled(p, Uin, U0, Uout, sc);
+  // PPMX / WENOZ: HLLC only, the two 2-CTA/SM tile shapes
+  if (p.recon >= 2) {
+    const bool stage2 = (Uin != U0);
+    const int tile = pick_tile_v3(p) == 1 ? 1 : 0;
+    if (p.recon == 2) return tile ? launch_v3<2, 0, 16, 8, 2>(p, Uin, U0, Uout, sc, stage2) : launch_v3<2, 0, 16, 10, 2>(p, Uin, U0, Uout, sc, stage2);
+    return tile ? launch_v3<3, 0, 16, 8, 2>(p, Uin, U0, Uout, sc, stage2) : launch_v3<3, 0, 16, 10, 2>(p, Uin, U0, Uout, sc, stage2);
+  }
   return p.recon == 0 ? launch_stage_v3_rs<0>(p, Uin, U0, Uout, sc) : launch_stage_v3_rs<1>(p, Uin, U0, Uout, sc);
 }
 
 cudaError_t launch_flux_correction(const ak_pack& p, const double* Uin, double* Uout, const StageCoef& sc) {
+  if (p.recon == 2) return launch_flux_correction_t<2, 0>(p, Uin, Uout, sc);
+  if (p.recon == 3) return launch_flux_correction_t<3, 0>(p, Uin, Uout, sc);
   switch (p.rsolver) {
     case 1:  return p.recon == 0 ? launch_flux_correction_t<0, 1>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 1>(p, Uin, Uout, sc);
     case 2:  return p.recon == 0 ? launch_flux_correction_t<0, 2>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 2>(p, Uin, Uout, sc);

@@ -190,13 +190,14 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
     }
   }
 
-  double wk[R][5], qlow[5], qp3[5], G[5];
+  constexpr int NW = (RECON >= 2) ? 4 : R;            // x3 window: PPMX / WENOZ need the five planes p-4 .. p
+  double wk[NW][5], qlow[5], qp3[5], G[5];
   // stage 2: max signal speed per direction over this thread's cells, kept as BIT PATTERNS: for x >= 0 they order
   // like the doubles, and every NaN / +inf orders above all finite values, so a corrupted cell is not skipped
   unsigned long long smax[3] = {0ull, 0ull, 0ull};
   int nfl = 0;
 #pragma unroll
-  for (int a = 0; a < R; a++)
+  for (int a = 0; a < NW; a++)
 #pragma unroll
     for (int n = 0; n < 5; n++) wk[a][n] = 1.0;
 #pragma unroll
@@ -262,6 +263,9 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
 #pragma unroll
     for (int n = 0; n < 5; n++) {
       if constexpr (RECON == 0) {
+      } else if constexpr (RECON >= 2) {
+        const double qv[5] = {wk[0][n], wk[1][n], wk[2][n], wk[3][n], wp[n]};
+        recon5<RECON>(qv, qm3[n], qpn[n]);
       } else {
         double hi = iface_lean(wk[0][n], wk[1][n], wk[2][n], wp[n]);
         double lo = qlow[n];
@@ -300,11 +304,11 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
 #pragma unroll
     for (int n = 0; n < 5; n++) { G[n] = Gn[n]; qp3[n] = qpn[n]; }
 #pragma unroll
-    for (int a = 0; a + 1 < R; a++)
+    for (int a = 0; a + 1 < NW; a++)
 #pragma unroll
       for (int n = 0; n < 5; n++) wk[a][n] = wk[a + 1][n];
 #pragma unroll
-    for (int n = 0; n < 5; n++) wk[R - 1][n] = wp[n];
+    for (int n = 0; n < 5; n++) wk[NW - 1][n] = wp[n];
   };
 
   int it = 0;

@@ -221,6 +221,38 @@ def sedov_prim(centre=(0.5, 0.5, 0.5), r0=0.05, p_in=100.0, p_out=1e-2) -> PrimF
     return fn
 
 
+SHU_OSHER_GAMMA = 1.4
+
+
+def shu_osher_prim(direction: int = 0, mach: float = 3.0, gamma: float = SHU_OSHER_GAMMA) -> PrimFn:
+    """Shock - entropy-wave interaction tube of the paper's Fig. 1 right (200 cells, density at t = 0.047).
+    A Mach-3 shock at x = -0.08 on [-0.1, 0.1] runs into gas at rest with density 1 + 0.2 sin(50 pi x), P = 1
+    (Q32: the classic tube on [-1, 1] to t = 0.47 scaled by 1/10, which is what t = 0.047 implies; the
+    Euler equations are invariant under that scaling).  The post-shock state is evaluated from the Rankine-Hugoniot
+    relations for `mach` here, not typed in."""
+    c1 = math.sqrt(gamma * 1.0 / 1.0)
+    r2 = (gamma + 1.0) * mach * mach / ((gamma - 1.0) * mach * mach + 2.0)
+    p2 = 1.0 + 2.0 * gamma / (gamma + 1.0) * (mach * mach - 1.0)
+    u2 = mach * c1 * (1.0 - 1.0 / r2)
+
+    def fn(X1, X2, X3):
+        x = (X1, X2, X3)[direction]
+        left = x < -0.08
+        rho = torch.where(left, torch.full_like(x, r2), 1.0 + 0.2 * torch.sin(50.0 * math.pi * x))
+        vel = [torch.zeros_like(x)] * 3
+        vel[direction] = torch.where(left, torch.full_like(x, u2), torch.zeros_like(x))
+        P = torch.where(left, torch.full_like(x, p2), torch.ones_like(x))
+        return (rho, vel[0], vel[1], vel[2], P)
+    return fn
+
+
+def shu_osher_mesh(N: int, ng: int, nblocks: int = 1) -> Mesh:
+    """N x 4 x 4 cells on [-0.1, 0.1] x [0, 1]^2 in `nblocks` blocks along x1, outflow ends."""
+    m = uniform_mesh((nblocks, 1, 1), (N // nblocks, 4, 4), ng)
+    m.xmin, m.xmax, m.bc = (-0.1, 0.0, 0.0), (0.1, 1.0, 1.0), (1, 1, 0, 0, 0, 0)
+    return m
+
+
 def modes_prim(mach: float, shear: bool, rho_pert: bool) -> PrimFn:
     rm = RandomModes.draw(mach)
 
