@@ -84,7 +84,8 @@ int ak_pack_bind(ak_pack*, void* u_a, void* u_b, void* scratch, void* cuda_strea
  * cells of the leaf block that covers its periodic image: same level -> copy; finer
  * neighbour -> conservative restriction (mean of 8, fixed order); coarser neighbour ->
  * limited-linear (minmod) prolongation of the conserved variables.  Reads active cells only,
- * writes ghost cells only; bit-exact against the oracle.  Asynchronous on the stream. */
+ * writes ghost cells only; bit-exact against the oracle.  Asynchronous on the stream.  Returns without a launch
+ * when the ghost cells are already current (the stage that wrote the state also wrote them: ak_pack_set_ghost_push). */
 int ak_fill_ghosts(ak_pack*);
 
 /* One Runge-Kutta stage.  Default integrator, SSP-RK2 in two registers:
@@ -160,6 +161,13 @@ int ak_pack_set_boundaries(ak_pack*, const int bc[6]);
  * conservative across level boundaries.  Off by default (north_star's stage list omits it); no effect on
  * single-level meshes. */
 int ak_pack_set_flux_correction(ak_pack*, int on);
+
+/* Fused ghost fill (default on).  On a single-level, fully periodic mesh with nx_d >= 2 ng the production kernel stores every cell it
+ * writes within ng of a MeshBlock face also into the ghost cells of the neighbouring blocks (exact copies, the same
+ * values ak_fill_ghosts would copy), so the ak_fill_ghosts that follows finds the ghost cells current and returns
+ * without a launch; a step is then two launches.  on = 0 restores the separate fill pass (results bit-identical).
+ * Refined meshes, non-periodic boundaries and variants 1, 2 always use the separate pass. */
+int ak_pack_set_ghost_push(ak_pack*, int on);
 
 /* Tile shape of the production kernel (variant 0): -1 = chosen from the block size (default);
  * 0 = 16x10 columns, 2 CTAs per SM; 1 = 16x8, 2 CTAs per SM; 2 = 16x22 and 3 = 32x11, 1 CTA per SM.

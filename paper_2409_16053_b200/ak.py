@@ -23,7 +23,7 @@ RSOLVER_HLLC, RSOLVER_LLF, RSOLVER_HLLE, RSOLVER_ROE = 0, 1, 2, 3
 SYMBOLS = [
     "ak_last_error", "ak_pack_create", "ak_pack_set_mesh", "ak_pack_set_block", "ak_pack_state_bytes",
     "ak_pack_scratch_bytes", "ak_pack_bind", "ak_fill_ghosts", "ak_hydro_stage", "ak_new_dt", "ak_step",
-    "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_download_async", "ak_pack_floor_count", "ak_pack_set_variant", "ak_pack_set_tile", "ak_pack_set_flux_correction", "ak_pack_set_boundaries", "ak_pack_set_integrator",
+    "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_download_async", "ak_pack_floor_count", "ak_pack_set_variant", "ak_pack_set_tile", "ak_pack_set_flux_correction", "ak_pack_set_ghost_push", "ak_pack_set_boundaries", "ak_pack_set_integrator",
     "ak_pack_launch_count", "ak_pack_destroy",
 ]
 
@@ -59,6 +59,7 @@ def lib():
         "ak_pack_download_async": (i, [vp, vp]),
         "ak_pack_floor_count": (ll, [vp]),
         "ak_pack_set_variant": (i, [vp, i]),
+        "ak_pack_set_ghost_push": (i, [vp, i]),
         "ak_pack_set_tile": (i, [vp, i]),
         "ak_pack_set_flux_correction": (i, [vp, i]),
         "ak_pack_set_boundaries": (i, [vp, C.POINTER(C.c_int)]),
@@ -176,6 +177,9 @@ class Pack:
 
     def set_flux_correction(self, on=True):
         _chk(lib().ak_pack_set_flux_correction(self._h, 1 if on else 0))
+
+    def set_ghost_push(self, on=True):
+        _chk(lib().ak_pack_set_ghost_push(self._h, 1 if on else 0))
 
     def set_tile(self, t):
         _chk(lib().ak_pack_set_tile(self._h, t))

@@ -251,6 +251,12 @@ extern "C" int ak_pack_set_flux_correction(ak_pack* p, int on) {
   return AK_OK;
 }
 
+extern "C" int ak_pack_set_ghost_push(ak_pack* p, int on) {
+  if (!p) return fail(AK_EINVAL, "null pack");
+  p->ghost_push = on != 0;
+  return AK_OK;
+}
+
 extern "C" int ak_pack_set_tile(ak_pack* p, int tile) {
   if (!p) return fail(AK_EINVAL, "null pack");
   if (tile < -1 || tile > 3) return fail(AK_EINVAL, "unknown tile shape");
@@ -260,6 +266,7 @@ extern "C" int ak_pack_set_tile(ak_pack* p, int tile) {
 
 extern "C" int ak_fill_ghosts(ak_pack* p) {
   if (!p || !p->bound) return fail(AK_ESTATE, "pack not bound");
+  if (p->ghosts_ok) return AK_OK;       // already current: the stage that wrote the state also wrote its ghost copies
   DeviceGuard guard(p->device);
   AK_CUDA(ak::launch_fill_ghosts(*p, p->u[p->cur]), "ak_fill_ghosts launch");
   p->launches += 1;
@@ -303,6 +310,12 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
   if (p->integrator != 2 && !v3) return fail(AK_EUNSUPPORTED, "forward Euler and SSPRK(3,3) exist in the production kernel only");
   const bool last = stage == p->integrator;
   sc.take_dt = (last && stage >= 2) ? 1 : 0;
+  // uniform, fully periodic meshes: the production kernel stores every boundary cell into the neighbours' ghost
+  // cells as it writes it, so the next ak_fill_ghosts has nothing left to do
+  bool periodic = true;
+  for (int f = 0; f < 6; f++) periodic = periodic && p->bc[f] == 0;
+  for (int d = 0; d < 3; d++) periodic = periodic && p->d.nx[d] >= 2 * p->d.ng;    // (a cell is near one face per direction)
+  sc.push = (v3 && p->ghost_push && p->d.max_level == 0 && periodic) ? 1 : 0;
   p->dt_cached = false;
   if (sc.take_dt && v3) AK_CUDA(cudaMemsetAsync(p->d.smax_bits, 0, 48, p->stream), "reset signal speeds");
   AK_CUDA(ak::launch_stage(*p, p->u[p->cur], u0, p->u[out], sc), "ak_hydro_stage launch");
@@ -314,7 +327,7 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
     p->dt_cached = false;               // the correction changed cells after their signal speeds were taken
   }
   p->cur = out;
-  p->ghosts_ok = false;
+  p->ghosts_ok = sc.push != 0;
   return AK_OK;
 }
 

@@ -38,6 +38,7 @@ struct StageCoef {
   double g0, g1;            // weights of U_in and U0
   double c[2][3];           // beta*dt/dx_d for level 0 and 1
   int take_dt;              // last stage of a step: also reduce the signal speeds of the result
+  int push;                 // uniform periodic meshes: the writer of a cell also stores it into the neighbours' ghost cells
 };
 
 }  // namespace ak
@@ -58,6 +59,7 @@ struct ak_pack {
   int variant = 0;
   int bc[6] = {0, 0, 0, 0, 0, 0};  // ak_pack_set_boundaries: x1min,x1max,x2min,x2max,x3min,x3max
   bool flux_correction = false;   // ak_pack_set_flux_correction
+  bool ghost_push = true;         // ak_pack_set_ghost_push: fuse the same-level periodic ghost fill into the stage kernel
   int tile = -1;                  // -1 = automatic (ak_pack_set_tile)
   long long launches = 0;
   int sm_count = 148;

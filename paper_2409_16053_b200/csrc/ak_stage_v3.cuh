@@ -46,6 +46,32 @@ struct V3Tile {
   static constexpr int NE = (TI + TJ + 31) / 32;                      // tile-edge faces per lane of the edge warp
 };
 
+// Ghost fill fused into the stage (uniform periodic meshes with nx_d >= 2 ng): the thread that writes
+// active cell (gi, gj, f) of block m also stores it into the ghost cells that are its periodic image in the
+// neighbouring blocks -- the block in direction E holds it at the index shifted by -E * nx.  (e1, e2, e3) say which
+// face the cell is within ng of in each direction (0: none); its images are the up to 7 non-empty sub-selections.
+// Exact copies of what ak_fill_ghosts would copy in a separate pass over the state; only threads near a block face
+// come here (loops not unrolled: the hot loop keeps its size).
+__device__ __forceinline__ void push_ghosts(const PackDev& P, double* __restrict__ Uout, int m, int gi, int gj, int f,
+                                         int e1, int e2, int e3, double u0, double u1, double u2, double u3, double u4) {
+  const int ng = P.ng;
+  const long long nc = P.ncell;
+  const int* nb = P.nbr + 27 * m;
+#pragma unroll 1
+  for (int a3 = 0; a3 <= (e3 != 0); a3++)
+#pragma unroll 1
+    for (int a2 = 0; a2 <= (e2 != 0); a2++)
+#pragma unroll 1
+      for (int a1 = 0; a1 <= (e1 != 0); a1++) {
+        if (!(a1 | a2 | a3)) continue;
+        const int E1 = a1 ? e1 : 0, E2 = a2 ? e2 : 0, E3 = a3 ? e3 : 0;
+        const int dst = nb[(E3 + 1) * 9 + (E2 + 1) * 3 + (E1 + 1)];
+        double* o = Uout + (long long)dst * 5 * nc +
+                    ((long long)(f + ng - E3 * P.nx[2]) * P.nt[1] + (gj + ng - E2 * P.nx[1])) * P.nt[0] + (gi + ng - E1 * P.nx[0]);
+        o[0] = u0; o[nc] = u1; o[2 * nc] = u2; o[3 * nc] = u3; o[4 * nc] = u4;
+      }
+}
+
 __device__ __forceinline__ void cta_sync(int nthreads) {
   asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }
@@ -168,6 +194,9 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
   const long long col = (long long)m * 5 * nc + (long long)(j0 + tj + ng) * P.nt[0] + (i0 + ti + ng);
   const int lev = P.blk[m].x;
   const double c1 = sc.c[lev][0], c2 = sc.c[lev][1], c3 = sc.c[lev][2];
+  // fused ghost fill: is this column within ng of an x1 / x2 face of its block?
+  const int pe1 = !sc.push ? 0 : (i0 + ti < ng ? -1 : (i0 + ti >= P.nx[0] - ng ? 1 : 0));
+  const int pe2 = !sc.push ? 0 : (j0 + tj < ng ? -1 : (j0 + tj >= P.nx[1] - ng ? 1 : 0));
 
   const int oW = (tj + R) * WI + ti + R;                // own cell inside a staged plane (variable stride WJ*WI)
   const int oQ1 = tj * (TI + 1) + ti;                   // lower x1 face of the own cell   (variable stride TJ*(TI+1))
@@ -284,6 +313,8 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
       double un[5];
 #pragma unroll
       for (int n = 0; n < 5; n++) { un[n] = fma(-c3, Gn[n] - G[n], Tc[n * NT]); o[n * nc] = un[n]; }
+      const int pe3 = !sc.push ? 0 : (c - 1 < ng ? -1 : (c - 1 >= P.nx[2] - ng ? 1 : 0));
+      if (pe1 | pe2 | pe3) push_ghosts(P, Uout, m, i0 + ti, j0 + tj, c - 1, pe1, pe2, pe3, un[0], un[1], un[2], un[3], un[4]);
       if (STAGE2 && sc.take_dt) {                  // (uniform over the grid)
         // S0 of the NEXT step (Eq.(3)) on U^{n+1} while it is in registers: the cell's signal speeds
         // |v_d| + c_s in the oracle's arithmetic (IEEE division and sqrt, no contraction: this translation unit

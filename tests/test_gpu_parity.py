@@ -222,6 +222,7 @@ def test_dt_reduction_bit_exact(orc, ak):
 def test_call_order_and_argument_errors(ak):
     w = I.config0()
     pg = ak.Pack(w.mesh, w.gamma, w.recon)
+    pg.set_ghost_push(False)                         # (with the fused fill a stage leaves the ghost cells current)
     pg.load(w.state())
     with pytest.raises(ak.AkError):
         pg.hydro_stage(1, 1e-3)                      # ghosts not filled
@@ -414,8 +415,9 @@ def test_flux_correction_off_drifts_and_on_is_inert_on_uniform_mesh(ak):
         l0 = pu.launch_count()
         for _ in range(2):
             pu.step(wu.cfl)
-        # step 1: dt_init + new_dt + 2 x (fill + stage); step 2: the dt comes from stage 2 of step 1; no correction launches
-        assert pu.launch_count() - l0 == 6 + 4
+        # step 1: dt_init + new_dt + fill + 2 stages (stage 1 writes the ghost copies itself, so the second fill has
+        # nothing to do); step 2: the dt comes from stage 2 of step 1 and both fills are already done; no correction launches
+        assert pu.launch_count() - l0 == 5 + 2
         res.append(P.gpu_state(pu))
     assert np.array_equal(res[0], res[1])
 
@@ -464,6 +466,43 @@ def test_llf_hlle_only_in_the_production_kernel(ak):
     pg.fill_ghosts()
     with pytest.raises(ak.AkError):
         pg.hydro_stage(1, 1e-3)
+
+
+# ------------------------------------------------------------ ghost fill fused into the stage --------
+@pytest.mark.parametrize("nrb,nx,ng,recon", [
+    ((2, 2, 2), (16, 16, 16), 2, 0), ((2, 2, 2), (16, 16, 16), 3, 1), ((1, 1, 1), (8, 8, 8), 2, 0), ((1, 1, 1), (4, 4, 4), 3, 1),
+    ((3, 1, 2), (2, 2, 2), 2, 0), ((2, 3, 1), (4, 2, 6), 2, 0), ((2, 1, 3), (24, 40, 6), 3, 1), ((1, 2, 1), (34, 10, 6), 2, 0),
+])
+def test_fused_ghost_push_equals_the_separate_fill(orc, ak, nrb, nx, ng, recon):
+    """Uniform periodic meshes: the stage kernel writes every boundary cell also into the neighbours' ghost cells.
+    After each stage -- WITHOUT calling the fill kernel -- every ghost cell must equal the oracle's fill of the GPU's
+    own active cells bit for bit (blocks smaller than 2 ng, where a cell is near both faces, a single self-periodic
+    block and ragged tiles included), no fill is launched after the first one, and the results are bit-identical to a
+    run with the push switched off."""
+    w = I.config3(nrb=1, nx=16) if recon else I.config1(nrb=1, nx=16)
+    w.mesh = I.uniform_mesh(nrb, nx, ng)
+    U0 = w.state()
+    pg = ak.Pack(w.mesh, w.gamma, recon)
+    pr = ak.Pack(w.mesh, w.gamma, recon)
+    pr.set_ghost_push(False)
+    pg.load(U0); pr.load(U0)
+    for step in range(3):
+        dt = pr.new_dt(w.cfl)
+        assert pg.new_dt(w.cfl) == dt
+        for stage in (1, 2):
+            l0 = pg.launch_count()
+            pg.fill_ghosts(); pr.fill_ghosts()
+            pushing = all(n >= 2 * ng for n in nx)       # (smaller blocks keep the separate fill pass)
+            assert pg.launch_count() - l0 == (1 if (step == 0 and stage == 1) or not pushing else 0)
+            pg.hydro_stage(stage, dt); pr.hydro_stage(stage, dt)
+            if pushing:
+                ug = P.gpu_state(pg)                         # ghosts as the stage left them
+                chk = orc.OrcPack(w.mesh, w.gamma, recon)
+                chk.load(ug); chk.fill_ghosts()
+                assert np.array_equal(chk.current(), ug), (step, stage)
+                chk.close()
+    pr.fill_ghosts(); pg.fill_ghosts()
+    assert np.array_equal(P.gpu_state(pg), P.gpu_state(pr))
 
 
 # ------------------------------------------------------------ strong collisions / non-finite states (VERDICT r1 1b, ADVICE r1) ----
