@@ -296,6 +296,8 @@ struct orc_pack {
   int nthreads = 1;
   int bc[6] = { 0, 0, 0, 0, 0, 0 };      // per face x1min,x1max,...: 0 periodic, 1 outflow, 2 reflect
   bool flux_correction = false;          // SURVEY 8(f) f1, off by default (north_star's stage list omits it)
+  bool fofc = false;                     // SURVEY 8(f) f2 / P:118: first-order flux correction, off by default
+  long long fofc_count = 0;              // cells flagged since bind
 
   size_t ncell() const { return (size_t)nt[0] * nt[1] * nt[2]; }
   size_t idx(int m, int n, int k, int j, int i) const {
@@ -369,7 +371,7 @@ extern "C" int orc_pack_bind(orc_pack* p, double* u_a, double* u_b) {
   if (vol != (double)p->nrb[0] * p->nrb[1] * p->nrb[2]) return fail("leaves do not cover the domain");
   if (p->max_level > 0 && (p->ng & 1)) return fail("static refinement needs even ng");
   for (int f = 0; f < 6; f++) if (p->bc[f] != 0 && p->max_level > 0) return fail("physical boundaries need a single-level mesh");
-  p->u[0] = u_a; p->u[1] = u_b; p->cur = 0; p->bound = true; p->floor_count = 0;
+  p->u[0] = u_a; p->u[1] = u_b; p->cur = 0; p->bound = true; p->floor_count = 0; p->fofc_count = 0;
   return 0;
 }
 
@@ -392,6 +394,8 @@ extern "C" int orc_set_integrator(orc_pack* p, int nstages, double* u_c) {
   return 0;
 }
 extern "C" int orc_set_flux_correction(orc_pack* p, int on) { if (!p) return fail("null pack"); p->flux_correction = on != 0; return 0; }
+extern "C" int orc_set_fofc(orc_pack* p, int on) { if (!p) return fail("null pack"); p->fofc = on != 0; return 0; }
+extern "C" long long orc_pack_fofc_count(const orc_pack* p) { return p ? p->fofc_count : -1; }
 extern "C" double* orc_pack_current(orc_pack* p) { return (p && p->bound) ? p->u[p->cur] : nullptr; }
 extern "C" long long orc_pack_floor_count(const orc_pack* p) { return p ? p->floor_count : -1; }
 extern "C" int orc_pack_destroy(orc_pack* p) { delete p; return 0; }
@@ -621,6 +625,49 @@ static void correct_coarse_fluxes(const orc_pack* p, std::vector<FaceFlux>& F) {
   }
 }
 
+// f2 / P:118 first-order flux correction (FOFC): "if the density or pressure in any cell were to go negative, the fluxes
+// on all faces of that cell are recalculated using first-order (piecewise constant) reconstruction and a diffusive
+// LLF Riemann solver".  Reading (Q31): a cell is flagged when the stage's tentative result has rho <= 0 or
+// E - |m|^2/(2 rho) <= 0 (NaN included); the flags are copied into the ghost cells like the state (same-level copies
+// and boundary images), so both blocks that share a face see the same pair of flags; every face with a flagged cell
+// on either side takes F = LLF(W_lower, W_upper) of the two CELL-CENTRED primitive states of U_in; then the update is
+// evaluated again.  Single-level meshes (the ordering against f1 that P:118 prescribes is then moot).
+static long long fofc_replace_fluxes(const orc_pack* p, const double* Uin, const double* Utent, std::vector<FaceFlux>& F) {
+  const int ng = p->ng, n1 = p->nt[0], n2 = p->nt[1], n3 = p->nt[2];
+  const size_t nc = p->ncell();
+  // flags live in variable 0 of a state-shaped scratch array so that the ghost fill of the state can be reused as it is
+  std::vector<double> flag((size_t)p->nmb * 5 * nc, 0.0);
+  long long nflag = 0;
+  for (int m = 0; m < p->nmb; m++)
+    for (int k = ng; k < p->nx[2] + ng; k++) for (int j = ng; j < p->nx[1] + ng; j++) for (int i = ng; i < p->nx[0] + ng; i++) {
+      const double rho = Utent[p->idx(m, 0, k, j, i)];
+      const double m1 = Utent[p->idx(m, 1, k, j, i)], m2 = Utent[p->idx(m, 2, k, j, i)], m3 = Utent[p->idx(m, 3, k, j, i)];
+      const double eint = Utent[p->idx(m, 4, k, j, i)] - 0.5 * (m1 * m1 + (m2 * m2 + m3 * m3)) / rho;
+      if (!(rho > 0.0) || !(eint > 0.0)) { flag[p->idx(m, 0, k, j, i)] = 1.0; nflag++; }
+    }
+  if (nflag == 0) return 0;
+  for (int m = 0; m < p->nmb; m++) fill_block(p, flag.data(), m);
+  const int str[3] = { 1, n1, n1 * n2 };
+  for (int m = 0; m < p->nmb; m++)
+    for (int d = 0; d < 3; d++) {
+      int hi[3] = { p->nx[0] + ng, p->nx[1] + ng, p->nx[2] + ng };
+      hi[d] += 1;
+      for (int k = ng; k < hi[2]; k++) for (int j = ng; j < hi[1]; j++) for (int i = ng; i < hi[0]; i++) {
+        const size_t c = ((size_t)k * n2 + j) * n1 + i, cm = c - str[d];
+        const size_t base = (size_t)m * 5 * nc;
+        if (flag[base + c] == 0.0 && flag[base + cm] == 0.0) continue;
+        double uL[5], uR[5], WL[5], WR[5], Fl[5];
+        for (int n = 0; n < 5; n++) { uL[n] = Uin[base + n * nc + cm]; uR[n] = Uin[base + n * nc + c]; }
+        orc_c2p(p->gamma, uL, WL, nullptr);
+        orc_c2p(p->gamma, uR, WR, nullptr);
+        orc_llf(p->gamma, d, WL, WR, Fl);
+        for (int n = 0; n < 5; n++) F[m][d][n * nc + c] = Fl[n];
+      }
+    }
+  (void)n3;
+  return nflag;
+}
+
 extern "C" int orc_hydro_stage(orc_pack* p, int stage, double dt) {
   if (!p || !p->bound) return fail("pack not bound");
   if (stage < 1 || stage > p->integrator) return fail("stage out of range for the integrator");
@@ -643,7 +690,19 @@ extern "C" int orc_hydro_stage(orc_pack* p, int stage, double dt) {
   const int out = (p->integrator == 1) ? 1 - p->cur : ((stage == p->integrator) ? 0 : stage);
   double* Uout = p->u[out];
   long long nfl = 0;
-  if (p->flux_correction && p->max_level > 0) {
+  if (p->fofc) {
+    if (p->max_level > 0) return fail("FOFC is implemented on single-level meshes");
+    // high-order fluxes of all blocks, the tentative update into a scratch copy, flags, replaced fluxes, final update
+    std::vector<FaceFlux> F(p->nmb);
+#pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) reduction(+ : nfl) if (p->nthreads > 1)
+    for (int m = 0; m < p->nmb; m++) nfl += block_fluxes(p, Uin, m, F[m]);
+    std::vector<double> tent((size_t)p->nmb * 5 * p->ncell(), 0.0);
+#pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) if (p->nthreads > 1)
+    for (int m = 0; m < p->nmb; m++) block_update(p, Uin, U0, tent.data(), m, F[m], g0, g1, beta, dt);
+    p->fofc_count += fofc_replace_fluxes(p, Uin, tent.data(), F);
+#pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) if (p->nthreads > 1)
+    for (int m = 0; m < p->nmb; m++) block_update(p, Uin, U0, Uout, m, F[m], g0, g1, beta, dt);
+  } else if (p->flux_correction && p->max_level > 0) {
     // all fluxes first, then the coarse faces at level boundaries are replaced, then every block is advanced
     std::vector<FaceFlux> F(p->nmb);
 #pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) reduction(+ : nfl) if (p->nthreads > 1)

@@ -46,6 +46,10 @@ int orc_pack_bind(orc_pack*, double* u_a, double* u_b);
 int orc_set_threads(orc_pack*, int nthreads);
 /* f1: replace the coarse flux at level-boundary faces by the mean of the four fine fluxes.  Off by default. */
 int orc_set_flux_correction(orc_pack*, int on);
+/* f2: first-order flux correction -- faces of cells whose tentative update has rho <= 0 or e_int <= 0 take the
+ * LLF flux of the cell-centred states; single-level meshes; off by default.  orc_pack_fofc_count: cells flagged since bind. */
+int orc_set_fofc(orc_pack*, int on);
+long long orc_pack_fofc_count(const orc_pack*);
 int orc_fill_ghosts(orc_pack*);                           /* G1-G4 on the current buffer           */
 int orc_hydro_stage(orc_pack*, int stage, double dt);     /* S1-S4; stage 1: A->B, stage 2: B,A->A (RK3: B,A->C; C,A->A) */
 /* f2: number of stages, 2 = SSPRK(2,2) (default) or 3 = SSPRK(3,3), which needs a third caller-owned buffer u_c. */

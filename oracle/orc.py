@@ -41,6 +41,9 @@ def lib():
     L.orc_pack_set_boundaries.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
     L.orc_set_threads.argtypes = [C.c_void_p, C.c_int]
     L.orc_set_flux_correction.argtypes = [C.c_void_p, C.c_int]
+    L.orc_set_fofc.argtypes = [C.c_void_p, C.c_int]
+    L.orc_pack_fofc_count.restype = C.c_longlong
+    L.orc_pack_fofc_count.argtypes = [C.c_void_p]
     L.orc_set_integrator.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
     L.orc_fill_ghosts.argtypes = [C.c_void_p]
     L.orc_hydro_stage.argtypes = [C.c_void_p, C.c_int, C.c_double]
@@ -176,6 +179,13 @@ class OrcPack:
     def set_flux_correction(self, on=True):
         """f1 of SURVEY 8(f): coarse fluxes at level-boundary faces <- mean of the four fine fluxes (off by default)."""
         _chk(lib().orc_set_flux_correction(self._h, 1 if on else 0))
+
+    def set_fofc(self, on=True):
+        """f2 of SURVEY 8(f): first-order flux correction (off by default)."""
+        _chk(lib().orc_set_fofc(self._h, 1 if on else 0))
+
+    def fofc_count(self):
+        return lib().orc_pack_fofc_count(self._h)
 
     def load(self, U):
         """Copy U^n (numpy or CPU torch tensor of the state shape) into buffer A and make it current."""
