@@ -162,6 +162,19 @@ int ak_pack_set_boundaries(ak_pack*, const int bc[6]);
  * single-level meshes. */
 int ak_pack_set_flux_correction(ak_pack*, int on);
 
+/* First-order flux correction, FOFC (paper P:118; off by default): after the stage kernel, every cell whose
+ * tentative result has rho <= 0 or E - |rho v|^2 / (2 rho) <= 0 (NaN included) is flagged, and every face with a flagged
+ * cell on either side trades its high-order flux for the LLF flux of the two cell-centred states of the stage's input
+ * and the cells on both sides are updated again from the stage's inputs (three extra launches per stage, which return at
+ * once when nothing was flagged).  Because that second update needs U^n, the last stage of a step cannot run in place:
+ * u_spare is a fourth caller-owned device buffer of ak_pack_state_bytes() (256-byte aligned, disjoint from the others)
+ * which the last stage writes and which then TRADES PLACES with buffer A (ak_pack_current() returns it).  Call on a bound
+ * pack between steps; ak_pack_bind with buffers that overlap the spare switches FOFC off again.  Single-level meshes,
+ * production kernel (ak_hydro_stage returns AK_EUNSUPPORTED otherwise).  on = 0: off (u_spare ignored).
+ * ak_pack_fofc_count: cells flagged since bind (synchronises). */
+int ak_pack_set_fofc(ak_pack*, int on, void* u_spare);
+long long ak_pack_fofc_count(ak_pack*);
+
 /* Fused ghost fill (default on).  On a single-level, fully periodic mesh with nx_d >= 2 ng the production kernel stores every cell it
  * writes within ng of a MeshBlock face also into the ghost cells of the neighbouring blocks (exact copies, the same
  * values ak_fill_ghosts would copy), so the ak_fill_ghosts that follows finds the ghost cells current and returns

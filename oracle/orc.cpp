@@ -169,7 +169,12 @@ extern "C" void orc_hllc(double gamma, int dir, const double WL[5], const double
   double rR = WR[0], uR = WR[iu], vR = WR[iv], wR = WR[iw], eR = WR[4];
   double pL = gm1 * eL, pR = gm1 * eR;
   double cL = std::sqrt(gamma * pL / rL), cR = std::sqrt(gamma * pR / rR);
-  double SL = std::fmin(uL - cL, uR - cR), SR = std::fmax(uL + cL, uR + cR);
+  // min / max written as comparisons in this operand order so that a NaN sound speed (an unphysical reconstructed state:
+  // negative pressure or density at the face) is NOT dropped the way fmin / fmax would drop it: a NaN c_L makes S_L NaN, a
+  // NaN c_R makes S_R NaN, either makes S* and with it the whole flux NaN, and the cell is then caught by FOFC (Q31) or
+  // reported by the time-step reduction.  For finite operands these are min and max.
+  const double sl1 = uL - cL, sl2 = uR - cR, sr1 = uL + cL, sr2 = uR + cR;
+  double SL = (sl2 < sl1) ? sl2 : sl1, SR = (sr1 > sr2) ? sr1 : sr2;
   double bm = std::fmin(SL, 0.0), bp = std::fmax(SR, 0.0);
   double mL = rL * (uL - SL), mR = rR * (SR - uR);
   double Ss = ((pL - pR) + (mL * uL + mR * uR)) / (mL + mR);                  // contact speed

@@ -23,7 +23,7 @@ RSOLVER_HLLC, RSOLVER_LLF, RSOLVER_HLLE, RSOLVER_ROE = 0, 1, 2, 3
 SYMBOLS = [
     "ak_last_error", "ak_pack_create", "ak_pack_set_mesh", "ak_pack_set_block", "ak_pack_state_bytes",
     "ak_pack_scratch_bytes", "ak_pack_bind", "ak_fill_ghosts", "ak_hydro_stage", "ak_new_dt", "ak_step",
-    "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_download_async", "ak_pack_floor_count", "ak_pack_set_variant", "ak_pack_set_tile", "ak_pack_set_flux_correction", "ak_pack_set_ghost_push", "ak_pack_set_boundaries", "ak_pack_set_integrator",
+    "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_download_async", "ak_pack_floor_count", "ak_pack_set_variant", "ak_pack_set_tile", "ak_pack_set_flux_correction", "ak_pack_set_ghost_push", "ak_pack_set_fofc", "ak_pack_fofc_count", "ak_pack_set_boundaries", "ak_pack_set_integrator",
     "ak_pack_launch_count", "ak_pack_destroy",
 ]
 
@@ -60,6 +60,8 @@ def lib():
         "ak_pack_floor_count": (ll, [vp]),
         "ak_pack_set_variant": (i, [vp, i]),
         "ak_pack_set_ghost_push": (i, [vp, i]),
+        "ak_pack_set_fofc": (i, [vp, i, vp]),
+        "ak_pack_fofc_count": (C.c_longlong, [vp]),
         "ak_pack_set_tile": (i, [vp, i]),
         "ak_pack_set_flux_correction": (i, [vp, i]),
         "ak_pack_set_boundaries": (i, [vp, C.POINTER(C.c_int)]),
@@ -119,11 +121,15 @@ class Pack:
         self.stream.synchronize()
         _chk(lib().ak_pack_bind(self._h, self.ua.data_ptr(), self.ub.data_ptr(), self.scratch.data_ptr(),
                                 self.stream.cuda_stream))
+        if getattr(self, "_fofc", False):
+            self.set_fofc(True)                  # (the spare and buffer A trade places every step: re-arm after the re-bind)
 
     def current(self) -> torch.Tensor:
         p = lib().ak_pack_current(self._h)
         if getattr(self, "uc", None) is not None and p == self.uc.data_ptr():
             return self.uc
+        if getattr(self, "uf", None) is not None and p == self.uf.data_ptr():
+            return self.uf
         return self.ua if p == self.ua.data_ptr() else self.ub
 
     def set_integrator(self, nstages):
@@ -177,6 +183,20 @@ class Pack:
 
     def set_flux_correction(self, on=True):
         _chk(lib().ak_pack_set_flux_correction(self._h, 1 if on else 0))
+
+    def set_fofc(self, on=True):
+        """P:118 first-order flux correction: allocates the spare buffer the last stage of a step then writes."""
+        if on and getattr(self, "uf", None) is None:
+            with torch.cuda.device(self.device):
+                self.uf = torch.zeros(self.mesh.state_shape(), dtype=torch.float64, device=self.device)
+        self._fofc = bool(on)
+        _chk(lib().ak_pack_set_fofc(self._h, 1 if on else 0, self.uf.data_ptr() if on else None))
+
+    def fofc_count(self):
+        n = lib().ak_pack_fofc_count(self._h)
+        if n < 0:
+            raise AkError(lib().ak_last_error().decode())
+        return n
 
     def set_ghost_push(self, on=True):
         _chk(lib().ak_pack_set_ghost_push(self._h, 1 if on else 0))

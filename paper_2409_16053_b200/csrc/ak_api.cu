@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <utility>
 
 static thread_local std::string g_err;
 static int fail(int code, const std::string& msg) { g_err = msg; return code; }
@@ -28,7 +29,7 @@ struct DeviceGuard {
 static size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
 
 // scratch layout: [0,256) reduction cells | block table int4[nmb] | leaf0 | leaf1 | same-level neighbours int[nmb][27]
-struct ScratchLayout { size_t blk, leaf0, leaf1, nbr, nbc, total; };
+struct ScratchLayout { size_t blk, leaf0, leaf1, nbr, nbc, flags, total; };
 static ScratchLayout scratch_layout(const ak_pack* p) {
   ScratchLayout s;
   const ak::PackDev& d = p->d;
@@ -38,7 +39,8 @@ static ScratchLayout scratch_layout(const ak_pack* p) {
   s.leaf1 = s.leaf0 + align256(sizeof(int) * n0);
   s.nbr = s.leaf1 + align256(sizeof(int) * 8 * n0);
   s.nbc = s.nbr + align256(sizeof(int) * 27 * (size_t)d.nmb);
-  s.total = s.nbc + align256(sizeof(int) * 27 * (size_t)d.nmb);
+  s.flags = s.nbc + align256(sizeof(int) * 27 * (size_t)d.nmb);      // FOFC: one byte per cell
+  s.total = s.flags + align256((size_t)d.nmb * (size_t)d.ncell);
   return s;
 }
 
@@ -186,6 +188,8 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
   d.dtmin_bits = (unsigned long long*)s;
   d.floor_cnt = (unsigned long long*)(s + 8);
   d.nonfinite = (unsigned long long*)(s + 16);
+  p->fofc_cnt = (unsigned long long*)(s + 24);           // [0] this stage, [1] since bind
+  p->fofc_flags = (unsigned char*)(s + sl.flags);
   d.smax_bits = (unsigned long long*)(s + 64);
   d.blk = (const int4*)(s + sl.blk);
   d.leaf0 = (const int*)(s + sl.leaf0);
@@ -197,6 +201,10 @@ extern "C" int ak_pack_bind(ak_pack* p, void* u_a, void* u_b, void* scratch, voi
   // a third register bound earlier (SSPRK(3,3)) stays valid only if it is still disjoint from the new buffers
   if (p->u[2] && (overlap(p->u[2], sb, u_a, sb) || overlap(p->u[2], sb, u_b, sb) || overlap(p->u[2], sb, scratch, sl.total))) {
     p->u[2] = nullptr; p->integrator = 2;
+  }
+  // likewise the FOFC spare (after a step it has traded places with A: re-arm FOFC after re-binding the old buffers)
+  if (p->u_spare && (overlap(p->u_spare, sb, u_a, sb) || overlap(p->u_spare, sb, u_b, sb) || overlap(p->u_spare, sb, scratch, sl.total))) {
+    p->u_spare = nullptr; p->fofc = false;
   }
   p->cur = 0; p->ghosts_ok = false; p->bound = true; p->launches = 0; p->dt_cached = false;
   p->tmap_box[0] = p->tmap_box[1] = 0;
@@ -249,6 +257,33 @@ extern "C" int ak_pack_set_flux_correction(ak_pack* p, int on) {
   if (!p) return fail(AK_EINVAL, "null pack");
   p->flux_correction = on != 0;
   return AK_OK;
+}
+
+extern "C" int ak_pack_set_fofc(ak_pack* p, int on, void* u_spare) {
+  if (!p) return fail(AK_EINVAL, "null pack");
+  if (!on) { p->fofc = false; p->u_spare = nullptr; return AK_OK; }
+  if (!p->bound) return fail(AK_ESTATE, "bind the pack first");
+  if (!u_spare) return fail(AK_EINVAL, "FOFC needs a spare state buffer (the last stage of a step cannot run in place)");
+  if ((uintptr_t)u_spare & 255) return fail(AK_EINVAL, "buffers must be 256-byte aligned");
+  if (p->cur != 0 && !(p->integrator == 1)) return fail(AK_ESTATE, "switch FOFC on between steps");
+  const size_t sb = ak_pack_state_bytes(p), ss = scratch_layout(p).total;
+  auto overlap = [](const void* a, size_t na, const void* b, size_t nb) {
+    return (uintptr_t)a < (uintptr_t)b + nb && (uintptr_t)b < (uintptr_t)a + na;
+  };
+  for (int b = 0; b < 3; b++) if (p->u[b] && overlap(u_spare, sb, p->u[b], sb)) return fail(AK_EINVAL, "device buffers overlap");
+  if (overlap(u_spare, sb, p->scratch, ss)) return fail(AK_EINVAL, "device buffers overlap");
+  p->fofc = true;
+  p->u_spare = (double*)u_spare;
+  return AK_OK;
+}
+
+extern "C" long long ak_pack_fofc_count(ak_pack* p) {
+  if (!p || !p->bound) { fail(AK_ESTATE, "pack not bound"); return -1; }
+  DeviceGuard guard(p->device);
+  unsigned long long n = 0;
+  if (cudaMemcpyAsync(&n, p->fofc_cnt + 1, 8, cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
+      cudaStreamSynchronize(p->stream) != cudaSuccess) { fail(AK_ECUDA, "ak_pack_fofc_count copy failed"); return -1; }
+  return (long long)n;
 }
 
 extern "C" int ak_pack_set_ghost_push(ak_pack* p, int on) {
@@ -305,22 +340,39 @@ extern "C" int ak_hydro_stage(ak_pack* p, int stage, double dt) {
       double dx = (p->xmax[d] - p->xmin[d]) / ((double)p->d.nrb[d] * p->d.nx[d] * (double)(1 << lev));
       sc.c[lev][d] = beta * dt / dx;
     }
+  if (p->fofc && (p->d.max_level > 0 || p->variant != 0 || ((p->d.ng - (p->recon == 0 ? 2 : 3)) & 1)))
+    return fail(AK_EUNSUPPORTED, "FOFC is implemented for the production kernel on single-level meshes");
   // stage 2 of the production kernel also leaves the max signal speeds of U^{n+1} for the next ak_new_dt
   const bool v3 = p->variant == 0 && !((p->d.ng - (p->recon == 0 ? 2 : 3)) & 1);
   if (p->integrator != 2 && !v3) return fail(AK_EUNSUPPORTED, "forward Euler and SSPRK(3,3) exist in the production kernel only");
   const bool last = stage == p->integrator;
-  sc.take_dt = (last && stage >= 2) ? 1 : 0;
+  sc.take_dt = (last && stage >= 2 && !p->fofc) ? 1 : 0;      // (FOFC may change cells after the stage)
   // uniform, fully periodic meshes: the production kernel stores every boundary cell into the neighbours' ghost
   // cells as it writes it, so the next ak_fill_ghosts has nothing left to do
   bool periodic = true;
   for (int f = 0; f < 6; f++) periodic = periodic && p->bc[f] == 0;
   for (int d = 0; d < 3; d++) periodic = periodic && p->d.nx[d] >= 2 * p->d.ng;    // (a cell is near one face per direction)
-  sc.push = (v3 && p->ghost_push && p->d.max_level == 0 && periodic) ? 1 : 0;
+  sc.push = (v3 && p->ghost_push && p->d.max_level == 0 && periodic && !p->fofc) ? 1 : 0;
   p->dt_cached = false;
   if (sc.take_dt && v3) AK_CUDA(cudaMemsetAsync(p->d.smax_bits, 0, 48, p->stream), "reset signal speeds");
-  AK_CUDA(ak::launch_stage(*p, p->u[p->cur], u0, p->u[out], sc), "ak_hydro_stage launch");
+  // with FOFC a cell may have to be updated again from U_in and U0, so the last stage must not overwrite U0 = A in place:
+  // it writes the spare buffer, which then trades places with A
+  const bool to_spare = p->fofc && p->integrator >= 2 && last;
+  double* uout = to_spare ? p->u_spare : p->u[out];
+  AK_CUDA(ak::launch_stage(*p, p->u[p->cur], u0, uout, sc), "ak_hydro_stage launch");
   p->launches += ak::stage_launches_per_call(*p);
   if (sc.take_dt && v3) p->dt_cached = true;
+  if (p->fofc) {
+    // first-order fluxes on the faces of cells whose tentative result is unphysical (before any flux correction
+    // at level boundaries -- moot here: single-level meshes)
+    AK_CUDA(ak::launch_fofc(*p, p->u[p->cur], u0, uout, sc), "FOFC launch");
+    p->launches += 3;
+    if (to_spare) {
+      std::swap(p->u[0], p->u_spare);
+      p->tmap_box[0] = p->tmap_box[1] = 0;        // the tensor maps follow the buffers
+      p->tmap0_box[0] = p->tmap0_box[1] = 0;
+    }
+  }
   if (p->flux_correction && p->d.max_level > 0) {
     AK_CUDA(ak::launch_flux_correction(*p, p->u[p->cur], p->u[out], sc), "flux correction launch");
     p->launches += 3;

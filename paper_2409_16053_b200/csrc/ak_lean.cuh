@@ -169,7 +169,7 @@ __device__ __forceinline__ double sqrt_ratio(double a, double b) {
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(t));
   const double e = fma(-(t * r), r, 1.0);
   r = fma(r, e * fma(0.375, e, 0.5), r);
-  return a * r;
+  return fabs(a) * r;              // (a, b < 0 together, an unphysical face state: the positive root, like sqrt(a / b))
 }
 
 // ---- S3  HLLC, rotated states (rho, u_normal, v, w, u_g) -------------------------------------------
@@ -183,7 +183,9 @@ __device__ __forceinline__ void hllc2(const GasConst& g, const double WL[5], con
   const double ggm1 = g.gamma * g.gm1;
   const double cL = sqrt_ratio(ggm1 * eL, rL), cR = sqrt_ratio(ggm1 * eR, rR);
   const double sl1 = uL - cL, sl2 = uR - cR, sr1 = uL + cL, sr2 = uR + cR;
-  const double SL = sl1 < sl2 ? sl1 : sl2, SR = sr1 > sr2 ? sr1 : sr2;
+  // (this operand order lets a NaN c_L reach S_L and a NaN c_R reach S_R: an unphysical face state gives a NaN flux on
+  // both sides, Q31; for finite operands min and max)
+  const double SL = sl2 < sl1 ? sl2 : sl1, SR = sr1 > sr2 ? sr1 : sr2;
   const double mL = rL * (uL - SL), mR = rR * (SR - uR);
   const double Ss = div2((pL - pR) + fma(mL, uL, mR * uR), mL + mR);
   const double psL = fma(-mL, Ss - uL, pL);
@@ -242,7 +244,7 @@ __device__ __forceinline__ void hllc2n(const GasConst& g, const double WL[N][5],
 #pragma unroll
   for (int f = 0; f < N; f++) {
     const double sl1 = WL[f][1] - cL[f], sl2 = WR[f][1] - cR[f], sr1 = WL[f][1] + cL[f], sr2 = WR[f][1] + cR[f];
-    SL[f] = sl1 < sl2 ? sl1 : sl2; SR[f] = sr1 > sr2 ? sr1 : sr2;
+    SL[f] = sl2 < sl1 ? sl2 : sl1; SR[f] = sr1 > sr2 ? sr1 : sr2;     // (NaN c_L -> S_L, NaN c_R -> S_R, as in hllc2)
     mL[f] = WL[f][0] * (WL[f][1] - SL[f]); mR[f] = WR[f][0] * (SR[f] - WR[f][1]);
   }
 #pragma unroll

@@ -59,6 +59,10 @@ struct ak_pack {
   int variant = 0;
   int bc[6] = {0, 0, 0, 0, 0, 0};  // ak_pack_set_boundaries: x1min,x1max,x2min,x2max,x3min,x3max
   bool flux_correction = false;   // ak_pack_set_flux_correction
+  bool fofc = false;              // ak_pack_set_fofc: first-order flux correction, single-level meshes
+  double* u_spare = nullptr;                  // FOFC: the last stage writes here instead of in place over A; then A and spare swap
+  unsigned char* fofc_flags = nullptr;        // scratch: one flag per cell of every block
+  unsigned long long* fofc_cnt = nullptr;     // scratch: cells flagged in the current stage, and since bind
   bool ghost_push = true;         // ak_pack_set_ghost_push: fuse the same-level periodic ghost fill into the stage kernel
   int tile = -1;                  // -1 = automatic (ak_pack_set_tile)
   long long launches = 0;
@@ -81,4 +85,6 @@ cudaError_t launch_stage(const ak_pack& p, const double* Uin, const double* U0, 
 int stage_launches_per_call(const ak_pack& p);
 // refined meshes, optional: three launches (one per direction) after launch_stage
 cudaError_t launch_flux_correction(const ak_pack& p, const double* Uin, double* Uout, const StageCoef& sc);
+// optional first-order flux correction after launch_stage (single-level meshes): memset + three launches
+cudaError_t launch_fofc(const ak_pack& p, const double* Uin, const double* U0, double* Uout, const StageCoef& sc);
 }  // namespace ak

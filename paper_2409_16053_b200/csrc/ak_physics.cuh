@@ -118,7 +118,8 @@ __device__ __forceinline__ void hllc(const GasConst& g, const double WL[5], cons
   const double rLinv = rcp_(rL), rRinv = rcp_(rR);
   const double cL = sqrt_(g.gamma * pL * rLinv), cR = sqrt_(g.gamma * pR * rRinv);
   // Davis's direct wave-speed estimates (Q2, round-2 reading; Toro Eq.(10.48))
-  const double SL = fmin(uL - cL, uR - cR), SR = fmax(uL + cL, uR + cR);
+  const double sl1 = uL - cL, sl2 = uR - cR, sr1 = uL + cL, sr2 = uR + cR;
+  const double SL = sl2 < sl1 ? sl2 : sl1, SR = sr1 > sr2 ? sr1 : sr2;    // (NaN c_L -> S_L, NaN c_R -> S_R)
   const double bm = fmin(SL, 0.0), bp = fmax(SR, 0.0);
   const double mL = rL * (uL - SL), mR = rR * (SR - uR);
   const double Ss = ((pL - pR) + (mL * uL + mR * uR)) * rcp_(mL + mR);

@@ -8,6 +8,7 @@
 #include "ak_stage_tiled.cuh"
 #include "ak_stage_v3.cuh"
 #include "ak_fluxcorr.cuh"
+#include "ak_fofc.cuh"
 
 #include <cstdlib>
 
@@ -72,6 +73,17 @@ cudaError_t launch_flux_correction(const ak_pack& p, const double* Uin, double* 
     case 2:  return p.recon == 0 ? launch_flux_correction_t<0, 2>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 2>(p, Uin, Uout, sc);
     case 3:  return p.recon == 0 ? launch_flux_correction_t<0, 3>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 3>(p, Uin, Uout, sc);
     default: return p.recon == 0 ? launch_flux_correction_t<0, 0>(p, Uin, Uout, sc) : launch_flux_correction_t<1, 0>(p, Uin, Uout, sc);
+  }
+}
+
+cudaError_t launch_fofc(const ak_pack& p, const double* Uin, const double* U0, double* Uout, const StageCoef& sc) {
+  if (p.recon == 2) return launch_fofc_t<2, 0>(p, Uin, U0, Uout, sc);
+  if (p.recon == 3) return launch_fofc_t<3, 0>(p, Uin, U0, Uout, sc);
+  switch (p.rsolver) {
+    case 1:  return p.recon == 0 ? launch_fofc_t<0, 1>(p, Uin, U0, Uout, sc) : launch_fofc_t<1, 1>(p, Uin, U0, Uout, sc);
+    case 2:  return p.recon == 0 ? launch_fofc_t<0, 2>(p, Uin, U0, Uout, sc) : launch_fofc_t<1, 2>(p, Uin, U0, Uout, sc);
+    case 3:  return p.recon == 0 ? launch_fofc_t<0, 3>(p, Uin, U0, Uout, sc) : launch_fofc_t<1, 3>(p, Uin, U0, Uout, sc);
+    default: return p.recon == 0 ? launch_fofc_t<0, 0>(p, Uin, U0, Uout, sc) : launch_fofc_t<1, 0>(p, Uin, U0, Uout, sc);
   }
 }
 
