@@ -16,9 +16,11 @@
  * convergence order, conservation, uniform-state preservation, mirror / permutation symmetry,
  * decomposition invariance, HLLC consistency / contact / supersonic / mirror properties, PLM and
  * PPM4 linear-data and monotonicity properties, brute-force ghost fill, dyadic-linear
- * restriction / prolongation.  PARITY UNPINNED beyond those properties: the particular HLLC
- * wave-speed estimate, the PPM4 variant (Q5) and the floors (Q7) -- the paper does
- * not fix them.
+ * restriction / prolongation; round 2: closed-form collision fluxes, strong two-shock tube, two-level dt,
+ * PPMX / WENOZ polynomial exactness and the paper's fourth-order linear-wave convergence, FOFC positivity,
+ * Shu-Osher tube.  PARITY UNPINNED beyond those properties: the particular HLLC wave-speed estimate
+ * (Q2: Davis's direct estimates since round 2), the PPM4 variant (Q5), the floors (Q7), the WENOZ and
+ * PPMX variants (Q29, Q30) and the FOFC criterion (Q31) -- the paper does not fix them.
  *
  * Layout: U[m][n][k][j][i], n = (rho, rho v1, rho v2, rho v3, E), i fastest, ghosts included
  * (P:63).  All pointers are HOST pointers owned by the caller.  Single-threaded unless

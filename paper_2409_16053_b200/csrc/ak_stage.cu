@@ -31,7 +31,7 @@ static cudaError_t launch_stage_v3(const ak_pack& p, const double* Uin, const do
   int tile = pick_tile_v3(p);
   if constexpr (RS != 0) { if (tile > 1) tile = 0; }   // LLF / HLLE: only the two 2-CTA/SM tiles are instantiated
   switch (tile) {
-    case 1:  return launch_v3<RECON, RS, 16, 8, 2>(p, Uin, U0, Uout, sc, stage2);
+    case 1:  return launch_v3<RECON, RS, 16, 8, (RECON == 0 ? 3 : 2)>(p, Uin, U0, Uout, sc, stage2);   // PLM: 3 CTAs/SM fit
     case 2:  if constexpr (RS == 0) return launch_v3<RECON, RS, 16, 22, 1>(p, Uin, U0, Uout, sc, stage2);
     case 3:  if constexpr (RS == 0) return launch_v3<RECON, RS, 32, 11, 1>(p, Uin, U0, Uout, sc, stage2);
     default: return launch_v3<RECON, RS, 16, 10, 2>(p, Uin, U0, Uout, sc, stage2);

@@ -465,7 +465,7 @@ cudaError_t launch_v3(const ak_pack& p, const double* Uin, const double* U0, dou
   // split k only when the tiles alone cannot fill the machine a few times over
   const long long target = (long long)p.sm_count * MINB * 4;
   int nchunk = (int)((target + ntiles - 1) / ntiles);
-  int maxchunk = P.nx[2] / 16 > 0 ? P.nx[2] / 16 : 1;
+  int maxchunk = P.nx[2] / 8 > 0 ? P.nx[2] / 8 : 1;
   if (nchunk > maxchunk) nchunk = maxchunk;
   if (nchunk < 1) nchunk = 1;
   const int KC = (P.nx[2] + nchunk - 1) / nchunk;

@@ -468,6 +468,43 @@ def test_llf_hlle_only_in_the_production_kernel(ak):
         pg.hydro_stage(1, 1e-3)
 
 
+# ------------------------------------------------------------ in place of compute-sanitizer (closed on this pool) --------
+@pytest.mark.parametrize("which", ["cfg3", "cfg1_ragged"])
+def test_every_cell_is_written_and_runs_repeat_bit_identically(ak, which):
+    """initcheck / racecheck stand-ins (profiles/r02_sanitizer.md): the output buffer of stage 1 and the ghost cells of
+    buffer A before stage 2 are poisoned with NaN -- afterwards every active AND ghost cell must be finite, i.e. written
+    by the stage kernel (fused fill) --, and two independent runs from the same input agree bit for bit, dt included
+    (a shared-memory or in-place race on the TMA ring would show up as run-to-run noise)."""
+    if which == "cfg3":
+        w = I.config3(nrb=2, nx=32)
+    else:
+        w = I.config1(nrb=2, nx=32)
+        w.mesh = I.uniform_mesh((2, 1, 3), (24, 40, 6), 2)
+    U0 = w.state()
+    g = w.mesh.ng
+    finals = []
+    for rep in range(2):
+        pg = ak.Pack(w.mesh, w.gamma, w.recon)
+        pg.load(U0)
+        dts = []
+        for step in range(3):
+            dt = pg.new_dt(w.cfl)
+            dts.append(dt)
+            pg.fill_ghosts()
+            pg.ub.fill_(float("nan"))                                    # stage 1 writes B
+            pg.hydro_stage(1, dt)
+            assert bool(torch.isfinite(pg.ub).all()), (rep, step, "stage 1 left cells of B unwritten")
+            pg.fill_ghosts()
+            poison = torch.full_like(pg.ua, float("nan"))
+            poison[:, :, g:-g, g:-g, g:-g] = pg.ua[:, :, g:-g, g:-g, g:-g]
+            pg.ua.copy_(poison)                                          # ghost cells of A only
+            pg.hydro_stage(2, dt)
+            assert bool(torch.isfinite(pg.ua).all()), (rep, step, "stage 2 left ghost cells of A unwritten")
+        finals.append((P.gpu_state(pg), dts))
+    assert finals[0][1] == finals[1][1]
+    assert np.array_equal(finals[0][0], finals[1][0])
+
+
 # ------------------------------------------------------------ ghost fill fused into the stage (DESIGN.md 6.3) --------
 @pytest.mark.parametrize("nrb,nx,ng,recon", [
     ((2, 2, 2), (16, 16, 16), 2, 0), ((2, 2, 2), (16, 16, 16), 3, 1), ((1, 1, 1), (8, 8, 8), 2, 0), ((1, 1, 1), (4, 4, 4), 3, 1),
