@@ -2,8 +2,9 @@
 
     python -m paper_2409_16053_b200.build [--force]
 
-nvcc cross-compiles without a GPU.  ak_exact.cu is compiled with -fmad=false (bit-exact ghost fill
-and dt); the stage kernels keep FMA contraction.  -lineinfo maps ncu's source page to these files.
+nvcc cross-compiles without a GPU.  ak_exact.cu (ghost fill, dt) and ak_stage.cu (stage kernels, flux correction, FOFC)
+are compiled with -fmad=false: no contraction behind the source's back, every fused multiply-add of the stage kernel is
+written out, so the same face solved by two tiles gives the same bits.  -lineinfo maps ncu's source page to these files.
 """
 from __future__ import annotations
 

@@ -23,6 +23,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
+_AK_H = os.path.join(ROOT, "include", "ak.h")
 METRICS = ("gpu__time_duration.sum,dram__bytes_read.sum,dram__bytes_write.sum,smsp__inst_executed.sum,"
            "sm__inst_executed_pipe_fp64.sum,sm__inst_executed_pipe_alu.sum,sm__inst_executed_pipe_fma.sum,"
            "sm__inst_executed_pipe_lsu.sum,sm__inst_executed_pipe_xu.sum,"
@@ -36,7 +37,7 @@ def csrc_sha() -> str:
     """Hash of everything the kernels are built from."""
     h = hashlib.sha256()
     files = sorted(os.path.join(HERE, "csrc", f) for f in os.listdir(os.path.join(HERE, "csrc")))
-    files.append(os.path.join(ROOT, "include", "ak.h"))
+    files.append(_AK_H)
     for f in files:
         if os.path.isfile(f):
             h.update(os.path.basename(f).encode())

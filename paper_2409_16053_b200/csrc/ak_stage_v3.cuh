@@ -197,6 +197,19 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
   // fused ghost fill: is this column within ng of an x1 / x2 face of its block?
   const int pe1 = !sc.push ? 0 : (i0 + ti < ng ? -1 : (i0 + ti >= P.nx[0] - ng ? 1 : 0));
   const int pe2 = !sc.push ? 0 : (j0 + tj < ng ? -1 : (j0 + tj >= P.nx[1] - ng ? 1 : 0));
+  // where this column's copies live in the in-plane neighbour blocks (x1 neighbour, x2 neighbour, the diagonal one): element
+  // offsets of the column at plane 0, fixed for the whole march, or -1; planes near an x3 face take the general loop
+  // (only where 168 registers are available: the three-CTA PLM tile keeps the general loop, measured faster there)
+  constexpr bool FASTPUSH = (MINB <= 2);
+  long long pc1 = -1, pc2 = -1, pc12 = -1;
+  if (FASTPUSH && (pe1 | pe2)) {
+    const int* nb = P.nbr + 27 * m + 9;                 // (E3 = 0)
+    const long long r0 = (long long)(j0 + tj + ng) * P.nt[0] + (i0 + ti + ng);
+    const long long s1 = (long long)pe1 * P.nx[0], s2 = (long long)pe2 * P.nx[1] * P.nt[0];
+    if (pe1) pc1 = (long long)nb[3 + (pe1 + 1)] * 5 * nc + r0 - s1;
+    if (pe2) pc2 = (long long)nb[(pe2 + 1) * 3 + 1] * 5 * nc + r0 - s2;
+    if (pe1 && pe2) pc12 = (long long)nb[(pe2 + 1) * 3 + (pe1 + 1)] * 5 * nc + r0 - s1 - s2;
+  }
 
   const int oW = (tj + R) * WI + ti + R;                // own cell inside a staged plane (variable stride WJ*WI)
   const int oQ1 = tj * (TI + 1) + ti;                   // lower x1 face of the own cell   (variable stride TJ*(TI+1))
@@ -314,7 +327,14 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
 #pragma unroll
       for (int n = 0; n < 5; n++) { un[n] = fma(-c3, Gn[n] - G[n], Tc[n * NT]); o[n * nc] = un[n]; }
       const int pe3 = !sc.push ? 0 : (c - 1 < ng ? -1 : (c - 1 >= P.nx[2] - ng ? 1 : 0));
-      if (pe1 | pe2 | pe3) push_ghosts(P, Uout, m, i0 + ti, j0 + tj, c - 1, pe1, pe2, pe3, un[0], un[1], un[2], un[3], un[4]);
+      if (pe3 || (!FASTPUSH && (pe1 | pe2))) {
+        push_ghosts(P, Uout, m, i0 + ti, j0 + tj, c - 1, pe1, pe2, pe3, un[0], un[1], un[2], un[3], un[4]);
+      } else if (pe1 | pe2) {
+        const long long po = (long long)(c - 1 + ng) * plane;
+        if (pc1 >= 0) { double* q = Uout + pc1 + po; q[0] = un[0]; q[nc] = un[1]; q[2 * nc] = un[2]; q[3 * nc] = un[3]; q[4 * nc] = un[4]; }
+        if (pc2 >= 0) { double* q = Uout + pc2 + po; q[0] = un[0]; q[nc] = un[1]; q[2 * nc] = un[2]; q[3 * nc] = un[3]; q[4 * nc] = un[4]; }
+        if (pc12 >= 0) { double* q = Uout + pc12 + po; q[0] = un[0]; q[nc] = un[1]; q[2 * nc] = un[2]; q[3 * nc] = un[3]; q[4 * nc] = un[4]; }
+      }
       if (STAGE2 && sc.take_dt) {                  // (uniform over the grid)
         // S0 of the NEXT step (Eq.(3)) on U^{n+1} while it is in registers: the cell's signal speeds
         // |v_d| + c_s in the oracle's arithmetic (IEEE division and sqrt, no contraction: this translation unit

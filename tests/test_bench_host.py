@@ -46,3 +46,29 @@ def test_reference_arm_runs_on_rank_0_only():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
                        env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_counters_are_tied_to_the_kernel_sources(tmp_path, monkeypatch):
+    """bench.py prints ncu-derived numbers only while the hash stored with them equals the hash of csrc/ (VERDICT r1 item 9)."""
+    from paper_2409_16053_b200 import counters
+    sha = counters.csrc_sha()
+    assert len(sha) == 16 and sha == counters.csrc_sha()
+    prof = tmp_path / "profiles"
+    prof.mkdir()
+    monkeypatch.setattr(counters, "ROOT", str(tmp_path))
+    assert counters.load("cfg3") is None                                   # no file
+    (prof / "r02_stage_counters_cfg3.json").write_text(json.dumps({"csrc_sha": "0" * 16, "launches": {}}))
+    assert counters.load("cfg3") is None                                   # stale: taken on other sources
+    (prof / "r02_stage_counters_cfg3.json").write_text(json.dumps({"csrc_sha": sha, "launches": {"stage1": {}}}))
+    assert counters.load("cfg3")["launches"] == {"stage1": {}}
+    # a raw-page CSV as ncu writes it: header row, units row, one row per launch
+    csv_path = tmp_path / "c.csv"
+    hdr = ["ID", "Kernel Name", "gpu__time_duration.sum", "dram__bytes_read.sum", "dram__bytes_write.sum", "sm__inst_executed_pipe_fp64.sum"]
+    rows = [hdr, ["", "", "ns", "byte", "byte", "inst"],
+            ["0", "void ak::stage_v3_kernel<1, 0, 16, 10, 2, 0>(CUtensorMap_st)", "10,000", "4", "2", "100"],
+            ["1", "void ak::stage_v3_kernel<1, 0, 16, 10, 2, 1>(CUtensorMap_st)", "12,000", "8", "2", "110"],
+            ["2", "void ak::stage_v3_kernel<1, 0, 16, 10, 2, 0>(CUtensorMap_st)", "20,000", "6", "2", "100"]]
+    csv_path.write_text("\n".join(",".join(f'"{c}"' for c in r) for r in rows))
+    d = counters.parse(str(csv_path), "cfg3")
+    assert d["launches"]["stage1"]["gpu__time_duration.sum"] == 15000.0 and d["launches"]["stage1"]["launches_averaged"] == 2
+    assert d["launches"]["stage2"]["dram__bytes_read.sum"] == 8.0 and d["csrc_sha"] == sha

@@ -138,7 +138,9 @@ def test_sod_converges_to_the_exact_solution(orc, rsolver, name):
         assert abs(U[0].sum() - U0[0].sum()) <= 1e-13 * U0[0].sum()
     r1, r2 = math.log2(errs[128] / errs[256]), math.log2(errs[256] / errs[512])
     assert 0.6 <= r1 <= 1.15 and 0.6 <= r2 <= 1.15, (errs, r1, r2)
-    # more diffusive than HLLC on the contact, but the same solution: errors within a factor 2.5 of each other
+    # the same solution as HLLC: errors within a factor 2.5 of each other.  LLF / HLLE smear the contact more than HLLC
+    # (error above it); Roe, which resolves the contact exactly and carries less numerical viscosity at the shock than
+    # HLLC's bounding wave speeds, ends slightly BELOW it -- hence the lower bound 0.9 (widened from 1.0 when Roe was added)
     _, Uc = sod_run(orc, 256, I.RECON_PLM, 2, rsolver=0)
     x = (np.arange(256) + 0.5) / 256
     rho_ex, _ = sod_sample(g, (x[x >= 0.5] - 0.75) / 0.1, ps, us)
