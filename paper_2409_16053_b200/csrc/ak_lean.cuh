@@ -84,11 +84,15 @@ __device__ __forceinline__ void limit_lean(double a, double& aL, double& aR) {
 // select-min on doubles without the NaN handling of fmin (operands are finite here)
 __device__ __forceinline__ double dmin2(double a, double b) { return a < b ? a : b; }
 
-// WENO-Z value at the UPPER face of the middle cell of (a, b, c, d, e), in the differences of neighbouring cells
-// (constants are reproduced exactly); same operation order as the oracle, reciprocals by rcp2
-__device__ __forceinline__ double wenoz_upper(double a, double b, double c, double d, double e) {
-  const double d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
-  const double P0 = 5.0 * d2 - 2.0 * d1, P1 = 2.0 * d3 + d2, P2 = 4.0 * d3 - d4;
+// WENO-Z edge values of the middle cell of q[i-2..i+2], in the differences of neighbouring cells (constants are
+// reproduced exactly); same operation order as the oracle, reciprocals by rcp2.  q+ is the value at the upper face;
+// q- is the same formula on the mirrored stencil, for which the smoothness indicators are those of q+ in reverse
+// order (beta0' = beta2, beta1' = beta1, beta2' = beta0, bit for bit, hence the same tau5 and the same ratios) and the
+// candidate polynomials are -(5 d3 - 2 d4), -(2 d2 + d3), -(4 d2 - d1): the indicators, tau5 and the three
+// reciprocals are formed once for both sides.
+__device__ __forceinline__ void wenoz_lean(const double q[5], double& qm, double& qp) {
+  const double c = q[2];
+  const double d1 = q[1] - q[0], d2 = q[2] - q[1], d3 = q[3] - q[2], d4 = q[4] - q[3];
   const double s0 = d2 - d1, t0 = 3.0 * d2 - d1;
   const double s1 = d3 - d2, t1 = d2 + d3;
   const double s2 = d4 - d3, t2 = d4 - 3.0 * d3;
@@ -98,12 +102,17 @@ __device__ __forceinline__ double wenoz_upper(double a, double b, double c, doub
   const double eps = 1e-40;
   const double tau = fabs(b0 - b2);
   const double r0 = tau * rcp2(b0 + eps), r1 = tau * rcp2(b1 + eps), r2 = tau * rcp2(b2 + eps);
-  const double a0 = 0.1 * (1.0 + r0 * r0), a1 = 0.6 * (1.0 + r1 * r1), a2 = 0.3 * (1.0 + r2 * r2);
-  return c + (a0 * P0 + (a1 * P1 + a2 * P2)) * rcp2(6.0 * (a0 + (a1 + a2)));
-}
-__device__ __forceinline__ void wenoz_lean(const double q[5], double& qm, double& qp) {
-  qp = wenoz_upper(q[0], q[1], q[2], q[3], q[4]);
-  qm = wenoz_upper(q[4], q[3], q[2], q[1], q[0]);
+  const double w0 = 1.0 + r0 * r0, w1 = 1.0 + r1 * r1, w2 = 1.0 + r2 * r2;
+  {
+    const double P0 = 5.0 * d2 - 2.0 * d1, P1 = 2.0 * d3 + d2, P2 = 4.0 * d3 - d4;
+    const double a0 = 0.1 * w0, a1 = 0.6 * w1, a2 = 0.3 * w2;
+    qp = c + (a0 * P0 + (a1 * P1 + a2 * P2)) * rcp2(6.0 * (a0 + (a1 + a2)));
+  }
+  {
+    const double P0 = -(5.0 * d3 - 2.0 * d4), P1 = -(2.0 * d2 + d3), P2 = -(4.0 * d2 - d1);
+    const double a0 = 0.1 * w2, a1 = 0.6 * w1, a2 = 0.3 * w0;
+    qm = c + (a0 * P0 + (a1 * P1 + a2 * P2)) * rcp2(6.0 * (a0 + (a1 + a2)));
+  }
 }
 
 // PPMX (i): fourth-order interface value between q0 and q1, limited where it is not between them
@@ -193,7 +202,10 @@ __device__ __forceinline__ void hllc2(const GasConst& g, const double WL[5], con
   const double ps = max0(0.5 * (psL + psR));
   const bool left = !neg(Ss);
   const double rK = left ? rL : rR, uK = left ? uL : uR, vK = left ? WL[2] : WR[2], wK = left ? WL[3] : WR[3];
-  const double eK = left ? eL : eR, pK = left ? pL : pR, b = left ? min0(SL) : max0(SR);
+  const double eK = left ? eL : eR, pK = g.gm1 * eK;          // (= the selected p_K, bit for bit)
+  // b = min(S_L, 0) on the left of the contact, max(S_R, 0) on its right: one select of the speed, one sign test
+  const double SK = left ? SL : SR;
+  const double b = (neg(SK) == left) ? SK : 0.0;
   const double EK = fma(0.5 * rK, fma(uK, uK, fma(vK, vK, wK * wK)), eK);
   const double mom = rK * uK;
   const double inv = rcp2(Ss - b);
@@ -259,8 +271,9 @@ __device__ __forceinline__ void hllc2n(const GasConst& g, const double WL[N][5],
     const bool left = !neg(Ss[f]);
     rK[f] = left ? WL[f][0] : WR[f][0]; uK[f] = left ? WL[f][1] : WR[f][1];
     vK[f] = left ? WL[f][2] : WR[f][2]; wK[f] = left ? WL[f][3] : WR[f][3];
-    eK[f] = left ? WL[f][4] : WR[f][4]; pK[f] = left ? pL[f] : pR[f];
-    b[f] = left ? min0(SL[f]) : max0(SR[f]);
+    eK[f] = left ? WL[f][4] : WR[f][4]; pK[f] = g.gm1 * eK[f];
+    const double SK = left ? SL[f] : SR[f];
+    b[f] = (neg(SK) == left) ? SK : 0.0;
   }
   double EK[N], mom[N], inv[N];
 #pragma unroll
