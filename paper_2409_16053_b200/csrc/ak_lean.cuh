@@ -1,8 +1,8 @@
 // ak_lean.cuh -- branch-free, instruction-lean forms of the per-cell / per-face arithmetic for the
 // production stage kernel (ak_stage_v3.cuh).  Same formulas as ak_physics.cuh (DESIGN.md section 2
-// readings Q1-Q7; paper P:101 reconstruction on primitives, P:103 HLLC, P:122-126 gamma-law gas); they
-// differ from it by rounding only (a few ulp) and are written against what profiles/r01_v1_stage_cfg3.md
-// showed to be expensive on sm_100a:
+// readings Q1-Q7, Q29-Q31; paper P:101 reconstruction on primitives, P:103 HLLC, P:122-126 gamma-law gas); they
+// differ from it by rounding only (a few ulp) and are written against what the ncu captures of round 1 showed to be
+// expensive on sm_100a (every FP64-pipe and every ALU-pipe instruction costs about two issue cycles):
 //   * fmin/fmax on doubles lower to DSETP + SEL/FSEL + several moves (NaN handling): replaced by one
 //     compare + select, or by a sign test of the high word on the integer pipe where the other operand is 0;
 //   * data-dependent branches (shock branch of the wave speeds, CW84 limiter cases) diverge inside a warp
