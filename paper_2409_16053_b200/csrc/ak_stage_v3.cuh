@@ -82,6 +82,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
                 double* __restrict__ Uout, StageCoef sc, int KC, int ntile_i) {
   using S = V3Tile<RECON, TI, TJ>;
   constexpr int R = S::R, WI = S::WI, WJ = S::WJ, NT = S::NT, NS = S::NS, NH = S::NH, NTH = S::NTH;
+  constexpr bool SHARE = (RECON == 1);        // PPM4: every interface value computed once and shared through the Q slots
   extern __shared__ __align__(1024) double sm[];
   // sm[0 .. 2 nUpad)        staged U plane ring, converted to W in place      [2][5][WJ][WI]
   // sm[oQ .. oQ + 2 nQ)     per plane parity: Q1 [5][TJ][TI+1] (q+ along x1 of cells -1..TI-1, then F1 at
@@ -153,15 +154,52 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
       const double* Ws = sm + b * S::nUpad;
       double* Q = sm + S::oQ + b * S::nQ;
       double qmE[NE][5];
+      if constexpr (SHARE) {
+        // PPM4 with interface values computed once per face: B1 -- the interface below halo cell -1 (register), the
+        // two interfaces of halo cell wI (the lower one also into the slot worker wI-1 reads as its upper interface)
+        double loA[NE][5], loB[NE][5], hiB[NE][5];
 #pragma unroll
-      for (int q = 0; q < NE; q++) {
-        if (inplane && extra[q]) {
+        for (int q = 0; q < NE; q++) {
+          if (inplane && extra[q]) {
 #pragma unroll
-          for (int n = 0; n < 5; n++) {
-            double qm, qp;
-            recon2<RECON>(Ws + n * (WJ * WI) + eA[q], eSt[q], qm, qp);
-            Q[n * eQn[q] + eQlo[q]] = qp;
-            recon2<RECON>(Ws + n * (WJ * WI) + eB[q], eSt[q], qmE[q][n], qp);
+            for (int n = 0; n < 5; n++) {
+              const double* pa = Ws + n * (WJ * WI) + eA[q];
+              const double* pb = Ws + n * (WJ * WI) + eB[q];
+              const int st = eSt[q];
+              loA[q][n] = iface_lean(pa[-2 * st], pa[-st], pa[0], pa[st]);
+              loB[q][n] = iface_lean(pb[-2 * st], pb[-st], pb[0], pb[st]);
+              hiB[q][n] = iface_lean(pb[-st], pb[0], pb[st], pb[2 * st]);
+              Q[n * eQn[q] + eQhi[q]] = loB[q][n];
+            }
+          }
+        }
+        cta_sync(NTH);                                  // interface values visible
+        // B2 -- limit the two halo cells: q+ of cell -1 replaces worker 0's interface value in its slot, q- of cell wI stays here
+#pragma unroll
+        for (int q = 0; q < NE; q++) {
+          if (inplane && extra[q]) {
+#pragma unroll
+            for (int n = 0; n < 5; n++) {
+              double lo = loA[q][n], hi = Q[n * eQn[q] + eQlo[q]];
+              limit_lean(Ws[n * (WJ * WI) + eA[q]], lo, hi);
+              Q[n * eQn[q] + eQlo[q]] = hi;
+              double lo2 = loB[q][n], hi2 = hiB[q][n];
+              limit_lean(Ws[n * (WJ * WI) + eB[q]], lo2, hi2);
+              qmE[q][n] = lo2;
+            }
+          }
+        }
+      } else {
+#pragma unroll
+        for (int q = 0; q < NE; q++) {
+          if (inplane && extra[q]) {
+#pragma unroll
+            for (int n = 0; n < 5; n++) {
+              double qm, qp;
+              recon2<RECON>(Ws + n * (WJ * WI) + eA[q], eSt[q], qm, qp);
+              Q[n * eQn[q] + eQlo[q]] = qp;
+              recon2<RECON>(Ws + n * (WJ * WI) + eB[q], eSt[q], qmE[q][n], qp);
+            }
           }
         }
       }
@@ -398,7 +436,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
             else        { qm2[n] = c[n] - h; Q2[n * ((TJ + 1) * TI) + oQ2 + TI] = c[n] + h; }
           }
         }
-      } else {
+      } else if constexpr (!SHARE) {
 #pragma unroll
         for (int n = 0; n < 5; n++) {
           const double* p = Ws + n * (WJ * WI) + oW;
@@ -407,6 +445,36 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
           Q1[n * (TJ * (TI + 1)) + oQ1 + 1] = qp;
           recon2<RECON>(p, WI, qm2[n], qp);
           Q2[n * ((TJ + 1) * TI) + oQ2 + TI] = qp;
+        }
+      }
+    }
+    if constexpr (SHARE) {
+      // B1: the interface values at the LOWER x1 and x2 faces of the own cell -- kept, and stored in that face's slot for
+      // the neighbour below, whose upper interface it is (the upper interfaces of the tile's last row / column come from
+      // the edge warp)
+      if (inplane && valid) {
+#pragma unroll
+        for (int n = 0; n < 5; n++) {
+          const double* p = Ws + n * (WJ * WI) + oW;
+          qm1[n] = iface_lean(p[-2], p[-1], p[0], p[1]);
+          qm2[n] = iface_lean(p[-2 * WI], p[-WI], p[0], p[WI]);
+          Q1[n * (TJ * (TI + 1)) + oQ1] = qm1[n];
+          Q2[n * ((TJ + 1) * TI) + oQ2] = qm2[n];
+        }
+      }
+      cta_sync(NTH);                                    // interface values visible
+      // B2: CW84 limiter on (lower interface, cell, upper interface); q+ overwrites the upper interface in the slot only
+      // this thread reads, q- stays in registers
+      if (inplane && valid) {
+#pragma unroll
+        for (int n = 0; n < 5; n++) {
+          const double a = Ws[n * (WJ * WI) + oW];
+          double hi = Q1[n * (TJ * (TI + 1)) + oQ1 + 1];
+          limit_lean(a, qm1[n], hi);
+          Q1[n * (TJ * (TI + 1)) + oQ1 + 1] = hi;
+          double hi2 = Q2[n * ((TJ + 1) * TI) + oQ2 + TI];
+          limit_lean(a, qm2[n], hi2);
+          Q2[n * ((TJ + 1) * TI) + oQ2 + TI] = hi2;
         }
       }
     }
