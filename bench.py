@@ -168,6 +168,8 @@ def run_ours(args):
         pack.set_flux_correction(True)
     if args.integrator == 3:
         pack.set_integrator(3)
+    if args.tile is not None:
+        pack.set_tile(args.tile)
     U0 = w.state(device=dev)
     pack.load(U0)
     ncell = mesh.ncells_active
@@ -215,7 +217,7 @@ def run_ours(args):
     achieved = alg_bytes / (stage_ms * 1e-3) / 1e9
     from paper_2409_16053_b200 import counters
     ctr = counters.load(args.workload) if (args.variant == 0 and args.rsolver == "hllc" and args.integrator == 2
-                                            and args.recon is None and not args.flux_correction) else None
+                                            and args.recon is None and not args.flux_correction and args.tile is None) else None
     traffic = args.traffic
     if traffic is None and ctr:
         L = ctr["launches"]
@@ -332,6 +334,7 @@ def main():
                     help="stages per step: 2 = SSPRK(2,2) (headline), 3 = SSPRK(3,3) (f2 variant, third state register)")
     ap.add_argument("--flux-correction", action="store_true",
                     help="refined meshes (cfg4): flux correction at coarse-fine faces on (SURVEY 8(f) f1; off by default)")
+    ap.add_argument("--tile", type=int, default=None, help="tile shape of the production kernel (ak_pack_set_tile; default: automatic)")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per stage launch from the committed ncu --set full capture (profiles/)")
     args = ap.parse_args()

@@ -83,6 +83,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
   using S = V3Tile<RECON, TI, TJ>;
   constexpr int R = S::R, WI = S::WI, WJ = S::WJ, NT = S::NT, NS = S::NS, NH = S::NH, NTH = S::NTH;
   constexpr bool SHARE = (RECON == 1);        // PPM4: every interface value computed once and shared through the Q slots
+  constexpr bool EDGEHALO = SHARE;            // ... and the edge warp, lighter by then, converts the cross-shaped halo
   extern __shared__ __align__(1024) double sm[];
   // sm[0 .. 2 nUpad)        staged U plane ring, converted to W in place      [2][5][WJ][WI]
   // sm[oQ .. oQ + 2 nQ)     per plane parity: Q1 [5][TJ][TI+1] (q+ along x1 of cells -1..TI-1, then F1 at
@@ -144,6 +145,23 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
           const int c = e - wJ;
           eSt[q] = WI; eA[q] = (R - 1) * WI + c + R; eB[q] = (R + wJ) * WI + c + R;
           eQlo[q] = S::nQ1 + c; eQhi[q] = S::nQ1 + wJ * TI + c; eQn[q] = (TJ + 1) * TI;
+        }
+      }
+    }
+    // cross-shaped halo of the tile (2 R (wI + wJ) cells per plane), NHE cells per lane, offsets fixed for the whole march
+    constexpr int NHE = EDGEHALO ? (2 * R * (TI + TJ) + 31) / 32 : 1;
+    int eH[NHE];
+    if constexpr (EDGEHALO) {
+      const int nh1 = 2 * R * wJ, nhalo = nh1 + 2 * R * wI;
+#pragma unroll
+      for (int q = 0; q < NHE; q++) {
+        const int h = lane + 32 * q;
+        eH[q] = -1;
+        if (h < nhalo) {
+          int ii, jj;
+          if (h < nh1) { jj = h / (2 * R); const int c = h - jj * (2 * R); ii = c < R ? c - R : wI + c - R; }
+          else { const int hh = h - nh1; const int r = hh / wI; ii = hh - r * wI; jj = r < R ? r - R : wJ + r - R; }
+          eH[q] = (jj + R) * WI + ii + R;
         }
       }
     }
@@ -217,6 +235,24 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
           flux3_12<RS>(g, ex2[q], L, qmE[q], F);
 #pragma unroll
           for (int n = 0; n < 5; n++) Q[n * eQn[q] + eQhi[q]] = F[n];
+        }
+      }
+      if constexpr (EDGEHALO) {
+        // conserved -> primitive of the halo cells of plane s+1 (the workers convert their own cells meanwhile)
+        if (s + 1 >= k0 && s + 1 < k1) {
+          double* Wn = sm + ((it + 1) & 1) * S::nUpad;
+          mbar_wait(&bars[(it + 1) & 1], ((it + 1) >> 1) & 1);
+#pragma unroll
+          for (int q = 0; q < NHE; q++) {
+            if (eH[q] >= 0) {
+              double u[5], w[5];
+#pragma unroll
+              for (int n = 0; n < 5; n++) u[n] = Wn[n * (WJ * WI) + eH[q]];
+              c2p_lean(u, w, g.ug_floor);
+#pragma unroll
+              for (int n = 0; n < 5; n++) Wn[n * (WJ * WI) + eH[q]] = w[n];
+            }
+          }
         }
       }
       cta_sync(NTH);                                    // fluxes of plane s visible
@@ -309,7 +345,7 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
         else Tn[n * NT] = u[n];                    // 0*U + 1*U of the stage-1 weights, exactly
       }
     }
-    if (inplane) {
+    if (!EDGEHALO && inplane) {
 #pragma unroll
       for (int q = 0; q < NH; q++) {
         if (oH[q] >= 0) {
