@@ -202,7 +202,7 @@ __device__ __forceinline__ void hllc2(const GasConst& g, const double WL[5], con
   const double ps = max0(0.5 * (psL + psR));
   const bool left = !neg(Ss);
   const double rK = left ? rL : rR, uK = left ? uL : uR, vK = left ? WL[2] : WR[2], wK = left ? WL[3] : WR[3];
-  const double eK = left ? eL : eR, pK = g.gm1 * eK;          // (= the selected p_K, bit for bit)
+  const double eK = left ? eL : eR, pK = left ? pL : pR;      // (p_K = (gamma-1) e_K would save the select but costs spills in the 128-register tile)
   // b = min(S_L, 0) on the left of the contact, max(S_R, 0) on its right: one select of the speed, one sign test
   const double SK = left ? SL : SR;
   const double b = (neg(SK) == left) ? SK : 0.0;
@@ -271,7 +271,7 @@ __device__ __forceinline__ void hllc2n(const GasConst& g, const double WL[N][5],
     const bool left = !neg(Ss[f]);
     rK[f] = left ? WL[f][0] : WR[f][0]; uK[f] = left ? WL[f][1] : WR[f][1];
     vK[f] = left ? WL[f][2] : WR[f][2]; wK[f] = left ? WL[f][3] : WR[f][3];
-    eK[f] = left ? WL[f][4] : WR[f][4]; pK[f] = g.gm1 * eK[f];
+    eK[f] = left ? WL[f][4] : WR[f][4]; pK[f] = left ? pL[f] : pR[f];
     const double SK = left ? SL[f] : SR[f];
     b[f] = (neg(SK) == left) ? SK : 0.0;
   }

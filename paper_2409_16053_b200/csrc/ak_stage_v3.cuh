@@ -83,7 +83,9 @@ stage_v3_kernel(const __grid_constant__ CUtensorMap tmU, const __grid_constant__
   using S = V3Tile<RECON, TI, TJ>;
   constexpr int R = S::R, WI = S::WI, WJ = S::WJ, NT = S::NT, NS = S::NS, NH = S::NH, NTH = S::NTH;
   constexpr bool SHARE = (RECON == 1);        // PPM4: every interface value computed once and shared through the Q slots
-  constexpr bool EDGEHALO = SHARE;            // ... and the edge warp, lighter by then, converts the cross-shaped halo
+  // ... and the edge warp converts the cross-shaped halo where that balances the schedulers (measured: PLM and PPM4;
+  // not PPMX / WENOZ, whose edge warp is the heavy one)
+  constexpr bool EDGEHALO = (RECON <= 1);
   extern __shared__ __align__(1024) double sm[];
   // sm[0 .. 2 nUpad)        staged U plane ring, converted to W in place      [2][5][WJ][WI]
   // sm[oQ .. oQ + 2 nQ)     per plane parity: Q1 [5][TJ][TI+1] (q+ along x1 of cells -1..TI-1, then F1 at
