@@ -107,6 +107,19 @@ int ak_hydro_stage(ak_pack*, int stage, double dt);
  * (48 bytes copied, no launch); otherwise a reduction kernel reads the state.  Both give the same bits. */
 int ak_new_dt(ak_pack*, double cfl, double* dt_out);
 
+/* The same CFL reduction (Eq.(3); the kernel ak_new_dt launches) for callers that may not allocate device
+ * memory -- code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc -- and have no pack
+ * with its caller-allocated scratch buffer.  u: DEVICE pointer to U[m][n][k][j][i] of a uniform single-level pack of nmb
+ * MeshBlocks of nx1 x nx2 x nx3 active cells with ng ghost layers (ghost cells are not read); dx1..3: cell sizes;
+ * dt_out: HOST pointer, receives cfl * min over active cells and directions of dx_d / (|v_d| + c_s), bit-identical to
+ * ak_new_dt on the same state.  The reduction cells and the block table live in a 128 KiB static device array inside the
+ * library (held by every GPU that loads the library until exit); nmb <= 8176, else AK_EUNSUPPORTED.  Calls no cudaMalloc,
+ * cudaFree or allocating library routine.  Runs on the device that owns u, on cuda_stream, and synchronises it.  All
+ * calls share the array: every call rewrites what it uses first, but calls that overlap on one GPU (two streams, two
+ * threads) race on it -- serialise them.  AK_ENONFINITE for a NaN / inf state. */
+int ak_new_dt_noalloc(const void* u, int nmb, int nx1, int nx2, int nx3, int ng, double gamma,
+                      double dx1, double dx2, double dx3, double cfl, void* cuda_stream, double* dt_out);
+
 /* Convenience: ak_new_dt, then (ak_fill_ghosts, ak_hydro_stage) for every stage of the integrator (2 by default,
  * 3 after ak_pack_set_integrator(p, 3, u_c)).  dt_out (HOST, may be NULL)
  * receives the step taken.  If dt_fixed > 0 it is used instead of the CFL value (lock-step parity

@@ -24,7 +24,7 @@ SYMBOLS = [
     "ak_last_error", "ak_pack_create", "ak_pack_set_mesh", "ak_pack_set_block", "ak_pack_state_bytes",
     "ak_pack_scratch_bytes", "ak_pack_bind", "ak_fill_ghosts", "ak_hydro_stage", "ak_new_dt", "ak_step",
     "ak_pack_current", "ak_pack_upload", "ak_pack_download", "ak_pack_download_async", "ak_pack_floor_count", "ak_pack_set_variant", "ak_pack_set_tile", "ak_pack_set_flux_correction", "ak_pack_set_ghost_push", "ak_pack_set_fofc", "ak_pack_fofc_count", "ak_pack_set_boundaries", "ak_pack_set_integrator",
-    "ak_pack_launch_count", "ak_pack_destroy",
+    "ak_pack_launch_count", "ak_pack_destroy", "ak_new_dt_noalloc",
 ]
 
 
@@ -68,6 +68,7 @@ def lib():
         "ak_pack_set_integrator": (i, [vp, i, vp]),
         "ak_pack_launch_count": (ll, [vp]),
         "ak_pack_destroy": (i, [vp]),
+        "ak_new_dt_noalloc": (i, [vp, i, i, i, i, i, d, d, d, d, d, vp, C.POINTER(d)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -79,6 +80,18 @@ def lib():
 def _chk(rc):
     if rc != AK_OK:
         raise AkError(f"ak error {rc}: {lib().ak_last_error().decode()}")
+
+
+def new_dt_noalloc(U, mesh, gamma, cfl, stream=None):
+    """ak_new_dt_noalloc: the CFL reduction on a device tensor U of mesh.state_shape() (uniform single-level mesh) with
+    the library's static scratch array -- no pack, no allocation (include/ak.h)."""
+    assert U.is_cuda and U.is_contiguous() and U.dtype == torch.float64 and tuple(U.shape) == tuple(mesh.state_shape())
+    st = stream if stream is not None else torch.cuda.current_stream(U.device)
+    dx = mesh.dx(0)
+    dt = C.c_double()
+    _chk(lib().ak_new_dt_noalloc(U.data_ptr(), mesh.nmb, *mesh.nx, mesh.ng, gamma, dx[0], dx[1], dx[2], cfl,
+                                 st.cuda_stream, C.byref(dt)))
+    return dt.value
 
 
 class Pack:

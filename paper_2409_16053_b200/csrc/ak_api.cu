@@ -18,6 +18,7 @@ static int cuda_fail(cudaError_t e, const char* where) {
 #define AK_CUDA(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, where); } while (0)
 
 extern "C" const char* ak_last_error(void) { return g_err.c_str(); }
+namespace ak { int set_error(int code, const char* msg) { return fail(code, msg); } }
 
 // every launching entry point runs on the device that owns the pack's buffers, whatever the caller's current device
 struct DeviceGuard {

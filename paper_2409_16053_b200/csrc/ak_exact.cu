@@ -5,6 +5,7 @@
 #define AK_EXACT_MATH 1
 #include "ak_pack.h"
 #include "ak_physics.cuh"
+#include <cstring>
 
 namespace ak {
 
@@ -276,3 +277,95 @@ cudaError_t launch_new_dt(const ak_pack& p, const double* U) {
 }
 
 }  // namespace ak
+
+// ---- S0 without any allocation: ak_new_dt_noalloc (include/ak.h) ---------------------------------------------------
+// Some callers cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it) and
+// have no pack with its caller-allocated scratch buffer either.  This entry point runs the SAME reduction kernel as
+// ak_new_dt (new_dt_kernel above, unchanged) on a caller-owned state buffer of a uniform single-level pack; the scratch
+// the kernel needs -- the reduction cells and the block table it reads each block's level from -- lives in the
+// file-scope device array below instead of a caller buffer.  Every GPU that loads the library holds its
+// AK_NOALLOC_SCRATCH_BYTES (128 KiB) until exit.  All calls share the array and it keeps the last call's contents:
+// every call rewrites the cells and the table entries it uses before the reduction reads them (noalloc_setup_kernel,
+// same stream), and two calls that overlap on one GPU (different streams or threads) race on it.
+#define AK_NOALLOC_SCRATCH_BYTES (128 * 1024)
+#define AK_NOALLOC_MAX_BLOCKS ((AK_NOALLOC_SCRATCH_BYTES - 256) / (int)sizeof(int4))      /* 8176 */
+static __device__ __align__(256) unsigned char g_noalloc_scratch[AK_NOALLOC_SCRATCH_BYTES];
+
+namespace ak {
+// layout of g_noalloc_scratch: [0, 8) min dt as ordered bits | [8, 16) unused | [16, 24) rows with a non-finite signal
+// speed | [256, 256 + 16 nmb) block table int4 (level, lx1, lx2, lx3): level 0 for every block of a uniform pack.
+// Device code names the array directly; host code must not (there the name is a host-side stand-in).
+__global__ void __launch_bounds__(256) noalloc_setup_kernel(int nmb) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m == 0) {
+    *reinterpret_cast<unsigned long long*>(g_noalloc_scratch) = 0x7FF0000000000000ull;        // +inf: identity of the min
+    *reinterpret_cast<unsigned long long*>(g_noalloc_scratch + 16) = 0ull;
+  }
+  if (m < nmb) reinterpret_cast<int4*>(g_noalloc_scratch + 256)[m] = make_int4(0, 0, 0, 0);
+}
+}  // namespace ak
+
+extern "C" int ak_new_dt_noalloc(const void* u, int nmb, int nx1, int nx2, int nx3, int ng, double gamma,
+                                 double dx1, double dx2, double dx3, double cfl, void* cuda_stream, double* dt_out) {
+  using namespace ak;
+  if (!u || !dt_out) return set_error(-1, "ak_new_dt_noalloc: null pointer");
+  if (nmb < 1 || nx1 < 1 || nx2 < 1 || nx3 < 1 || ng < 0 || ng > 4) return set_error(-1, "ak_new_dt_noalloc: bad pack shape");
+  if (!(gamma > 1.0) || !(cfl > 0.0) || !(dx1 > 0.0) || !(dx2 > 0.0) || !(dx3 > 0.0))
+    return set_error(-1, "ak_new_dt_noalloc: gamma must exceed 1; cfl and the cell sizes must be positive");
+  if (nmb > AK_NOALLOC_MAX_BLOCKS)
+    return set_error(-3, "ak_new_dt_noalloc: more than 8176 MeshBlocks do not fit the library's 128 KiB static scratch array "
+                         "(use ak_new_dt on a pack with caller-allocated scratch)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // the device that owns u runs the kernels (no allocation: attribute queries and cudaSetDevice only)
+  cudaPointerAttributes pa;
+  cudaError_t e = cudaPointerGetAttributes(&pa, u);
+  if (e != cudaSuccess) return set_error(-4, cudaGetErrorString(e));
+  if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) return set_error(-1, "ak_new_dt_noalloc: u is not a device pointer");
+  if (pa.device < 0 || pa.device >= 64) return set_error(-3, "ak_new_dt_noalloc: device ordinal beyond 63");
+  int prev = -1;
+  if (cudaGetDevice(&prev) != cudaSuccess) return set_error(-4, "ak_new_dt_noalloc: cudaGetDevice failed");
+  if (prev != pa.device && cudaSetDevice(pa.device) != cudaSuccess) return set_error(-4, "ak_new_dt_noalloc: cudaSetDevice failed");
+  int rc = 0;
+  do {
+    // device address of the static array: once per device, with that device current
+    static unsigned char* scratch_of_device[64] = {};
+    unsigned char* s = scratch_of_device[pa.device];
+    if (!s) {
+      e = cudaGetSymbolAddress((void**)&s, g_noalloc_scratch);
+      if (e != cudaSuccess || !s) { rc = set_error(-4, "ak_new_dt_noalloc: cudaGetSymbolAddress failed"); break; }
+      scratch_of_device[pa.device] = s;
+    }
+    PackDev P{};
+    P.nmb = nmb; P.ng = ng; P.gamma = gamma; P.max_level = 0;
+    P.nx[0] = nx1; P.nx[1] = nx2; P.nx[2] = nx3;
+    for (int d = 0; d < 3; d++) { P.nt[d] = P.nx[d] + 2 * ng; P.nrb[d] = 1; }
+    P.ncell = (long long)P.nt[0] * P.nt[1] * P.nt[2];
+    P.dx0[0] = dx1; P.dx0[1] = dx2; P.dx0[2] = dx3;
+    P.dtmin_bits = (unsigned long long*)s;
+    P.floor_cnt = (unsigned long long*)(s + 8);
+    P.nonfinite = (unsigned long long*)(s + 16);
+    P.blk = (const int4*)(s + 256);
+    noalloc_setup_kernel<<<(nmb + 255) / 256, 256, 0, st>>>(nmb);
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, pa.device);
+    const int rpw = P.nx[0] <= 16 ? 32 / P.nx[0] : 1;                       // (as in launch_new_dt)
+    const long long nrows = (long long)P.nmb * ((P.nx[1] + rpw - 1) / rpw) * P.nx[2];
+    const long long want = (nrows + 7) / 8;
+    const int grid = (int)(want < (long long)sms * 8 ? want : (long long)sms * 8);
+    new_dt_kernel<<<grid, 256, 0, st>>>(P, (const double*)u, nrows);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) { rc = set_error(-4, cudaGetErrorString(e)); break; }
+    unsigned long long cells[3];
+    e = cudaMemcpyAsync(cells, s, 24, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { rc = set_error(-4, cudaGetErrorString(e)); break; }
+    double dtmin;
+    memcpy(&dtmin, &cells[0], 8);
+    if (cells[2] || !(dtmin > 0.0) || !(dtmin < __builtin_huge_val())) {
+      rc = set_error(-5, "non-finite signal speed in the state (NaN or inf in an active cell)"); break;
+    }
+    *dt_out = cfl * dtmin;
+  } while (0);
+  if (prev != pa.device) cudaSetDevice(prev);
+  return rc;
+}

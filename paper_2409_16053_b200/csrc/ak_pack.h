@@ -77,6 +77,8 @@ struct ak_pack {
 };
 
 namespace ak {
+// records the message ak_last_error() returns (thread-local, ak_api.cu) and hands `code` back
+int set_error(int code, const char* msg);
 // launchers implemented in the .cu translation units; return cudaGetLastError()
 cudaError_t launch_fill_ghosts(const ak_pack& p, double* U);
 cudaError_t launch_new_dt(const ak_pack& p, const double* U);       // leaves the min in dtmin_bits
