@@ -189,7 +189,20 @@ __global__ void __launch_bounds__(256) fill_ghosts_flat_kernel(PackDev P, double
     i = ii < ng ? ii : ii + P.nx[0];
   }
   double val[5];
-  ghost_general(P, U, m, i, j, k, val);
+  // fast path: where the same-level neighbour table names a block, the ghost cell is a plain copy of the cell one block
+  // length away (no leaf-map lookups, no wrapping); only cells next to another level take the general path
+  const int d1 = (i < ng) ? -1 : (i >= P.nx[0] + ng ? 1 : 0);
+  const int d2 = (j < ng) ? -1 : (j >= P.nx[1] + ng ? 1 : 0);
+  const int d3 = (k < ng) ? -1 : (k >= P.nx[2] + ng ? 1 : 0);
+  const int src = P.nbr[27 * m + (d3 + 1) * 9 + (d2 + 1) * 3 + (d1 + 1)];
+  if (src >= 0) {
+    const double* q = U + (long long)src * 5 * P.ncell +
+                      ((long long)(k - d3 * P.nx[2]) * n2 + (j - d2 * P.nx[1])) * n1 + (i - d1 * P.nx[0]);
+#pragma unroll
+    for (int n = 0; n < 5; n++) val[n] = q[n * P.ncell];
+  } else {
+    ghost_general(P, U, m, i, j, k, val);
+  }
   const long long o = (long long)m * 5 * P.ncell + ((long long)k * n2 + j) * n1 + i;
   for (int n = 0; n < 5; n++) U[o + n * P.ncell] = val[n];
 }
