@@ -304,3 +304,53 @@ def table1() -> Workload:
     """Shape of the paper's Table 1 GPU workload: 512x256x256 in 128^3 blocks, linear wave."""
     return Workload("table1_soundwave_16x128", uniform_mesh((4, 2, 2), (128, 128, 128), 2), RECON_PLM, 10,
                     sound_wave_prim())
+
+
+# --------------------------------------------------------------------------------------------
+# MHD states (SURVEY 8(f) row f4): 8 variables per cell, the last three the face-centred field
+# --------------------------------------------------------------------------------------------
+def make_state_mhd(mesh: Mesh, prim_fn: PrimFn, A_fn, B0=(0.0, 0.0, 0.0), gamma: float = GAMMA, device="cpu") -> torch.Tensor:
+    """U[m][8][k][j][i] = (rho, rho v, E, b1, b2, b3) with b_d the area-averaged field on the LOWER d-face of each cell
+    ("area-averages on cell-faces").  The faces come from a vector potential evaluated on the cell EDGES,
+    b = curl A by Stokes' theorem, plus a uniform field B0, so that the discrete divergence vanishes to round-off;
+    A_fn(x1, x2, x3) -> (A1, A2, A3) at arbitrary points.  E = P/(gamma-1) + rho v^2/2 + B^2/2 with the
+    cell-centred B the mean of the two faces.  Faces are set on the active cells and on the first ghost layer above them
+    (the upper face of the last active cell); ghost cells otherwise stay zero (the ghost fill writes them)."""
+    n1, n2, n3 = mesh.nx
+    ng = mesh.ng
+    U = torch.zeros((mesh.nmb, 8) + tuple(mesh.state_shape()[2:]), dtype=torch.float64, device=device)
+    for m in range(mesh.nmb):
+        level, *lx = mesh.blocks[m]
+        dx = mesh.dx(level)
+        xc = mesh.centres(m, device)                                   # cell centres of the active cells
+        # face / edge coordinates: nx+1 lower-face positions per direction
+        xf = [mesh.xmin[d] + (torch.arange(mesh.nx[d] + 1, dtype=torch.float64, device=device) + float(lx[d] * mesh.nx[d])) * dx[d]
+              for d in range(3)]
+
+        def grid(a1, a2, a3):
+            return a1[None, None, :], a2[None, :, None], a3[:, None, None]
+
+        def A(comp, a1, a2, a3):
+            X1, X2, X3 = grid(a1, a2, a3)
+            return torch.broadcast_to(torch.as_tensor(A_fn(X1, X2, X3)[comp], dtype=torch.float64, device=device),
+                                      (a3.numel(), a2.numel(), a1.numel()))
+        # b1 on x1-faces (x1f, x2c, x3c): dA3/dx2 - dA2/dx3, differences of edge values over the face
+        A3 = A(2, xf[0], xf[1], xc[2]); A2 = A(1, xf[0], xc[1], xf[2])
+        b1 = (A3[:, 1:, :] - A3[:, :-1, :]) / dx[1] - (A2[1:, :, :] - A2[:-1, :, :]) / dx[2] + B0[0]
+        # b2 on x2-faces (x1c, x2f, x3c): dA1/dx3 - dA3/dx1
+        A1 = A(0, xc[0], xf[1], xf[2]); A3 = A(2, xf[0], xf[1], xc[2])
+        b2 = (A1[1:, :, :] - A1[:-1, :, :]) / dx[2] - (A3[:, :, 1:] - A3[:, :, :-1]) / dx[0] + B0[1]
+        # b3 on x3-faces (x1c, x2c, x3f): dA2/dx1 - dA1/dx2
+        A2 = A(1, xf[0], xc[1], xf[2]); A1 = A(0, xc[0], xf[1], xf[2])
+        b3 = (A2[:, :, 1:] - A2[:, :, :-1]) / dx[0] - (A1[:, 1:, :] - A1[:, :-1, :]) / dx[1] + B0[2]
+        U[m, 5, ng:ng + n3, ng:ng + n2, ng:ng + n1 + 1] = b1
+        U[m, 6, ng:ng + n3, ng:ng + n2 + 1, ng:ng + n1] = b2
+        U[m, 7, ng:ng + n3 + 1, ng:ng + n2, ng:ng + n1] = b3
+        X1, X2, X3 = grid(*xc)
+        rho, v1, v2, v3, P = (torch.broadcast_to(torch.as_tensor(q, dtype=torch.float64, device=device), (n3, n2, n1))
+                              for q in prim_fn(X1, X2, X3))
+        bc1 = 0.5 * (b1[:, :, 1:] + b1[:, :, :-1]); bc2 = 0.5 * (b2[:, 1:, :] + b2[:, :-1, :]); bc3 = 0.5 * (b3[1:, :, :] + b3[:-1, :, :])
+        act = U[m, :, ng:ng + n3, ng:ng + n2, ng:ng + n1]
+        act[0] = rho; act[1] = rho * v1; act[2] = rho * v2; act[3] = rho * v3
+        act[4] = P / (gamma - 1.0) + 0.5 * rho * (v1 * v1 + v2 * v2 + v3 * v3) + 0.5 * (bc1 * bc1 + bc2 * bc2 + bc3 * bc3)
+    return U

@@ -1,0 +1,278 @@
+"""Pins for the MHD + constrained-transport oracle (oracle/orc_mhd.cpp; paper P:116).
+
+Nothing here compares the oracle with itself:
+  * HLLD: consistency with the physical flux of Eq.(5), mirror symmetry, a stationary contact across which the density jumps
+    while the field threads it, supersonic upwinding;
+  * the hydrodynamic limit: with B = 0 the Sod tube converges to the exact Riemann solution (solver in test_oracle_scheme);
+  * div B = 0 to round-off, conservation of mass, momentum, energy and of the mean field, on a 3-D multi-block periodic mesh
+    with a field from a vector potential;
+  * a uniform magnetised state in motion is preserved bit for bit;
+  * a plane-parallel problem (Brio-Wu states) stays plane-parallel bit for bit, and run along x2 or x3 it matches x1;
+  * "For PPM4 and PLM reconstruction, all waves converge at second-order" -- fast, Alfven and slow waves whose
+    eigenvectors are computed here numerically from the primitive-variable Jacobian of Eq.(5).
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2409_16053_b200 import inputs as I
+
+G53 = 5.0 / 3.0
+
+
+@pytest.fixture(scope="module")
+def om():
+    from oracle import orc_mhd
+    orc_mhd.build()
+    return orc_mhd
+
+
+def phys_flux(g, bx, W):
+    r, u, v, w, e, by, bz = W
+    p = (g - 1) * e
+    b2 = bx * bx + by * by + bz * bz
+    pt = p + 0.5 * b2
+    E = e + 0.5 * r * (u * u + v * v + w * w) + 0.5 * b2
+    vb = u * bx + v * by + w * bz
+    return np.array([r * u, r * u * u + pt - bx * bx, r * u * v - bx * by, r * u * w - bx * bz, (E + pt) * u - bx * vb,
+                     by * u - bx * v, bz * u - bx * w])
+
+
+def rand_state(rng):
+    return [10 ** rng.uniform(-1, 1), *rng.normal(size=3), 10 ** rng.uniform(-1, 1), *rng.normal(size=2)]
+
+
+# ---------------------------------------------------------------- HLLD -----------------------------
+def test_hlld_consistency(om):
+    rng = np.random.default_rng(1)
+    for _ in range(300):
+        W, bx = rand_state(rng), rng.normal() * rng.integers(0, 2)        # (half of the cases with Bx = 0)
+        F, Fx = om.hlld(G53, bx, W, W), phys_flux(G53, bx, W)
+        assert np.abs(F - Fx).max() <= 1e-13 * (np.abs(Fx).max() + 1.0)
+
+
+def test_hlld_mirror_symmetry(om):
+    # x -> -x together with B -> -B (an invariance of Eq.(5)): L <-> R, u -> -u, Bx -> -Bx, transverse components unchanged;
+    # then every flux component but the normal momentum changes sign
+    rng = np.random.default_rng(2)
+    sign = np.array([-1.0, 1.0, -1.0, -1.0, -1.0, -1.0, -1.0])
+    for _ in range(300):
+        WL, WR, bx = rand_state(rng), rand_state(rng), rng.normal()
+        F = om.hlld(G53, bx, WL, WR)
+        ML, MR = list(WR), list(WL)
+        ML[1], MR[1] = -ML[1], -MR[1]
+        Fm = om.hlld(G53, -bx, ML, MR)
+        assert np.abs(Fm - sign * F).max() <= 1e-12 * (np.abs(F).max() + 1.0)
+
+
+def test_hlld_keeps_a_stationary_contact_and_upwinds_supersonic_flow(om):
+    # density jumps, everything else continuous, gas at rest, field threading the contact: only the stresses remain
+    bx, by, bz, ug = 0.8, -0.6, 0.3, 1.5
+    WL, WR = [1.0, 0, 0, 0, ug, by, bz], [0.1, 0, 0, 0, ug, by, bz]
+    F = om.hlld(G53, bx, WL, WR)
+    pt = (G53 - 1) * ug + 0.5 * (bx * bx + by * by + bz * bz)
+    np.testing.assert_allclose(F, [0.0, pt - bx * bx, -bx * by, -bx * bz, 0.0, 0.0, 0.0], atol=1e-15)
+    assert F[0] == 0.0
+    # faster than the fast speed to the right / left: the upwind physical flux
+    rng = np.random.default_rng(3)
+    WL, WR = rand_state(rng), rand_state(rng)
+    WL[1], WR[1] = 30.0, 31.0
+    np.testing.assert_allclose(om.hlld(G53, 0.7, WL, WR), phys_flux(G53, 0.7, WL), rtol=1e-14)
+    WL[1], WR[1] = -31.0, -30.0
+    np.testing.assert_allclose(om.hlld(G53, 0.7, WL, WR), phys_flux(G53, 0.7, WR), rtol=1e-14)
+
+
+# ---------------------------------------------------------------- helpers --------------------------
+ZERO_A = lambda X1, X2, X3: (0 * X1 + 0 * X2 + 0 * X3,) * 3
+
+
+def act(mesh):
+    g = mesh.ng
+    return (slice(None), slice(None), slice(g, -g), slice(g, -g), slice(g, -g))
+
+
+def divb(mesh, U):
+    g, (n1, n2, n3) = mesh.ng, mesh.nx
+    dx = mesh.dx(0)
+    b1, b2, b3 = U[:, 5], U[:, 6], U[:, 7]
+    s = (slice(None), slice(g, g + n3), slice(g, g + n2), slice(g, g + n1))
+    up1 = (slice(None), slice(g, g + n3), slice(g, g + n2), slice(g + 1, g + n1 + 1))
+    up2 = (slice(None), slice(g, g + n3), slice(g + 1, g + n2 + 1), slice(g, g + n1))
+    up3 = (slice(None), slice(g + 1, g + n3 + 1), slice(g, g + n2), slice(g, g + n1))
+    return (b1[up1] - b1[s]) / dx[0] + (b2[up2] - b2[s]) / dx[1] + (b3[up3] - b3[s]) / dx[2]
+
+
+def run(om, mesh, U0, gamma=G53, cfl=0.3, nsteps=None, tend=None, threads=4):
+    p = om.OrcMhdPack(mesh, gamma, threads=threads)
+    p.load(U0)
+    t, n = 0.0, 0
+    while (nsteps is None or n < nsteps) and (tend is None or t < tend):
+        dt = p.new_dt(cfl)
+        if tend is not None and t + dt > tend:
+            dt = tend - t
+        p.step(cfl, dt)
+        t += dt
+        n += 1
+    assert p.floor_count() == 0
+    p.fill_ghosts()
+    out = p.current().copy()
+    p.close()
+    return out
+
+
+def tri(x):
+    """Periodic triangle wave with slope +1 on [0.25, 0.75) and -1 elsewhere: the integral of the double Brio-Wu field."""
+    x = x - torch.floor(x)
+    return torch.where((x >= 0.25) & (x < 0.75), x - 0.5, torch.where(x < 0.25, -x, 1.0 - x))
+
+
+def brio_wu(N, d, ng=3):
+    """Two mirrored Brio-Wu problems on a periodic line along direction d (left state on [0.25, 0.75)), gamma = 2."""
+    nx = [4, 4, 4]
+    nx[d] = N
+    mesh = I.uniform_mesh((1, 1, 1), tuple(nx), ng)
+    d2 = (d + 2) % 3
+
+    def prim(X1, X2, X3):
+        x = (X1, X2, X3)[d] + 0 * X1 + 0 * X2 + 0 * X3
+        inside = (x >= 0.25) & (x < 0.75)
+        z = torch.zeros_like(x)
+        return (torch.where(inside, 1.0, 0.125).to(torch.float64), z, z, z, torch.where(inside, 1.0, 0.1).to(torch.float64))
+
+    def A(X1, X2, X3):
+        x = (X1, X2, X3)[d] + 0 * X1 + 0 * X2 + 0 * X3
+        out = [torch.zeros_like(x)] * 3
+        out[d2] = -tri(x)                                   # B_{d+1} = -dA_{d+2}/dx_d = +1 inside, -1 outside
+        return tuple(out)
+
+    B0 = [0.0, 0.0, 0.0]
+    B0[d] = 0.75
+    return mesh, I.make_state_mhd(mesh, prim, A, tuple(B0), gamma=2.0).numpy()
+
+
+# ---------------------------------------------------------------- scheme ---------------------------
+def test_hydrodynamic_limit_sod_against_the_exact_solution(om):
+    from tests.test_oracle_scheme import exact_riemann, sod_sample
+    g = 1.4
+    ps, us = exact_riemann(g, 1.0, 0.0, 1.0, 0.125, 0.0, 0.1)
+    errs = {}
+    for N in (128, 256):
+        mesh = I.uniform_mesh((1, 1, 1), (N, 4, 4), 3)
+
+        def prim(X1, X2, X3):
+            x = X1 + 0 * X2 + 0 * X3
+            inside = (x >= 0.25) & (x < 0.75)
+            z = torch.zeros_like(x)
+            return (torch.where(inside, 1.0, 0.125).to(torch.float64), z, z, z, torch.where(inside, 1.0, 0.1).to(torch.float64))
+
+        U0 = I.make_state_mhd(mesh, prim, ZERO_A, gamma=g).numpy()
+        U = run(om, mesh, U0, gamma=g, tend=0.1)
+        prof = U[0, :, 3, 3, 3:-3]
+        x = (np.arange(N) + 0.5) / N
+        right = x >= 0.5
+        rho_ex, _ = sod_sample(g, (x[right] - 0.75) / 0.1, ps, us)
+        errs[N] = np.abs(prof[0, right] - rho_ex).mean()
+        assert np.all(U[:, 5:] == 0.0)                                     # no field is generated
+        assert np.abs(prof[0] - prof[0, ::-1]).max() <= 1e-13              # the two halves mirror each other
+    assert errs[256] < 5e-3 and 0.7 <= math.log2(errs[128] / errs[256]) <= 1.15, errs
+
+
+def test_divb_conservation_and_mean_field_on_a_multiblock_mesh(om):
+    mesh = I.uniform_mesh((2, 2, 1), (8, 6, 10), 3)
+    k = 2 * math.pi
+
+    def A(X1, X2, X3):
+        return (0.1 * torch.sin(k * X2) * torch.cos(k * X3) + 0 * X1, 0.1 * torch.sin(k * X3 + 0.3) * torch.cos(k * X1) + 0 * X2,
+                0.1 * torch.cos(k * X1 + 0.7) * torch.sin(k * X2) + 0 * X3)
+
+    prim = lambda X1, X2, X3: (1.0 + 0.2 * torch.sin(k * X1) * torch.cos(k * X2) + 0 * X3, 0.3 * torch.sin(k * X2) + 0 * X1 + 0 * X3,
+                               -0.2 * torch.cos(k * X3) + 0 * X1 + 0 * X2, 0.1 * torch.sin(k * X1 + 1.0) + 0 * X2 + 0 * X3,
+                               0.6 + 0 * X1 + 0 * X2 + 0 * X3)
+    U0 = I.make_state_mhd(mesh, prim, A, (0.3, -0.2, 0.1)).numpy()
+    assert np.abs(divb(mesh, U0)).max() <= 1e-13
+    U = run(om, mesh, U0, nsteps=6)
+    assert np.abs(divb(mesh, U)).max() <= 2e-13                            # (|B|/dx ~ 10: a few ulp of that)
+    a = act(mesh)
+    for n in range(8):                                                    # mass, momentum, energy and the mean field
+        t0, t1 = U0[a][:, n].sum(), U[a][:, n].sum()
+        scale = np.abs(U0[a][:, n]).sum() + 1.0
+        assert abs(t1 - t0) <= 1e-13 * scale, (n, t0, t1)
+    assert np.abs(U[a] - U0[a]).max() > 1e-3                               # (something happened)
+
+
+def test_uniform_magnetised_state_is_preserved_bit_exactly(om):
+    mesh = I.uniform_mesh((2, 1, 2), (6, 8, 4), 3)
+    prim = lambda X1, X2, X3: (1.3 + 0 * X1 + 0 * X2 + 0 * X3, 0.4 + 0 * X1 + 0 * X2 + 0 * X3, -0.7 + 0 * X1 + 0 * X2 + 0 * X3,
+                               0.2 + 0 * X1 + 0 * X2 + 0 * X3, 0.9 + 0 * X1 + 0 * X2 + 0 * X3)
+    U0 = I.make_state_mhd(mesh, prim, ZERO_A, (0.5, -0.3, 0.8)).numpy()
+    U = run(om, mesh, U0, nsteps=2)
+    a = act(mesh)
+    assert np.array_equal(U[a], U0[a])
+
+
+def test_plane_parallel_brio_wu_stays_plane_parallel_and_is_direction_independent(om):
+    profs = []
+    for d in range(3):
+        mesh, U0 = brio_wu(64, d)
+        U = run(om, mesh, U0, gamma=2.0, tend=0.05)
+        A = U[0][:, 3:-3, 3:-3, 3:-3]                                       # (n, k, j, i)
+        line = np.moveaxis(A, 3 - d, 1)                                     # (n, along, t, t)
+        assert np.array_equal(line, np.broadcast_to(line[:, :, :1, :1], line.shape))       # transverse planes identical
+        prof = line[:, :, 0, 0]
+        d1, d2 = (d + 1) % 3, (d + 2) % 3
+        profs.append(prof[[0, 1 + d, 1 + d1, 1 + d2, 4, 5 + d, 5 + d1, 5 + d2]])            # rotated into the x1 frame
+        assert np.all(prof[5 + d] == 0.75)                                  # the normal field of a 1-D problem never changes
+        assert np.abs(prof[0] - prof[0, ::-1]).max() <= 1e-13 and prof[0].min() > 0.1 and prof[0].max() <= 1.0 + 1e-12
+    for p in profs[1:]:
+        assert np.abs(p - profs[0]).max() <= 1e-13
+    # the compound structure has formed: the tangential field has changed sign across the fan and v_x > 0.3 somewhere
+    assert (profs[0][1] / profs[0][0]).max() > 0.3 and profs[0][6].min() < -0.9 and profs[0][6].max() > 0.9
+
+
+# ---------------------------------------------------------------- linear waves -------------
+def mhd_eigenmode(family):
+    """Right-going eigenvector of the primitive Jacobian d(rho, u, v, w, p, By, Bz)/dt + A d/dx = 0 of Eq.(5) about the
+    Gardiner-Stone background (rho = 1, p = 1/gamma, B = (1, sqrt 2, 1/2), at rest): speeds 2, 1, 1/2."""
+    g, r, p, bx, by, bz = G53, 1.0, 1.0 / G53, 1.0, math.sqrt(2.0), 0.5
+    A = np.zeros((7, 7))
+    A[0, 1] = r
+    A[1, 4], A[1, 5], A[1, 6] = 1 / r, by / r, bz / r
+    A[2, 5] = -bx / r
+    A[3, 6] = -bx / r
+    A[4, 1] = g * p
+    A[5, 1], A[5, 2] = by, -bx
+    A[6, 1], A[6, 3] = bz, -bx
+    lam, R = np.linalg.eig(A)
+    speed = {"fast": 2.0, "alfven": 1.0, "slow": 0.5}[family]
+    k = int(np.argmin(np.abs(lam - speed)))
+    assert abs(lam[k].real - speed) < 1e-12 and abs(lam[k].imag) < 1e-12
+    v = R[:, k].real
+    return speed, v / np.abs(v).max(), (r, p, bx, by, bz)
+
+
+def wave_error(om, family, N, amp=1e-6):
+    speed, R, (r0, p0, bx, by0, bz0) = mhd_eigenmode(family)
+    mesh = I.uniform_mesh((1, 1, 1), (N, 4, 4), 3)
+    k = 2 * math.pi
+
+    def prim(X1, X2, X3):
+        s = torch.sin(k * X1) + 0 * X2 + 0 * X3
+        return (r0 + amp * R[0] * s, amp * R[1] * s, amp * R[2] * s, amp * R[3] * s, p0 + amp * R[4] * s)
+
+    def A(X1, X2, X3):                                   # dBy = -dA3/dx1, dBz = +dA2/dx1
+        c = torch.cos(k * X1) / k + 0 * X2 + 0 * X3
+        return (0 * c, -amp * R[6] * c, amp * R[5] * c)
+
+    U0 = I.make_state_mhd(mesh, prim, A, (bx, by0, bz0)).numpy()
+    U = run(om, mesh, U0, tend=1.0 / speed)
+    a = act(mesh)
+    return math.sqrt(sum(np.abs(U[a][0, n] - U0[a][0, n]).mean() ** 2 for n in range(8)))
+
+
+@pytest.mark.parametrize("family", ["fast", "alfven", "slow"])
+def test_linear_mhd_waves_converge_at_second_order(om, family):
+    e = {N: wave_error(om, family, N) for N in (16, 32, 64)}
+    assert e[64] < e[32] < e[16] < 1e-6
+    assert 3.0 <= e[32] / e[64] <= 5.0, (family, e)
