@@ -1,0 +1,57 @@
+/* ak_mhd.h -- C-ABI boundary of the MHD + constrained-transport stage, first cut.
+ *
+ * Newtonian ideal MHD, paper Eq.(5) with the gamma-law energy E = p_g/(gamma-1) + rho v^2/2 + B^2/2 (/root/reference/PAPER.md
+ * lines 146-150, cited as P:NN), on a MeshBlockPack resident in device memory.  "The magnetic field is discretized
+ * as area-averages on cell-faces, and the constrained transport (CT) algorithm of Evans & Hawley (1988) is used to preserve the
+ * divergence-free constraint with upwinded electric fields calculated using the method of Gardiner & Stone (2005, 2008)"
+ * (P:116); HLLD Riemann solver.  Readings: DESIGN.md Q33-Q37.  Scope of this cut: uniform single-level periodic packs,
+ * PLM (van Leer) reconstruction, HLLD, SSPRK(2,2); the kernels are not fused (face fluxes and corner EMFs pass through a
+ * caller-owned work buffer in device memory).
+ *
+ * One step:   akm_new_dt(p, cfl, &dt);  for stage in 1, 2: { akm_fill_ghosts(p); akm_stage(p, stage, dt); }
+ *
+ * State layout: U[m][n][k][j][i], n = 0..7 = (rho, rho v1, rho v2, rho v3, E, b1, b2, b3), i fastest, fp64, ng >= 3 ghost
+ * layers included; b_d of cell (k,j,i) is the field on the LOWER d-face of that cell.  Memory is caller-owned (device
+ * pointers, 256-byte aligned); the descriptor is a small host object.  All functions are host functions; int results are
+ * AK-style codes: 0 ok, -1 bad argument, -2 call order, -3 unsupported, -4 CUDA error, -5 non-finite state;
+ * akm_last_error() returns a thread-local message.  No CPU fallback exists.
+ */
+#ifndef AK_MHD_H
+#define AK_MHD_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct akm_pack akm_pack;
+
+/* nrb1 x nrb2 x nrb3 root blocks of nx1 x nx2 x nx3 cells on the periodic box [xmin, xmax) (HOST arrays of 3);
+ * lx[3 m + d] (HOST) = logical location of block m; nmb = nrb1 nrb2 nrb3.  NULL on invalid arguments. */
+akm_pack* akm_pack_create(int nmb, int nx1, int nx2, int nx3, int ng, double gamma, int nrb1, int nrb2, int nrb3,
+                          const int* lx, const double* xmin, const double* xmax);
+size_t akm_pack_state_bytes(const akm_pack*);   /* one state buffer: nmb * 8 * (nx1+2ng)(nx2+2ng)(nx3+2ng) * 8 bytes */
+size_t akm_pack_work_bytes(const akm_pack*);    /* work buffer: primitives, face fluxes, corner EMFs, tables          */
+/* u_a holds U^n (ghost cells arbitrary) and becomes current; u_b is the second register; work the work buffer; all DEVICE
+ * pointers, pairwise disjoint; cuda_stream a cudaStream_t (NULL = legacy stream) on which every kernel is launched. */
+int akm_pack_bind(akm_pack*, void* u_a, void* u_b, void* work, void* cuda_stream);
+/* Periodic copy of all 8 variables into the ghost cells of the current buffer; bit-exact.  Asynchronous. */
+int akm_fill_ghosts(akm_pack*);
+/* One SSPRK(2,2) stage (stage 1: A -> B; stage 2: B and A -> A): primitives, PLM + HLLD in x1, x2, x3, corner EMFs, flux
+ * divergence for the cells and curl of the EMFs for the faces (div B is preserved to round-off).  Needs akm_fill_ghosts
+ * on the current buffer first (-2 otherwise).  Asynchronous. */
+int akm_stage(akm_pack*, int stage, double dt);
+/* cfl * min over active cells and d of dx_d / (|v_d| + c_fast,d) (Eq.(3), with the fast magnetosonic speed);
+ * dt_out is a HOST pointer; synchronises the stream; -5 for a NaN / inf state. */
+int akm_new_dt(akm_pack*, double cfl, double* dt_out);
+/* akm_new_dt (unless dt_fixed > 0), then the two (fill, stage) pairs; dt_out (HOST, may be NULL) receives the step taken. */
+int akm_step(akm_pack*, double cfl, double dt_fixed, double* dt_out);
+void* akm_pack_current(const akm_pack*);        /* device pointer of the buffer holding the latest state             */
+long long akm_pack_floor_count(akm_pack*);      /* floor activations since bind (synchronises); negative on error    */
+long long akm_pack_launch_count(const akm_pack*);
+int akm_pack_destroy(akm_pack*);
+const char* akm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

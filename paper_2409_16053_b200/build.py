@@ -22,11 +22,14 @@ UNITS = {                      # translation unit -> extra flags
     "ak_api.cu": [],
     "ak_exact.cu": ["-fmad=false"],
     "ak_stage.cu": ["-fmad=false", "-Xptxas", "-v"],
+    "mhd/ak_mhd.cu": ["-fmad=false", "-Xptxas", "-v"],        # MHD + CT (include/ak_mhd.h)
 }
 
 
 def _sources():
-    return [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(INCLUDE, "ak.h")]
+    src = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if os.path.isfile(os.path.join(CSRC, f))]
+    src += [os.path.join(CSRC, "mhd", f) for f in os.listdir(os.path.join(CSRC, "mhd"))]
+    return src + [os.path.join(INCLUDE, "ak.h"), os.path.join(INCLUDE, "ak_mhd.h")]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -37,14 +40,14 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(bdir, exist_ok=True)
     objs = []
     for unit, extra in UNITS.items():
-        obj = os.path.join(bdir, unit.replace(".cu", ".o"))
+        obj = os.path.join(bdir, os.path.basename(unit).replace(".cu", ".o"))
         cmd = [nvcc, *ARCH, *COMMON, *extra, "-c", os.path.join(CSRC, unit), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or r.returncode:
             sys.stderr.write(r.stdout + r.stderr)
         if r.returncode:
             raise RuntimeError(f"nvcc failed on {unit}")
-        with open(os.path.join(bdir, unit + ".log"), "w") as f:
+        with open(os.path.join(bdir, os.path.basename(unit) + ".log"), "w") as f:
             f.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
         objs.append(obj)
     subprocess.run([nvcc, *ARCH, "-shared", "-o", SO, *objs], check=True)

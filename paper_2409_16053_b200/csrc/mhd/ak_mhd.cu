@@ -1,0 +1,504 @@
+// ak_mhd.cu -- MHD + constrained-transport stage over a MeshBlockPack (include/ak_mhd.h), first cut:
+// correct and device-resident, not yet fused.  Paper: Eq.(5) and the gamma-law energy, face-centred field with
+// CT and Gardiner-Stone upwinded EMFs, HLLD.  Readings DESIGN.md Q33-Q37.
+// Compiled with -fmad=false and IEEE division / sqrt: every expression rounds once per operation in the order written,
+// because the sign of a mass flux decides which side a corner EMF is upwinded from and a contracted product could flip it.
+// Kernels, all one thread per cell with i fastest (coalesced), launched in this order per stage:
+//   prim_kernel      U -> W = (rho, v, u_g, B_cc)                                   work: W[8]
+//   flux_kernel<D>   PLM on W along D, HLLD at the lower D-face of every cell        work: F_D[7]
+//   emf_kernel       corner EMFs from the face fluxes, upwinded                     work: Ec[3]
+//   update_kernel    cells: flux divergence; faces: curl of the corner EMFs; stage weights
+// plus fill_kernel (periodic ghost copy of all 8 variables) and dt_kernel (CFL reduction with the fast speed).
+// This file is part of the CUDA path only; the CPU oracle of the tests shares nothing with it.
+#include "ak_mhd.h"
+
+#include <cuda_runtime.h>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <string>
+#include <vector>
+
+namespace {
+
+thread_local std::string g_err;
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+int cuda_fail(cudaError_t e, const char* where) { return fail(-4, std::string(where) + ": " + cudaGetErrorString(e)); }
+#define AKM_CUDA(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, where); } while (0)
+
+constexpr double RHO_FLOOR = 1e-20, P_FLOOR = 1e-20;
+
+// plain-data view of the pack for the kernels
+struct Dev {
+  int nmb, nx[3], ng, nt[3], nrb[3];
+  long long ncell;            // cells per block incl. ghosts = stride between variables
+  double gamma, dx[3];
+  const int* lx;              // [nmb][3]
+  const int* leaf;            // [nrb3][nrb2][nrb1] -> block
+  double* W;                  // [nmb][8][ncell]
+  double* F[3];               // [nmb][7][ncell] per direction: 0..4 hydro fluxes (unrotated), 5 = flux of B_{d+1}, 6 = of B_{d+2}
+  double* Ec;                 // [nmb][3][ncell] corner EMFs
+  unsigned long long* cells;  // [0] min dt as ordered bits, [1] floor count, [2] non-finite count
+};
+
+// ---- HLLD (Miyoshi & Kusano 2005, restated; Q34): rotated states (rho, u, v, w, u_g, By, Bz), normal field bx ----
+struct Side { double r, u, v, w, by, bz, pt, E, vb, cf, U[7], F[7]; };
+
+__device__ void side_init(double gamma, double bx, const double W[7], Side& s) {
+  s.r = W[0]; s.u = W[1]; s.v = W[2]; s.w = W[3]; s.by = W[5]; s.bz = W[6];
+  const double e = W[4], p = (gamma - 1.0) * e;
+  const double b2 = bx * bx + (s.by * s.by + s.bz * s.bz);
+  s.pt = p + 0.5 * b2;
+  s.E = e + 0.5 * s.r * (s.u * s.u + (s.v * s.v + s.w * s.w)) + 0.5 * b2;
+  s.vb = s.u * bx + (s.v * s.by + s.w * s.bz);
+  const double gp = gamma * p, sum = gp + b2;
+  double disc = sum * sum - 4.0 * gp * (bx * bx);
+  if (disc < 0.0) disc = 0.0;
+  s.cf = sqrt((sum + sqrt(disc)) / (2.0 * s.r));
+  s.U[0] = s.r; s.U[1] = s.r * s.u; s.U[2] = s.r * s.v; s.U[3] = s.r * s.w; s.U[4] = s.E; s.U[5] = s.by; s.U[6] = s.bz;
+  s.F[0] = s.r * s.u; s.F[1] = s.r * s.u * s.u + s.pt - bx * bx; s.F[2] = s.r * s.u * s.v - bx * s.by;
+  s.F[3] = s.r * s.u * s.w - bx * s.bz; s.F[4] = (s.E + s.pt) * s.u - bx * s.vb; s.F[5] = s.by * s.u - bx * s.v;
+  s.F[6] = s.bz * s.u - bx * s.w;
+}
+
+__device__ void star_state(double bx, const Side& s, double SK, double SM, double pts, double Us[7], double& vbs) {
+  const double sdu = SK - s.u, sdm = SK - SM;
+  const double rs = s.r * sdu / sdm;
+  const double den = s.r * sdu * sdm - bx * bx;
+  double vs, ws, bys, bzs;
+  if (fabs(den) < 1e-8 * pts) {
+    vs = s.v; ws = s.w; bys = s.by; bzs = s.bz;
+  } else {
+    const double f1 = bx * (SM - s.u) / den, f2 = (s.r * sdu * sdu - bx * bx) / den;
+    vs = s.v - s.by * f1; ws = s.w - s.bz * f1;
+    bys = s.by * f2; bzs = s.bz * f2;
+  }
+  vbs = SM * bx + (vs * bys + ws * bzs);
+  const double Es = (sdu * s.E - s.pt * s.u + pts * SM + bx * (s.vb - vbs)) / sdm;
+  Us[0] = rs; Us[1] = rs * SM; Us[2] = rs * vs; Us[3] = rs * ws; Us[4] = Es; Us[5] = bys; Us[6] = bzs;
+}
+
+__device__ void hlld(double gamma, double bn, const double WL[7], const double WR[7], double F[7]) {
+  Side L, R;
+  side_init(gamma, bn, WL, L);
+  side_init(gamma, bn, WR, R);
+  const double cfm = fmax(L.cf, R.cf);
+  const double SL = fmin(L.u, R.u) - cfm, SR = fmax(L.u, R.u) + cfm;
+  if (SL >= 0.0) { for (int n = 0; n < 7; n++) F[n] = L.F[n]; return; }
+  if (SR <= 0.0) { for (int n = 0; n < 7; n++) F[n] = R.F[n]; return; }
+  const double mL = L.r * (SL - L.u), mR = R.r * (SR - R.u);
+  const double SM = ((mR * R.u - mL * L.u) - (R.pt - L.pt)) / (mR - mL);
+  const double pts = ((mR * L.pt - mL * R.pt) + mL * mR * (R.u - L.u)) / (mR - mL);
+  double UsL[7], UsR[7], vbsL, vbsR;
+  star_state(bn, L, SL, SM, pts, UsL, vbsL);
+  star_state(bn, R, SR, SM, pts, UsR, vbsR);
+  const double sqL = sqrt(UsL[0]), sqR = sqrt(UsR[0]);
+  const double SsL = SM - fabs(bn) / sqL, SsR = SM + fabs(bn) / sqR;
+  const bool left = (SM >= 0.0);
+  const Side& K = left ? L : R;
+  const double* Us = left ? UsL : UsR;
+  const double SK = left ? SL : SR, SsK = left ? SsL : SsR;
+  const bool outer = left ? (SsL >= 0.0) : (SsR <= 0.0);
+  if (outer || 0.5 * bn * bn < 1e-8 * pts) {
+    for (int n = 0; n < 7; n++) F[n] = K.F[n] + SK * (Us[n] - K.U[n]);
+    return;
+  }
+  const double sgn = (bn > 0.0) ? 1.0 : -1.0, isum = 1.0 / (sqL + sqR);
+  const double vsL = UsL[2] / UsL[0], wsL = UsL[3] / UsL[0], vsR = UsR[2] / UsR[0], wsR = UsR[3] / UsR[0];
+  const double vss = (sqL * vsL + sqR * vsR + (UsR[5] - UsL[5]) * sgn) * isum;
+  const double wss = (sqL * wsL + sqR * wsR + (UsR[6] - UsL[6]) * sgn) * isum;
+  const double byss = (sqL * UsR[5] + sqR * UsL[5] + sqL * sqR * (vsR - vsL) * sgn) * isum;
+  const double bzss = (sqL * UsR[6] + sqR * UsL[6] + sqL * sqR * (wsR - wsL) * sgn) * isum;
+  const double vbss = SM * bn + (vss * byss + wss * bzss);
+  double Uss[7];
+  Uss[0] = Us[0]; Uss[1] = Us[1]; Uss[2] = Us[0] * vss; Uss[3] = Us[0] * wss;
+  Uss[4] = left ? UsL[4] - sqL * (vbsL - vbss) * sgn : UsR[4] + sqR * (vbsR - vbss) * sgn;
+  Uss[5] = byss; Uss[6] = bzss;
+  for (int n = 0; n < 7; n++) F[n] = K.F[n] + SsK * Uss[n] - (SsK - SK) * Us[n] - SK * K.U[n];
+}
+
+__device__ __forceinline__ void plm(double qm1, double q0, double qp1, double& qm, double& qp) {
+  const double dL = q0 - qm1, dR = qp1 - q0, prod = dL * dR;
+  const double h = (prod > 0.0) ? prod / (dL + dR) : 0.0;
+  qm = q0 - h; qp = q0 + h;
+}
+
+// (k, j, i) of a flat cell index inside one block
+__device__ __forceinline__ void kji(const Dev& P, long long c, int& k, int& j, int& i) {
+  i = (int)(c % P.nt[0]); j = (int)((c / P.nt[0]) % P.nt[1]); k = (int)(c / ((long long)P.nt[0] * P.nt[1]));
+}
+
+// ---- S1: primitives with the cell-centred field = mean of the two faces (Q33); not for the outermost upper layer ----
+__global__ void __launch_bounds__(256) prim_kernel(Dev P, const double* __restrict__ U) {
+  const int m = blockIdx.y;
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= P.ncell) return;
+  int k, j, i; kji(P, c, k, j, i);
+  if (i >= P.nt[0] - 1 || j >= P.nt[1] - 1 || k >= P.nt[2] - 1) return;
+  const long long nc = P.ncell, str[3] = {1, P.nt[0], (long long)P.nt[0] * P.nt[1]};
+  const double* Ub = U + (long long)m * 8 * nc;
+  int nfl = 0;
+  double rho = Ub[c];
+  if (!(rho >= RHO_FLOOR)) { rho = RHO_FLOOR; nfl++; }
+  const double rinv = 1.0 / rho, m1 = Ub[nc + c], m2 = Ub[2 * nc + c], m3 = Ub[3 * nc + c];
+  double B[3];
+  for (int d = 0; d < 3; d++) B[d] = 0.5 * (Ub[(5 + d) * nc + c] + Ub[(5 + d) * nc + c + str[d]]);
+  double ug = Ub[4 * nc + c] - 0.5 * rinv * (m1 * m1 + (m2 * m2 + m3 * m3)) - 0.5 * (B[0] * B[0] + (B[1] * B[1] + B[2] * B[2]));
+  if (!(ug >= P_FLOOR / (P.gamma - 1.0))) { ug = P_FLOOR / (P.gamma - 1.0); nfl++; }
+  double* Wb = P.W + (long long)m * 8 * nc;
+  Wb[c] = rho; Wb[nc + c] = m1 * rinv; Wb[2 * nc + c] = m2 * rinv; Wb[3 * nc + c] = m3 * rinv; Wb[4 * nc + c] = ug;
+  for (int d = 0; d < 3; d++) Wb[(5 + d) * nc + c] = B[d];
+  // (the oracle counts the floors of every cell it converts, ghosts included: so does this)
+  if (nfl) atomicAdd(P.cells + 1, (unsigned long long)nfl);
+}
+
+// ---- S2 + S3: PLM + HLLD at the lower D-face of every cell whose stencil exists ----
+template <int D>
+__global__ void __launch_bounds__(128) flux_kernel(Dev P, const double* __restrict__ U) {
+  constexpr int D1 = (D + 1) % 3, D2 = (D + 2) % 3;
+  const int m = blockIdx.y;
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= P.ncell) return;
+  int idx[3]; kji(P, c, idx[2], idx[1], idx[0]);
+  if (idx[D] < 2 || idx[D] >= P.nt[D] - 2 || idx[D1] >= P.nt[D1] - 1 || idx[D2] >= P.nt[D2] - 1) return;
+  const long long nc = P.ncell, str[3] = {1, P.nt[0], (long long)P.nt[0] * P.nt[1]};
+  const long long st = str[D], cm = c - st;
+  const double* Wb = P.W + (long long)m * 8 * nc;
+  const int var[7] = {0, 1 + D, 1 + D1, 1 + D2, 4, 5 + D1, 5 + D2};
+  double WL[7], WR[7], F[7];
+#pragma unroll
+  for (int q = 0; q < 7; q++) {
+    const double* w = Wb + var[q] * nc;
+    double qm, qp;
+    plm(w[cm - st], w[cm], w[cm + st], qm, qp); WL[q] = qp;
+    plm(w[c - st], w[c], w[c + st], qm, qp);    WR[q] = qm;
+  }
+  hlld(P.gamma, U[(long long)m * 8 * nc + (5 + D) * nc + c], WL, WR, F);
+  double* Fb = P.F[D] + (long long)m * 7 * nc;
+  Fb[c] = F[0]; Fb[(1 + D) * nc + c] = F[1]; Fb[(1 + D1) * nc + c] = F[2]; Fb[(1 + D2) * nc + c] = F[3];
+  Fb[4 * nc + c] = F[4]; Fb[5 * nc + c] = F[5]; Fb[6 * nc + c] = F[6];
+}
+
+// upwinded (face - centre) EMF difference: from the side the mass flux comes from; the mean where it vanishes (Q36)
+__device__ __forceinline__ double upwind(double mflux, double from_lower, double from_upper) {
+  if (mflux > 0.0) return from_lower;
+  if (mflux < 0.0) return from_upper;
+  return 0.5 * (from_lower + from_upper);
+}
+__device__ __forceinline__ double ecc(const double* __restrict__ Wb, long long nc, long long c, int e) {
+  const int a = (e + 1) % 3, b = (e + 2) % 3;          // E_e = -(v_a B_b - v_b B_a)
+  return -(Wb[(1 + a) * nc + c] * Wb[(5 + b) * nc + c] - Wb[(1 + b) * nc + c] * Wb[(5 + a) * nc + c]);
+}
+
+// ---- CT: E_e on the edges along e at the lower-a, lower-b corner of each cell (Q35, Q36) ----
+__global__ void __launch_bounds__(128) emf_kernel(Dev P) {
+  const int m = blockIdx.y;
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= P.ncell) return;
+  int idx[3]; kji(P, c, idx[2], idx[1], idx[0]);
+  const long long nc = P.ncell, str[3] = {1, P.nt[0], (long long)P.nt[0] * P.nt[1]};
+  const double* Wb = P.W + (long long)m * 8 * nc;
+  for (int e = 0; e < 3; e++) {
+    const int a = (e + 1) % 3, b = (e + 2) % 3;
+    bool in = true;
+    for (int d = 0; d < 3; d++) in = in && idx[d] >= P.ng && idx[d] < P.nx[d] + P.ng + (d == e ? 0 : 1);
+    if (!in) continue;
+    const double* Fa = P.F[a] + (long long)m * 7 * nc;
+    const double* Fb = P.F[b] + (long long)m * 7 * nc;
+    const long long sa = str[a], sb = str[b];
+    // E_e at an a-face = -F_a(B_b) (slot 5 of direction a), at a b-face = +F_b(B_a) (slot 6 of direction b)
+    const double Eaf0 = -Fa[5 * nc + c], Eaf1 = -Fa[5 * nc + c - sb], Ebf0 = Fb[6 * nc + c], Ebf1 = Fb[6 * nc + c - sa];
+    const double mean = 0.25 * ((Eaf1 + Eaf0) + (Ebf1 + Ebf0));
+    const double E00 = ecc(Wb, nc, c, e), E10 = ecc(Wb, nc, c - sa, e), E01 = ecc(Wb, nc, c - sb, e), E11 = ecc(Wb, nc, c - sa - sb, e);
+    const double l2 = upwind(Fa[c - sb], Ebf1 - E11, Ebf0 - E01);
+    const double r2 = upwind(Fa[c],      Ebf1 - E10, Ebf0 - E00);
+    const double l1 = upwind(Fb[c - sa], Eaf1 - E11, Eaf0 - E10);
+    const double r1 = upwind(Fb[c],      Eaf1 - E01, Eaf0 - E00);
+    P.Ec[(long long)m * 3 * nc + e * nc + c] = mean + 0.25 * ((l1 + r1) + (l2 + r2));
+  }
+}
+
+// ---- S4: cells by the flux divergence, faces by the curl of the corner EMFs, with the stage weights ----
+__global__ void __launch_bounds__(128) update_kernel(Dev P, const double* __restrict__ Uin, const double* __restrict__ U0,
+                                                     double* __restrict__ Uout, double g0, double g1, double c1, double c2, double c3) {
+  const int m = blockIdx.y;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long nact = (long long)P.nx[0] * P.nx[1] * P.nx[2];
+  if (t >= nact) return;
+  const int i = (int)(t % P.nx[0]) + P.ng, j = (int)((t / P.nx[0]) % P.nx[1]) + P.ng, k = (int)(t / ((long long)P.nx[0] * P.nx[1])) + P.ng;
+  const long long nc = P.ncell, str[3] = {1, P.nt[0], (long long)P.nt[0] * P.nt[1]};
+  const long long c = k * str[2] + j * str[1] + i;
+  const double cdt[3] = {c1, c2, c3};
+  const double* Ub = Uin + (long long)m * 8 * nc;
+  const double* U0b = U0 + (long long)m * 8 * nc;
+  double* Uo = Uout + (long long)m * 8 * nc;
+  for (int n = 0; n < 5; n++) {
+    double v = g0 * Ub[n * nc + c] + g1 * U0b[n * nc + c];
+    for (int d = 0; d < 3; d++) {
+      const double* Fd = P.F[d] + (long long)m * 7 * nc + n * nc;
+      v = v - cdt[d] * (Fd[c + str[d]] - Fd[c]);
+    }
+    Uo[n * nc + c] = v;
+  }
+  const double* Ec = P.Ec + (long long)m * 3 * nc;
+  for (int a = 0; a < 3; a++) {                        // db_a/dt = -(d_b E_c - d_c E_b), (a, b, c) cyclic
+    const int b = (a + 1) % 3, cc = (a + 2) % 3;
+    double v = g0 * Ub[(5 + a) * nc + c] + g1 * U0b[(5 + a) * nc + c];
+    v = v - cdt[b] * (Ec[cc * nc + c + str[b]] - Ec[cc * nc + c]);
+    v = v + cdt[cc] * (Ec[b * nc + c + str[cc]] - Ec[b * nc + c]);
+    Uo[(5 + a) * nc + c] = v;
+  }
+}
+
+// ---- ghost fill: every ghost cell takes all 8 variables of its periodic image (an active cell) ----
+__global__ void __launch_bounds__(256) fill_kernel(Dev P, double* __restrict__ U) {
+  const int m = blockIdx.y;
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= P.ncell) return;
+  int idx[3]; kji(P, c, idx[2], idx[1], idx[0]);
+  bool ghost = false;
+  int sl[3], s[3];
+  for (int d = 0; d < 3; d++) {
+    const int a = idx[d] - P.ng;
+    if (a < 0 || a >= P.nx[d]) ghost = true;
+    const int N = P.nrb[d] * P.nx[d];
+    int g = (P.lx[3 * m + d] * P.nx[d] + a) % N;
+    if (g < 0) g += N;
+    sl[d] = g / P.nx[d]; s[d] = g - sl[d] * P.nx[d] + P.ng;
+  }
+  if (!ghost) return;
+  const int src = P.leaf[(sl[2] * P.nrb[1] + sl[1]) * P.nrb[0] + sl[0]];
+  const long long nc = P.ncell;
+  const long long cs = ((long long)s[2] * P.nt[1] + s[1]) * P.nt[0] + s[0];
+  for (int n = 0; n < 8; n++) U[((long long)m * 8 + n) * nc + c] = U[((long long)src * 8 + n) * nc + cs];
+}
+
+// ---- S0: CFL reduction with the fast speed per direction (Q37); candidates are positive: ordered-bits atomicMin ----
+__global__ void dt_init_kernel(Dev P) { P.cells[0] = 0x7FF0000000000000ull; P.cells[2] = 0ull; }
+
+__global__ void __launch_bounds__(256) dt_kernel(Dev P, const double* __restrict__ U) {
+  const int m = blockIdx.y;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long nact = (long long)P.nx[0] * P.nx[1] * P.nx[2];
+  double best = __longlong_as_double(0x7FF0000000000000ll);
+  bool bad = false;
+  if (t < nact) {
+    const int i = (int)(t % P.nx[0]) + P.ng, j = (int)((t / P.nx[0]) % P.nx[1]) + P.ng, k = (int)(t / ((long long)P.nx[0] * P.nx[1])) + P.ng;
+    const long long nc = P.ncell, str[3] = {1, P.nt[0], (long long)P.nt[0] * P.nt[1]};
+    const long long c = (long long)m * 8 * nc + k * str[2] + j * str[1] + i;
+    double rho = U[c];
+    if (!(rho >= RHO_FLOOR)) rho = RHO_FLOOR;
+    const double rinv = 1.0 / rho, m1 = U[c + nc], m2 = U[c + 2 * nc], m3 = U[c + 3 * nc];
+    double B[3];
+    for (int d = 0; d < 3; d++) B[d] = 0.5 * (U[c + (5 + d) * nc] + U[c + (5 + d) * nc + str[d]]);
+    const double b2 = B[0] * B[0] + (B[1] * B[1] + B[2] * B[2]);
+    double ug = U[c + 4 * nc] - 0.5 * rinv * (m1 * m1 + (m2 * m2 + m3 * m3)) - 0.5 * b2;
+    if (!(ug >= P_FLOOR / (P.gamma - 1.0))) ug = P_FLOOR / (P.gamma - 1.0);
+    const double gp = P.gamma * ((P.gamma - 1.0) * ug), sum = gp + b2;
+    const double v[3] = {m1 * rinv, m2 * rinv, m3 * rinv};
+    for (int d = 0; d < 3; d++) {
+      double disc = sum * sum - 4.0 * gp * (B[d] * B[d]);
+      if (disc < 0.0) disc = 0.0;
+      const double cf = sqrt((sum + sqrt(disc)) / (2.0 * rho));
+      const double s = fabs(v[d]) + cf;
+      if (!(s > 0.0 && s < __longlong_as_double(0x7FF0000000000000ll))) { bad = true; continue; }
+      const double cand = P.dx[d] / s;
+      if (cand < best) best = cand;
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
+  if ((threadIdx.x & 31) == 0) atomicMin(P.cells, (unsigned long long)__double_as_longlong(best));
+  if (bad) atomicAdd(P.cells + 2, 1ull);
+}
+
+}  // namespace
+
+// =================================== host side: the C-ABI of include/ak_mhd.h ===================================
+struct akm_pack {
+  Dev d{};
+  double xmin[3]{}, xmax[3]{};
+  std::vector<int> lx, leaf;
+  double* u[2] = {nullptr, nullptr};
+  void* work = nullptr;
+  cudaStream_t stream = nullptr;
+  int cur = 0, device = -1;
+  bool bound = false, ghosts_ok = false;
+  long long launches = 0;
+};
+
+namespace {
+size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
+struct WorkLayout { size_t cells, lx, leaf, W, F[3], Ec, total; };
+WorkLayout work_layout(const akm_pack* p) {
+  WorkLayout w;
+  const size_t nc = (size_t)p->d.ncell * p->d.nmb;
+  w.cells = 0;
+  w.lx = 256;
+  w.leaf = w.lx + align256(sizeof(int) * 3 * (size_t)p->d.nmb);
+  w.W = w.leaf + align256(sizeof(int) * (size_t)p->d.nmb);
+  w.F[0] = w.W + align256(8 * nc * sizeof(double));
+  w.F[1] = w.F[0] + align256(7 * nc * sizeof(double));
+  w.F[2] = w.F[1] + align256(7 * nc * sizeof(double));
+  w.Ec = w.F[2] + align256(7 * nc * sizeof(double));
+  w.total = w.Ec + align256(3 * nc * sizeof(double));
+  return w;
+}
+struct Guard {
+  int prev = -1;
+  explicit Guard(int dev) { if (dev >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != dev) cudaSetDevice(dev); else prev = -1; }
+  ~Guard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+}  // namespace
+
+extern "C" const char* akm_last_error(void) { return g_err.c_str(); }
+
+extern "C" akm_pack* akm_pack_create(int nmb, int nx1, int nx2, int nx3, int ng, double gamma, int nrb1, int nrb2, int nrb3,
+                                     const int* lx, const double* xmin, const double* xmax) {
+  if (nmb < 1 || !lx || !xmin || !xmax) { fail(-1, "bad arguments"); return nullptr; }
+  if (ng < 3 || ng > 8) { fail(-1, "MHD with PLM needs 3 <= ng <= 8 (cell-centred fields of the outermost layer are not defined)"); return nullptr; }
+  if (!(gamma > 1.0)) { fail(-1, "gamma <= 1"); return nullptr; }
+  if ((long long)nmb != (long long)nrb1 * nrb2 * nrb3) { fail(-1, "a uniform pack has nrb1*nrb2*nrb3 blocks"); return nullptr; }
+  akm_pack* p = new akm_pack;
+  Dev& d = p->d;
+  d.nmb = nmb; d.ng = ng; d.gamma = gamma;
+  const int nx[3] = {nx1, nx2, nx3}, nrb[3] = {nrb1, nrb2, nrb3};
+  for (int e = 0; e < 3; e++) {
+    if (nx[e] < ng || nrb[e] < 1 || !(xmax[e] > xmin[e])) { fail(-1, "nx_d >= ng, nrb_d >= 1 and a non-empty domain are required"); delete p; return nullptr; }
+    d.nx[e] = nx[e]; d.nt[e] = nx[e] + 2 * ng; d.nrb[e] = nrb[e];
+    p->xmin[e] = xmin[e]; p->xmax[e] = xmax[e];
+    d.dx[e] = (xmax[e] - xmin[e]) / ((double)nrb[e] * nx[e]);
+  }
+  d.ncell = (long long)d.nt[0] * d.nt[1] * d.nt[2];
+  p->lx.assign(lx, lx + 3 * (size_t)nmb);
+  p->leaf.assign(nmb, -1);
+  for (int m = 0; m < nmb; m++) {
+    const int* l = &p->lx[3 * (size_t)m];
+    for (int e = 0; e < 3; e++) if (l[e] < 0 || l[e] >= nrb[e]) { fail(-1, "logical location out of range"); delete p; return nullptr; }
+    int& slot = p->leaf[((size_t)l[2] * nrb2 + l[1]) * nrb1 + l[0]];
+    if (slot >= 0) { fail(-1, "duplicate block"); delete p; return nullptr; }
+    slot = m;
+  }
+  return p;
+}
+
+extern "C" size_t akm_pack_state_bytes(const akm_pack* p) { return p ? (size_t)p->d.nmb * 8 * (size_t)p->d.ncell * 8 : 0; }
+extern "C" size_t akm_pack_work_bytes(const akm_pack* p) { return p ? work_layout(p).total : 0; }
+
+extern "C" int akm_pack_bind(akm_pack* p, void* u_a, void* u_b, void* work, void* cuda_stream) {
+  if (!p) return fail(-1, "null pack");
+  if (!u_a || !u_b || !work) return fail(-1, "null device buffer");
+  if (((uintptr_t)u_a | (uintptr_t)u_b | (uintptr_t)work) & 255) return fail(-1, "buffers must be 256-byte aligned");
+  const size_t sb = akm_pack_state_bytes(p);
+  const WorkLayout wl = work_layout(p);
+  auto overlap = [](const void* a, size_t na, const void* b, size_t nb) {
+    return (uintptr_t)a < (uintptr_t)b + nb && (uintptr_t)b < (uintptr_t)a + na;
+  };
+  if (overlap(u_a, sb, u_b, sb) || overlap(u_a, sb, work, wl.total) || overlap(u_b, sb, work, wl.total))
+    return fail(-1, "device buffers overlap");
+  cudaPointerAttributes pa;
+  AKM_CUDA(cudaPointerGetAttributes(&pa, u_a), "cudaPointerGetAttributes");
+  if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) return fail(-1, "u_a is not a device pointer");
+  p->device = pa.device;
+  Guard guard(p->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  char* w = (char*)work;
+  AKM_CUDA(cudaMemsetAsync(w, 0, 256, st), "memset work");
+  AKM_CUDA(cudaMemcpyAsync(w + wl.lx, p->lx.data(), sizeof(int) * p->lx.size(), cudaMemcpyHostToDevice, st), "upload block table");
+  AKM_CUDA(cudaMemcpyAsync(w + wl.leaf, p->leaf.data(), sizeof(int) * p->leaf.size(), cudaMemcpyHostToDevice, st), "upload leaf map");
+  AKM_CUDA(cudaStreamSynchronize(st), "bind sync");
+  Dev& d = p->d;
+  d.cells = (unsigned long long*)w;
+  d.lx = (const int*)(w + wl.lx);
+  d.leaf = (const int*)(w + wl.leaf);
+  d.W = (double*)(w + wl.W);
+  for (int e = 0; e < 3; e++) d.F[e] = (double*)(w + wl.F[e]);
+  d.Ec = (double*)(w + wl.Ec);
+  p->u[0] = (double*)u_a; p->u[1] = (double*)u_b; p->work = work; p->stream = st;
+  p->cur = 0; p->bound = true; p->ghosts_ok = false; p->launches = 0;
+  return 0;
+}
+
+extern "C" int akm_fill_ghosts(akm_pack* p) {
+  if (!p || !p->bound) return fail(-2, "pack not bound");
+  Guard guard(p->device);
+  const Dev& d = p->d;
+  dim3 grid((unsigned)((d.ncell + 255) / 256), (unsigned)d.nmb);
+  fill_kernel<<<grid, 256, 0, p->stream>>>(d, p->u[p->cur]);
+  AKM_CUDA(cudaGetLastError(), "akm_fill_ghosts launch");
+  p->launches += 1;
+  p->ghosts_ok = true;
+  return 0;
+}
+
+extern "C" int akm_stage(akm_pack* p, int stage, double dt) {
+  if (!p || !p->bound) return fail(-2, "pack not bound");
+  if (stage < 1 || stage > 2) return fail(-1, "stage must be 1 or 2");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(-1, "dt must be positive and finite");
+  if (p->cur != stage - 1) return fail(-2, "stages must be called in order, starting from U^n in buffer A");
+  if (!p->ghosts_ok) return fail(-2, "akm_fill_ghosts must precede akm_stage");
+  Guard guard(p->device);
+  static const double C2[2][3] = {{0.0, 1.0, 1.0}, {0.5, 0.5, 0.5}};        // SSPRK(2,2), Q1
+  const double g0 = C2[stage - 1][0], g1 = C2[stage - 1][1], beta = C2[stage - 1][2];
+  const Dev& d = p->d;
+  const double* Uin = p->u[p->cur];
+  double* Uout = p->u[stage == 2 ? 0 : 1];
+  dim3 gall256((unsigned)((d.ncell + 255) / 256), (unsigned)d.nmb), gall128((unsigned)((d.ncell + 127) / 128), (unsigned)d.nmb);
+  const long long nact = (long long)d.nx[0] * d.nx[1] * d.nx[2];
+  dim3 gact((unsigned)((nact + 127) / 128), (unsigned)d.nmb);
+  prim_kernel<<<gall256, 256, 0, p->stream>>>(d, Uin);
+  flux_kernel<0><<<gall128, 128, 0, p->stream>>>(d, Uin);
+  flux_kernel<1><<<gall128, 128, 0, p->stream>>>(d, Uin);
+  flux_kernel<2><<<gall128, 128, 0, p->stream>>>(d, Uin);
+  emf_kernel<<<gall128, 128, 0, p->stream>>>(d);
+  update_kernel<<<gact, 128, 0, p->stream>>>(d, Uin, p->u[0], Uout, g0, g1, beta * dt / d.dx[0], beta * dt / d.dx[1], beta * dt / d.dx[2]);
+  AKM_CUDA(cudaGetLastError(), "akm_stage launch");
+  p->launches += 6;
+  p->cur = (stage == 2) ? 0 : 1;
+  p->ghosts_ok = false;
+  return 0;
+}
+
+extern "C" int akm_new_dt(akm_pack* p, double cfl, double* dt_out) {
+  if (!p || !p->bound) return fail(-2, "pack not bound");
+  if (!dt_out) return fail(-1, "null dt_out");
+  if (!(cfl > 0.0)) return fail(-1, "cfl must be positive");
+  Guard guard(p->device);
+  const Dev& d = p->d;
+  const long long nact = (long long)d.nx[0] * d.nx[1] * d.nx[2];
+  dim3 gact((unsigned)((nact + 255) / 256), (unsigned)d.nmb);
+  dt_init_kernel<<<1, 1, 0, p->stream>>>(d);
+  dt_kernel<<<gact, 256, 0, p->stream>>>(d, p->u[p->cur]);
+  AKM_CUDA(cudaGetLastError(), "akm_new_dt launch");
+  p->launches += 2;
+  unsigned long long cells[3];
+  AKM_CUDA(cudaMemcpyAsync(cells, d.cells, 24, cudaMemcpyDeviceToHost, p->stream), "akm_new_dt copy");
+  AKM_CUDA(cudaStreamSynchronize(p->stream), "akm_new_dt sync");
+  double dtmin;
+  std::memcpy(&dtmin, &cells[0], 8);
+  if (cells[2] || !(dtmin > 0.0) || !std::isfinite(dtmin)) return fail(-5, "non-finite signal speed in the state (NaN or inf in an active cell)");
+  *dt_out = cfl * dtmin;
+  return 0;
+}
+
+extern "C" int akm_step(akm_pack* p, double cfl, double dt_fixed, double* dt_out) {
+  double dt = dt_fixed;
+  if (!(dt_fixed > 0.0)) { int rc = akm_new_dt(p, cfl, &dt); if (rc) return rc; }
+  for (int stage = 1; stage <= 2; stage++) {
+    int rc = akm_fill_ghosts(p); if (rc) return rc;
+    rc = akm_stage(p, stage, dt); if (rc) return rc;
+  }
+  if (dt_out) *dt_out = dt;
+  return 0;
+}
+
+extern "C" void* akm_pack_current(const akm_pack* p) { return (p && p->bound) ? (void*)p->u[p->cur] : nullptr; }
+extern "C" long long akm_pack_launch_count(const akm_pack* p) { return p ? p->launches : -1; }
+extern "C" long long akm_pack_floor_count(akm_pack* p) {
+  if (!p || !p->bound) { fail(-2, "pack not bound"); return -1; }
+  Guard guard(p->device);
+  unsigned long long n = 0;
+  if (cudaMemcpyAsync(&n, p->d.cells + 1, 8, cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
+      cudaStreamSynchronize(p->stream) != cudaSuccess) { fail(-4, "akm_pack_floor_count copy failed"); return -1; }
+  return (long long)n;
+}
+extern "C" int akm_pack_destroy(akm_pack* p) { delete p; return 0; }

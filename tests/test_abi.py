@@ -19,6 +19,24 @@ def L():
     return ak.lib()
 
 
+def test_every_symbol_of_the_mhd_header_is_exported(L):
+    from paper_2409_16053_b200 import ak_mhd
+    hdr = open(os.path.join(ROOT, "include", "ak_mhd.h")).read()
+    declared = set(re.findall(r"\b(akm_[a-z_0-9]+)\s*\(", hdr))
+    assert declared == set(ak_mhd.SYMBOLS), declared ^ set(ak_mhd.SYMBOLS)
+    for name in declared:
+        assert hasattr(L, name), name
+    # argument checks that need no device
+    h = L.akm_pack_create
+    h.restype = C.c_void_p
+    lx = (C.c_int * 3)(0, 0, 0)
+    lo, hi = (C.c_double * 3)(0, 0, 0), (C.c_double * 3)(1, 1, 1)
+    assert not h(1, 8, 8, 8, 2, C.c_double(5 / 3), 1, 1, 1, lx, lo, hi)          # ng < 3
+    L.akm_last_error.restype = C.c_char_p
+    assert b"ng" in L.akm_last_error()
+    assert not h(2, 8, 8, 8, 3, C.c_double(5 / 3), 1, 1, 1, lx, lo, hi)          # nmb != nrb1 nrb2 nrb3
+
+
 def test_every_declared_symbol_is_exported(L):
     hdr = open(os.path.join(ROOT, "include", "ak.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)

@@ -1,0 +1,156 @@
+"""GPU parity of the MHD + constrained-transport path (include/ak_mhd.h, csrc/mhd/ak_mhd.cu) against the
+oracle (oracle/orc_mhd.cpp) through the C-ABI binding: ghost cells bit-exact, states within the tolerances of the hydro path
+(Q14-style metric <= 1e-12 per stage, <= 1e-9 over the run), div B to round-off on the GPU, conserved totals, dt.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2409_16053_b200 import inputs as I
+from tests import parity as P
+from tests.test_oracle_mhd import G53, ZERO_A, act, brio_wu, divb
+
+pytestmark = pytest.mark.gpu
+TOL_STAGE, TOL_RUN = 1e-12, 1e-9
+
+
+@pytest.fixture(scope="module")
+def om():
+    from oracle import orc_mhd
+    orc_mhd.build()
+    return orc_mhd
+
+
+@pytest.fixture(scope="module")
+def akm():
+    from paper_2409_16053_b200 import ak_mhd
+    ak_mhd.lib()
+    assert torch.cuda.is_available()
+    return ak_mhd
+
+
+def q_mhd(Ug, Uo, gamma):
+    """Per cell max of |d rho|/rho, |d m|/(rho (|v| + c_f)), |dE|/E, |d b|/(|B| + sqrt(rho) c_f-scale); denominators from the oracle."""
+    rho, m, E, b = Uo[:, 0], Uo[:, 1:4], Uo[:, 4], Uo[:, 5:8]
+    b2 = (b ** 2).sum(1)
+    p = np.maximum((gamma - 1.0) * (E - 0.5 * (m ** 2).sum(1) / rho - 0.5 * b2), 0.0)
+    cf = np.sqrt((gamma * p + b2) / rho)
+    vmag = np.sqrt((m ** 2).sum(1)) / rho
+    d = np.abs(Ug - Uo)
+    e = np.maximum(d[:, 0] / rho, d[:, 4] / E)
+    e = np.maximum(e, d[:, 1:4].max(1) / (rho * (vmag + cf)))
+    e = np.maximum(e, d[:, 5:8].max(1) / (np.sqrt(rho) * (vmag + cf)))
+    return float(e.max())
+
+
+def turbulent_state(mesh, mach=0.5):
+    k = 2 * math.pi
+
+    def A(X1, X2, X3):
+        return (0.1 * torch.sin(k * X2) * torch.cos(2 * k * X3) + 0 * X1, 0.1 * torch.sin(k * X3 + 0.3) * torch.cos(k * X1) + 0 * X2,
+                0.1 * torch.cos(2 * k * X1 + 0.7) * torch.sin(k * X2) + 0 * X3)
+
+    prim = lambda X1, X2, X3: (1.0 + 0.3 * torch.sin(k * X1) * torch.cos(k * X2) + 0 * X3,
+                               mach * torch.sin(k * X2 + 0.2) * torch.cos(k * X3) + 0 * X1,
+                               -mach * torch.cos(k * X3) * torch.sin(2 * k * X1) + 0 * X2,
+                               mach * torch.sin(k * X1 + 1.0) * torch.sin(k * X2) + 0 * X3, 0.6 + 0 * X1 + 0 * X2 + 0 * X3)
+    return I.make_state_mhd(mesh, prim, A, (0.4, -0.3, 0.2))
+
+
+def lockstep(om, akm, mesh, U0, gamma, nsteps, cfl=0.3):
+    po = om.OrcMhdPack(mesh, gamma, threads=P.NTHREADS)
+    pg = akm.MhdPack(mesh, gamma)
+    po.load(U0.numpy())
+    pg.load(U0)
+    a = act(mesh)
+    errs = []
+    for step in range(nsteps):
+        dt = po.new_dt(cfl)
+        dtg = pg.new_dt(cfl)
+        assert abs(dtg - dt) <= 1e-13 * dt, (step, dt, dtg)
+        for stage in (1, 2):
+            po.fill_ghosts(); pg.fill_ghosts()
+            if step == 0:
+                ug = pg.current().cpu().numpy()
+                chk = om.OrcMhdPack(mesh, gamma)
+                chk.load(ug); chk.fill_ghosts()
+                assert np.array_equal(chk.current(), ug), f"ghost fill differs at stage {stage}"
+                chk.close()
+            po.stage(stage, dt); pg.stage(stage, dt)
+            if step == 0:
+                e = q_mhd(pg.current().cpu().numpy()[a], po.current()[a], gamma)
+                assert e <= TOL_STAGE * stage, f"stage {stage}: {e:.3e}"
+        errs.append(q_mhd(pg.current().cpu().numpy()[a], po.current()[a], gamma))
+    assert po.floor_count() == 0 and pg.floor_count() == 0
+    return errs, po, pg
+
+
+@pytest.mark.parametrize("nrb,nx", [((2, 2, 2), (16, 16, 16)), ((2, 1, 3), (24, 10, 6)), ((1, 1, 1), (4, 6, 8))])
+def test_turbulent_field_matches_the_oracle(om, akm, nrb, nx):
+    mesh = I.uniform_mesh(nrb, nx, 3)
+    U0 = turbulent_state(mesh)
+    errs, po, pg = lockstep(om, akm, mesh, U0, G53, 6)
+    P.report(f"[parity] MHD turbulent field nmb={mesh.nmb} nx={nx}: worst per step {max(errs):.3e} (bar {TOL_RUN:.0e}), first step {errs[0]:.3e}")
+    assert max(errs) <= TOL_RUN
+    pg.fill_ghosts()
+    ug = pg.current().cpu().numpy()
+    assert np.abs(divb(mesh, ug)).max() <= 2e-13                          # div B on the GPU state
+    a = act(mesh)
+    for n in range(8):                                                   # totals incl. the mean field, GPU vs initial
+        scale = np.abs(U0.numpy()[a][:, n]).sum() + 1.0
+        assert abs(ug[a][:, n].sum() - U0.numpy()[a][:, n].sum()) <= 1e-12 * scale, n
+    # free-running: each side computes its own dt
+    p2 = akm.MhdPack(mesh, G53)
+    p2.load(U0)
+    for _ in range(6):
+        p2.step(0.3)
+    assert q_mhd(p2.current().cpu().numpy()[a], po.current()[a], G53) <= TOL_RUN
+    assert p2.launch_count() == 6 * (2 + 2 * 7)                          # dt_init + dt + 2 x (fill + 6 stage kernels) per step
+
+
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_brio_wu_on_the_gpu(om, akm, d):
+    mesh, U0 = brio_wu(64, d)
+    U0 = torch.from_numpy(U0)
+    po = om.OrcMhdPack(mesh, 2.0, threads=P.NTHREADS)
+    pg = akm.MhdPack(mesh, 2.0)
+    po.load(U0.numpy()); pg.load(U0)
+    t = 0.0
+    while t < 0.05:
+        dt = min(po.new_dt(0.3), 0.05 - t)
+        po.step(0.3, dt); pg.step(0.3, dt)
+        t += dt
+    a = act(mesh)
+    e = q_mhd(pg.current().cpu().numpy()[a], po.current()[a], 2.0)
+    P.report(f"[parity] MHD Brio-Wu along x{d + 1}, 64 cells: {e:.3e}")
+    assert e <= TOL_RUN and pg.floor_count() == 0
+
+
+def test_uniform_state_dt_and_errors_on_the_gpu(om, akm):
+    mesh = I.uniform_mesh((2, 1, 2), (6, 8, 4), 3)
+    prim = lambda X1, X2, X3: (1.3 + 0 * X1 + 0 * X2 + 0 * X3, 0.4 + 0 * X1 + 0 * X2 + 0 * X3, -0.7 + 0 * X1 + 0 * X2 + 0 * X3,
+                               0.2 + 0 * X1 + 0 * X2 + 0 * X3, 0.9 + 0 * X1 + 0 * X2 + 0 * X3)
+    U0 = I.make_state_mhd(mesh, prim, ZERO_A, (0.5, -0.3, 0.8))
+    pg = akm.MhdPack(mesh, G53)
+    pg.load(U0)
+    po = om.OrcMhdPack(mesh, G53)
+    po.load(U0.numpy())
+    assert pg.new_dt(0.3) == po.new_dt(0.3)                              # same state, same bits
+    pg.step(0.3); pg.step(0.3)
+    a = act(mesh)
+    assert np.array_equal(pg.current().cpu().numpy()[a], U0.numpy()[a])  # preserved bit for bit
+    with pytest.raises(akm.AkmError):
+        pg.stage(1, 1e-3)                                                # ghosts not filled
+    pg.fill_ghosts()
+    with pytest.raises(akm.AkmError):
+        pg.stage(2, 1e-3)                                                # stage 2 before stage 1
+    bad = U0.clone()
+    bad[0, 2, 4, 5, 6] = float("nan")
+    pg.load(bad)
+    with pytest.raises(akm.AkmError) as ei:
+        pg.new_dt(0.3)
+    assert "non-finite" in str(ei.value)
+    with pytest.raises(akm.AkmError):
+        akm.MhdPack(I.uniform_mesh((1, 1, 1), (8, 8, 8), 2), G53)        # ng < 3
