@@ -143,6 +143,90 @@ def run_reference(args):
     }))
 
 
+def mhd_workload(name):
+    """MHD workloads: a seeded turbulent field with a mean field on a uniform periodic pack, ng = 3."""
+    import math
+    import torch
+    from paper_2409_16053_b200 import inputs as I
+    nrb, nx = {"mhd_256": (2, 128), "mhd_128": (2, 64), "mhd_64": (2, 32)}[name]
+    mesh = I.uniform_mesh((nrb,) * 3, (nx,) * 3, 3)
+    rm = I.RandomModes.draw(0.5)
+    k = 2 * math.pi
+
+    def prim(X1, X2, X3):
+        v1, v2, v3 = (f(X1, X2, X3) for f in rm.v)
+        return (1.0 + rm.g(X1, X2, X3), v1, v2, v3, torch.ones_like(v1))
+
+    def A(X1, X2, X3):
+        return (0.05 * torch.sin(k * X2) * torch.cos(2 * k * X3) + 0 * X1, 0.05 * torch.sin(k * X3 + 0.3) * torch.cos(k * X1) + 0 * X2,
+                0.05 * torch.cos(2 * k * X1 + 0.7) * torch.sin(k * X2) + 0 * X3)
+    return mesh, prim, A, (0.4, 0.3, 0.2)
+
+
+def run_mhd(args):
+    """The MHD + CT path (include/ak_mhd.h): same contract, metric and timing rules as the hydro line."""
+    import torch
+    from paper_2409_16053_b200 import ak_mhd, inputs as I
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    mesh, prim, A, B0 = mhd_workload(args.workload)
+    U0 = I.make_state_mhd(mesh, prim, A, B0, device=dev)
+    pack = ak_mhd.MhdPack(mesh, I.GAMMA, device=dev)
+    pack.load(U0)
+    ncell, state_bytes = mesh.ncells_active, U0.numel() * 8
+    sampler = ClockSampler(local)
+    sampler.start()
+    for _ in range(args.warmup):
+        pack.step(I.CFL)
+    torch.cuda.synchronize(dev)
+    l0 = pack.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stage_ev = []
+    e0.record(pack.stream)
+    for _ in range(args.steps):
+        dt = pack.new_dt(I.CFL)
+        for stage in (1, 2):
+            pack.fill_ghosts()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(pack.stream); pack.stage(stage, dt); b.record(pack.stream)
+            stage_ev.append((stage, a, b))
+    e1.record(pack.stream)
+    torch.cuda.synchronize(dev)
+    clocks = sampler.stop()
+    launches = pack.launch_count() - l0
+    floors = pack.floor_count()
+    elapsed_ms = e0.elapsed_time(e1)
+    value = ncell * args.steps / (elapsed_ms * 1e-3)
+    st_ms = {s_: statistics.mean(a.elapsed_time(b) for ss, a, b in stage_ev if ss == s_) for s_ in (1, 2)}
+    stage_ms = (st_ms[1] + st_ms[2]) / 2
+    peaks, which = measured_peaks()
+    alg = (128.0 + 192.0) / 2 * ncell           # stage 1 reads 8 and writes 8 variables, stage 2 reads 16 and writes 8
+    ach = alg / (stage_ms * 1e-3) / 1e9
+    host = torch.empty(U0.shape, dtype=torch.float64).pin_memory()
+    host.copy_(U0)
+    t0 = time.perf_counter()
+    for _ in range(2):                          # end to end: host -> device, one step, device -> host
+        pack.load(host)
+        pack.step(I.CFL)
+        host.copy_(pack.current())
+    torch.cuda.synchronize(dev)
+    e2e = {"value": ncell * 2 / (time.perf_counter() - t0), "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes, "steps": 2}
+    print(json.dumps({
+        "metric": "3D MHD cell-updates/sec (fp64)", "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": f"{args.workload}: MHD + CT, PLM + HLLD, SSPRK2, {mesh.nmb} MeshBlocks of {mesh.nx[0]}^3, ng 3, Mach-0.5 modes + mean field",
+                   "cells": ncell, "state_bytes": state_bytes, "l2_policy": "inputs larger than L2" if state_bytes > 4e8 else "state fits L2",
+                   "parallelism": "single GPU"},
+        "roofline": {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"], "traffic": None,
+                     "peak_source": which + " (MEASURED_PEAKS.json hbm_gbs)", "kernel": "akm_stage (six kernels: prim, 3 x flux, emf, update)",
+                     "kernel_ms": stage_ms, "kernel_share_of_step": 2 * stage_ms * args.steps / elapsed_ms, "algorithmic_bytes_per_launch": alg},
+        "cpu_baseline": None, "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "stage_ms": st_ms,
+        "floor_activations": floors,
+    }))
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -340,6 +424,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload.startswith("mhd"):
+        run_mhd(args)
     else:
         run_ours(args)
 

@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(256) prim_kernel(Dev P, const double* __restri
 
 // ---- S2 + S3: PLM + HLLD at the lower D-face of every cell whose stencil exists ----
 template <int D>
-__global__ void __launch_bounds__(128) flux_kernel(Dev P, const double* __restrict__ U) {
+__global__ void __launch_bounds__(128, 8) flux_kernel(Dev P, const double* __restrict__ U) {
   constexpr int D1 = (D + 1) % 3, D2 = (D + 2) % 3;
   const int m = blockIdx.y;
   const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -306,9 +306,20 @@ __global__ void __launch_bounds__(256) dt_kernel(Dev P, const double* __restrict
       if (cand < best) best = cand;
     }
   }
+  // warp shuffles, then the CTA's eight warps through shared memory: one atomic per CTA
   for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
-  if ((threadIdx.x & 31) == 0) atomicMin(P.cells, (unsigned long long)__double_as_longlong(best));
-  if (bad) atomicAdd(P.cells + 2, 1ull);
+  __shared__ double wmin[8];
+  __shared__ int anybad;
+  if (threadIdx.x == 0) anybad = 0;
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) wmin[threadIdx.x >> 5] = best;
+  if (bad) anybad = 1;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; w++) best = fmin(best, wmin[w]);
+    atomicMin(P.cells, (unsigned long long)__double_as_longlong(best));
+    if (anybad) atomicAdd(P.cells + 2, 1ull);
+  }
 }
 
 }  // namespace
