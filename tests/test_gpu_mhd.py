@@ -87,11 +87,11 @@ def lockstep(om, akm, mesh, U0, gamma, nsteps, cfl=0.3):
     return errs, po, pg
 
 
-@pytest.mark.parametrize("nrb,nx", [((2, 2, 2), (16, 16, 16)), ((2, 1, 3), (24, 10, 6)), ((1, 1, 1), (4, 6, 8))])
+@pytest.mark.parametrize("nrb,nx", [((2, 2, 2), (16, 16, 16)), ((2, 1, 3), (24, 10, 6)), ((1, 1, 1), (4, 6, 8)), ((2, 2, 2), (32, 32, 32))])
 def test_turbulent_field_matches_the_oracle(om, akm, nrb, nx):
     mesh = I.uniform_mesh(nrb, nx, 3)
     U0 = turbulent_state(mesh)
-    errs, po, pg = lockstep(om, akm, mesh, U0, G53, 6)
+    errs, po, pg = lockstep(om, akm, mesh, U0, G53, 6 if nx[0] < 32 else 3)
     P.report(f"[parity] MHD turbulent field nmb={mesh.nmb} nx={nx}: worst per step {max(errs):.3e} (bar {TOL_RUN:.0e}), first step {errs[0]:.3e}")
     assert max(errs) <= TOL_RUN
     pg.fill_ghosts()
@@ -104,10 +104,11 @@ def test_turbulent_field_matches_the_oracle(om, akm, nrb, nx):
     # free-running: each side computes its own dt
     p2 = akm.MhdPack(mesh, G53)
     p2.load(U0)
-    for _ in range(6):
+    nst = 6 if nx[0] < 32 else 3
+    for _ in range(nst):
         p2.step(0.3)
     assert q_mhd(p2.current().cpu().numpy()[a], po.current()[a], G53) <= TOL_RUN
-    assert p2.launch_count() == 6 * (2 + 2 * 7)                          # dt_init + dt + 2 x (fill + 6 stage kernels) per step
+    assert p2.launch_count() == nst * (2 + 2 * 7)                          # dt_init + dt + 2 x (fill + 6 stage kernels) per step
 
 
 @pytest.mark.parametrize("d", [0, 1, 2])
