@@ -42,9 +42,13 @@ struct Dev {
 };
 
 // ---- HLLD (Miyoshi & Kusano 2005, restated; Q34): rotated states (rho, u, v, w, u_g, By, Bz), normal field bx ----
-struct Side { double r, u, v, w, by, bz, pt, E, vb, cf, U[7], F[7]; };
+// Written so that few values are live at a time (the sweeps are latency-bound and run at 64 registers): only the scalars of
+// both sides that the wave speeds need, the conserved vector and physical flux of the side the face lies on, and of the
+// other side's star state only what the double-star state takes from it.  Every value is formed by the same operations
+// in the same order as in the definition, so the result does not depend on this arrangement.
+struct Side { double r, u, v, w, by, bz, pt, E, vb, cf; };
 
-__device__ void side_init(double gamma, double bx, const double W[7], Side& s) {
+__device__ __forceinline__ void side_init(double gamma, double bx, const double W[7], Side& s) {
   s.r = W[0]; s.u = W[1]; s.v = W[2]; s.w = W[3]; s.by = W[5]; s.bz = W[6];
   const double e = W[4], p = (gamma - 1.0) * e;
   const double b2 = bx * bx + (s.by * s.by + s.bz * s.bz);
@@ -55,27 +59,31 @@ __device__ void side_init(double gamma, double bx, const double W[7], Side& s) {
   double disc = sum * sum - 4.0 * gp * (bx * bx);
   if (disc < 0.0) disc = 0.0;
   s.cf = sqrt((sum + sqrt(disc)) / (2.0 * s.r));
-  s.U[0] = s.r; s.U[1] = s.r * s.u; s.U[2] = s.r * s.v; s.U[3] = s.r * s.w; s.U[4] = s.E; s.U[5] = s.by; s.U[6] = s.bz;
-  s.F[0] = s.r * s.u; s.F[1] = s.r * s.u * s.u + s.pt - bx * bx; s.F[2] = s.r * s.u * s.v - bx * s.by;
-  s.F[3] = s.r * s.u * s.w - bx * s.bz; s.F[4] = (s.E + s.pt) * s.u - bx * s.vb; s.F[5] = s.by * s.u - bx * s.v;
-  s.F[6] = s.bz * s.u - bx * s.w;
+}
+__device__ __forceinline__ void cons_flux(double bx, const Side& s, double U[7], double F[7]) {
+  U[0] = s.r; U[1] = s.r * s.u; U[2] = s.r * s.v; U[3] = s.r * s.w; U[4] = s.E; U[5] = s.by; U[6] = s.bz;
+  F[0] = s.r * s.u; F[1] = s.r * s.u * s.u + s.pt - bx * bx; F[2] = s.r * s.u * s.v - bx * s.by;
+  F[3] = s.r * s.u * s.w - bx * s.bz; F[4] = (s.E + s.pt) * s.u - bx * s.vb; F[5] = s.by * s.u - bx * s.v;
+  F[6] = s.bz * s.u - bx * s.w;
 }
 
-__device__ void star_state(double bx, const Side& s, double SK, double SM, double pts, double Us[7], double& vbs) {
+// star state of side K behind the outer wave SK: density, transverse velocities and fields, v.B (and the energy if asked for)
+struct Star { double rs, vs, ws, bys, bzs, vbs; };
+__device__ __forceinline__ void star_state(double bx, const Side& s, double SK, double SM, double pts, Star& t) {
   const double sdu = SK - s.u, sdm = SK - SM;
-  const double rs = s.r * sdu / sdm;
+  t.rs = s.r * sdu / sdm;
   const double den = s.r * sdu * sdm - bx * bx;
-  double vs, ws, bys, bzs;
   if (fabs(den) < 1e-8 * pts) {
-    vs = s.v; ws = s.w; bys = s.by; bzs = s.bz;
+    t.vs = s.v; t.ws = s.w; t.bys = s.by; t.bzs = s.bz;
   } else {
     const double f1 = bx * (SM - s.u) / den, f2 = (s.r * sdu * sdu - bx * bx) / den;
-    vs = s.v - s.by * f1; ws = s.w - s.bz * f1;
-    bys = s.by * f2; bzs = s.bz * f2;
+    t.vs = s.v - s.by * f1; t.ws = s.w - s.bz * f1;
+    t.bys = s.by * f2; t.bzs = s.bz * f2;
   }
-  vbs = SM * bx + (vs * bys + ws * bzs);
-  const double Es = (sdu * s.E - s.pt * s.u + pts * SM + bx * (s.vb - vbs)) / sdm;
-  Us[0] = rs; Us[1] = rs * SM; Us[2] = rs * vs; Us[3] = rs * ws; Us[4] = Es; Us[5] = bys; Us[6] = bzs;
+  t.vbs = SM * bx + (t.vs * t.bys + t.ws * t.bzs);
+}
+__device__ __forceinline__ double star_energy(double bx, const Side& s, double SK, double SM, double pts, const Star& t) {
+  return ((SK - s.u) * s.E - s.pt * s.u + pts * SM + bx * (s.vb - t.vbs)) / (SK - SM);
 }
 
 __device__ void hlld(double gamma, double bn, const double WL[7], const double WR[7], double F[7]) {
@@ -84,37 +92,43 @@ __device__ void hlld(double gamma, double bn, const double WL[7], const double W
   side_init(gamma, bn, WR, R);
   const double cfm = fmax(L.cf, R.cf);
   const double SL = fmin(L.u, R.u) - cfm, SR = fmax(L.u, R.u) + cfm;
-  if (SL >= 0.0) { for (int n = 0; n < 7; n++) F[n] = L.F[n]; return; }
-  if (SR <= 0.0) { for (int n = 0; n < 7; n++) F[n] = R.F[n]; return; }
+  double UK[7];
+  if (SL >= 0.0) { cons_flux(bn, L, UK, F); return; }
+  if (SR <= 0.0) { cons_flux(bn, R, UK, F); return; }
   const double mL = L.r * (SL - L.u), mR = R.r * (SR - R.u);
   const double SM = ((mR * R.u - mL * L.u) - (R.pt - L.pt)) / (mR - mL);
   const double pts = ((mR * L.pt - mL * R.pt) + mL * mR * (R.u - L.u)) / (mR - mL);
-  double UsL[7], UsR[7], vbsL, vbsR;
-  star_state(bn, L, SL, SM, pts, UsL, vbsL);
-  star_state(bn, R, SR, SM, pts, UsR, vbsR);
-  const double sqL = sqrt(UsL[0]), sqR = sqrt(UsR[0]);
+  Star tL, tR;
+  star_state(bn, L, SL, SM, pts, tL);
+  star_state(bn, R, SR, SM, pts, tR);
+  const double sqL = sqrt(tL.rs), sqR = sqrt(tR.rs);
   const double SsL = SM - fabs(bn) / sqL, SsR = SM + fabs(bn) / sqR;
   const bool left = (SM >= 0.0);
   const Side& K = left ? L : R;
-  const double* Us = left ? UsL : UsR;
+  const Star& tK = left ? tL : tR;
   const double SK = left ? SL : SR, SsK = left ? SsL : SsR;
+  const double EsK = star_energy(bn, K, SK, SM, pts, tK);
+  const double Us[7] = {tK.rs, tK.rs * SM, tK.rs * tK.vs, tK.rs * tK.ws, EsK, tK.bys, tK.bzs};
+  double FK[7];
+  cons_flux(bn, K, UK, FK);
   const bool outer = left ? (SsL >= 0.0) : (SsR <= 0.0);
   if (outer || 0.5 * bn * bn < 1e-8 * pts) {
-    for (int n = 0; n < 7; n++) F[n] = K.F[n] + SK * (Us[n] - K.U[n]);
+    for (int n = 0; n < 7; n++) F[n] = FK[n] + SK * (Us[n] - UK[n]);
     return;
   }
+  // double-star state; the star velocities go through the conserved momenta as in the definition (rs vs / rs)
   const double sgn = (bn > 0.0) ? 1.0 : -1.0, isum = 1.0 / (sqL + sqR);
-  const double vsL = UsL[2] / UsL[0], wsL = UsL[3] / UsL[0], vsR = UsR[2] / UsR[0], wsR = UsR[3] / UsR[0];
-  const double vss = (sqL * vsL + sqR * vsR + (UsR[5] - UsL[5]) * sgn) * isum;
-  const double wss = (sqL * wsL + sqR * wsR + (UsR[6] - UsL[6]) * sgn) * isum;
-  const double byss = (sqL * UsR[5] + sqR * UsL[5] + sqL * sqR * (vsR - vsL) * sgn) * isum;
-  const double bzss = (sqL * UsR[6] + sqR * UsL[6] + sqL * sqR * (wsR - wsL) * sgn) * isum;
+  const double vsL = (tL.rs * tL.vs) / tL.rs, wsL = (tL.rs * tL.ws) / tL.rs, vsR = (tR.rs * tR.vs) / tR.rs, wsR = (tR.rs * tR.ws) / tR.rs;
+  const double vss = (sqL * vsL + sqR * vsR + (tR.bys - tL.bys) * sgn) * isum;
+  const double wss = (sqL * wsL + sqR * wsR + (tR.bzs - tL.bzs) * sgn) * isum;
+  const double byss = (sqL * tR.bys + sqR * tL.bys + sqL * sqR * (vsR - vsL) * sgn) * isum;
+  const double bzss = (sqL * tR.bzs + sqR * tL.bzs + sqL * sqR * (wsR - wsL) * sgn) * isum;
   const double vbss = SM * bn + (vss * byss + wss * bzss);
   double Uss[7];
   Uss[0] = Us[0]; Uss[1] = Us[1]; Uss[2] = Us[0] * vss; Uss[3] = Us[0] * wss;
-  Uss[4] = left ? UsL[4] - sqL * (vbsL - vbss) * sgn : UsR[4] + sqR * (vbsR - vbss) * sgn;
+  Uss[4] = left ? EsK - sqL * (tL.vbs - vbss) * sgn : EsK + sqR * (tR.vbs - vbss) * sgn;
   Uss[5] = byss; Uss[6] = bzss;
-  for (int n = 0; n < 7; n++) F[n] = K.F[n] + SsK * Uss[n] - (SsK - SK) * Us[n] - SK * K.U[n];
+  for (int n = 0; n < 7; n++) F[n] = FK[n] + SsK * Uss[n] - (SsK - SK) * Us[n] - SK * UK[n];
 }
 
 __device__ __forceinline__ void plm(double qm1, double q0, double qp1, double& qm, double& qp) {
