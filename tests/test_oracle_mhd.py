@@ -284,7 +284,7 @@ def oblique_wave_error(om, family, N, amp=1e-6):
     speed, R, (r0, p0, bpar, bp10, bp20) = mhd_eigenmode(family)
     ct, st = 1.0 / math.sqrt(5.0), 2.0 / math.sqrt(5.0)
     lam = ct
-    mesh = I.uniform_mesh((1, 1, 1), (2 * N, N, 4), 3)
+    mesh = I.uniform_mesh((4, 2, 1), (N // 2, N // 2, 4), 3)       # (8 blocks only spread the oracle over threads)
     mesh.xmax = (1.0, 0.5, 4.0 / (2 * N))                 # cubic cells
     k = 2 * math.pi / lam
 
@@ -303,15 +303,15 @@ def oblique_wave_error(om, family, N, amp=1e-6):
 
     U0 = I.make_state_mhd(mesh, prim, A, rot(bpar, bp10, bp20)).numpy()
     assert np.abs(divb(mesh, U0)).max() <= 1e-12
-    U = run(om, mesh, U0, tend=lam / speed)
+    U = run(om, mesh, U0, tend=lam / speed, threads=8)
     a = act(mesh)
-    return math.sqrt(sum(np.abs(U[a][0, n] - U0[a][0, n]).mean() ** 2 for n in range(8)))
+    return math.sqrt(sum(np.abs(U[a][:, n] - U0[a][:, n]).mean() ** 2 for n in range(8)))
 
 
 @pytest.mark.parametrize("family", ["fast", "alfven", "slow"])
 def test_oblique_linear_waves_converge_at_second_order(om, family):
     """Multi-dimensional CT (Q35, Q36): with the corner EMFs wrong (a dropped or mis-signed upwind term, a wrong face) the wave
     is damped or distorted at first order or grows; with them right the unsplit scheme keeps its second order obliquely."""
-    e = {N: oblique_wave_error(om, family, N) for N in (16, 32, 64)}          # 14, 29, 57 cells per wavelength
-    assert e[64] < e[32] < e[16] < 1e-6
+    e = {N: oblique_wave_error(om, family, N) for N in (32, 64)}              # 29, 57 cells per wavelength
+    assert e[64] < e[32] < 1e-6
     assert 3.0 <= e[32] / e[64] <= 5.0, (family, e)        # (14 -> 29 cells per wavelength is pre-asymptotic, as in 1-D: 2.6)
