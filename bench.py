@@ -59,7 +59,11 @@ class ClockSampler:
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
-        self.rows, self.proc, self.index = [], None, index
+        self.rows, self.proc, self.index, self.first = [], None, index, 0
+
+    def mark(self):
+        """Start of the timed region: only rows sampled from here on are reported."""
+        self.first = len(self.rows)
 
     def start(self):
         try:
@@ -77,6 +81,7 @@ class ClockSampler:
     def stop(self):
         if self.proc:
             self.proc.terminate()
+        self.rows = self.rows[self.first:]
         sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
         mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
@@ -179,7 +184,11 @@ def run_mhd(args):
     sampler.start()
     for _ in range(args.warmup):
         pack.step(I.CFL)
+    t_w = time.perf_counter()
+    while not sampler.rows and sampler.proc and time.perf_counter() - t_w < 3.0:
+        pack.step(I.CFL)
     torch.cuda.synchronize(dev)
+    sampler.mark()
     l0 = pack.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     stage_ev = []
@@ -269,8 +278,12 @@ def run_ours(args):
     sampler.start()                    # nvidia-smi needs a few 100 ms to come up: start it under the warm-up load
     for _ in range(args.warmup):
         pack.step(w.cfl)
+    t_w = time.perf_counter()
+    while not sampler.rows and sampler.proc and time.perf_counter() - t_w < 3.0:
+        pack.step(w.cfl)               # nvidia-smi takes a few 100 ms to deliver its first row: stay under load meanwhile
     stage_ev = []
     barrier()
+    sampler.mark()
     l0 = pack.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(pack.stream)
