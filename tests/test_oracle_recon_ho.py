@@ -14,6 +14,7 @@ from paper_2409_16053_b200 import inputs as I
 from tests.test_oracle_scheme import act
 
 GOLD_C = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "appendix_c.json")))
+GOLD_R = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "recon.json")))    # tests/golden/make_recon.py
 RECON_PPMX, RECON_WENOZ = 2, 3
 
 
@@ -24,6 +25,17 @@ def poly_avg(c, i):
 
 def poly_val(c, x):
     return sum(ck * x ** k for k, ck in enumerate(c))
+
+
+def test_worked_numbers_of_the_stand_alone_script(orc):
+    # a second, vectorised numpy implementation of readings Q29 / Q30 on the 9-point sequence of SURVEY A.3 (steps, an
+    # extremum, a monotone ramp): a wrong branch or coefficient in either implementation shows at O(0.1)
+    q = GOLD_R["recon_q"]
+    for name, fn in (("ppmx", orc.ppmx), ("wenoz", orc.wenoz)):
+        for i, (qm, qp) in GOLD_R[name].items():
+            i = int(i)
+            a, b = fn(q[i - 2:i + 3])
+            assert a == pytest.approx(qm, rel=0, abs=1e-14) and b == pytest.approx(qp, rel=0, abs=1e-14), (name, i)
 
 
 # ------------------------------------------------------------------ WENOZ -------------------------

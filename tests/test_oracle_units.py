@@ -1,7 +1,7 @@
 """Pins for the oracle's single-operation formulas (SURVEY 8(c) "Pins"): c2p, PLM, PPM4, HLLC.
 
 Each test checks the oracle against something other than itself: a closed form, an invariant the
-mathematics fixes, or the independently computed worked numbers of tests/golden/appendix_a.json.
+mathematics fixes, or the worked numbers written by the stand-alone scripts under tests/golden/.
 """
 import json
 import math
@@ -10,7 +10,9 @@ import os
 import numpy as np
 import pytest
 
-GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "appendix_a.json")))
+# reconstruction worked numbers: written by the stand-alone script tests/golden/make_recon.py (numpy forms of
+# make_appendix_c.py; calls nothing under oracle/); they reproduce SURVEY.md Appendix A.3 for PLM and PPM4
+GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "recon.json")))
 # HLLC worked numbers for the round-2 wave-speed reading (Q2): written by the stand-alone script
 # tests/golden/make_hllc_davis.py (star-STATE form of Toro Eqs.(10.37)-(10.39); calls nothing under oracle/)
 GOLD_HLLC = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "hllc_davis.json")))
