@@ -34,6 +34,13 @@ size_t akm_pack_work_bytes(const akm_pack*);    /* work buffer: primitives, face
 /* u_a holds U^n (ghost cells arbitrary) and becomes current; u_b is the second register; work the work buffer; all DEVICE
  * pointers, pairwise disjoint; cuda_stream a cudaStream_t (NULL = legacy stream) on which every kernel is launched. */
 int akm_pack_bind(akm_pack*, void* u_a, void* u_b, void* work, void* cuda_stream);
+/* Arithmetic of the flux sweeps.  on = 0 (default): reciprocals and square roots from the MUFU seed + one cubically convergent step
+ * (1-2 ulp), quotients by a shared divisor through one reciprocal.  on = 1: IEEE division and sqrt in the definition's operation
+ * order; the whole path is then bit-identical to the oracle the tests compare with (verification mode, ~30 % slower).  The two
+ * differ by rounding only (<= 1e-14 per stage in the tests' metric); the upwind switch of the corner EMFs is ramped (DESIGN.md
+ * Q36), so a face mass flux at round-off level does not decide a side. */
+int akm_pack_set_exact(akm_pack*, int on);
+
 /* Periodic copy of all 8 variables into the ghost cells of the current buffer; bit-exact.  Asynchronous. */
 int akm_fill_ghosts(akm_pack*);
 /* One SSPRK(2,2) stage (stage 1: A -> B; stage 2: B and A -> A): primitives, PLM + HLLD in x1, x2, x3, corner EMFs, flux

@@ -184,12 +184,14 @@ static inline void plm(double qm1, double q0, double qp1, double* q_minus, doubl
   *q_minus = q0 - h; *q_plus = q0 + h;
 }
 
-// upwinded (face - centre) difference of an EMF (Gardiner & Stone 2005, restated; Q36): taken on the side the mass flux
-// through the transverse face comes from; the mean where that flux vanishes
-static inline double upwind(double mflux, double from_lower, double from_upper) {
-  if (mflux > 0.0) return from_lower;
-  if (mflux < 0.0) return from_upper;
-  return 0.5 * (from_lower + from_upper);
+// upwinded (face - centre) difference of an EMF (Gardiner & Stone 2005 / 2008, restated; Q36): taken on the side the mass
+// flux through the transverse face comes from.  The switch is ramped: weight w of the lower side = 1/2 + nu clipped to
+// [0, 1], nu = 1024 dt F_mass / (dx (rho_1 + rho_2)) with rho_1,2 the densities of the two cells the face separates -- the
+// pure upwind value once the contact moves more than 2^-10 of a cell per step, the mean at rest, and a CONTINUOUS function
+// of the state in between, so that a mass flux at round-off level does not decide the result.
+static inline double upwind(double k, double mflux, double rho1, double rho2, double from_lower, double from_upper) {
+  const double w = 0.5 + std::fmax(-0.5, std::fmin(0.5, (k * mflux) / (rho1 + rho2)));
+  return w * from_lower + (1.0 - w) * from_upper;
 }
 
 // one block, one stage
@@ -240,7 +242,7 @@ static long long block_stage(const orcm_pack* p, const double* Uin, const double
       Fd[d][4 * nc + c] = F[4]; Fd[d][5 * nc + c] = F[5]; Fd[d][6 * nc + c] = F[6];
     }
   }
-  // CT (Q35, Q36): cell-centred E = -v x B, face EMFs from the Riemann fluxes, corner EMFs by upwinding
+  // CT (Q35, Q36): cell-centred E = -v x B, face EMFs from the Riemann fluxes, corner EMFs by (ramped) upwinding
   std::vector<double> Ecc(3 * nc, 0.0), Ec(3 * nc, 0.0);
   for (size_t c = 0; c < nc; c++) {
     const double v1 = W[nc + c], v2 = W[2 * nc + c], v3 = W[3 * nc + c], B1 = W[5 * nc + c], B2 = W[6 * nc + c], B3 = W[7 * nc + c];
@@ -253,16 +255,18 @@ static long long block_stage(const orcm_pack* p, const double* Uin, const double
     auto Eaf = [&](size_t c) { return -Fa[5 * nc + c]; };
     auto Ebf = [&](size_t c) { return Fb[6 * nc + c]; };
     const double* E0 = &Ecc[e * nc];
+    const double ka = 1024.0 * dt / p->dx(a), kb = 1024.0 * dt / p->dx(b);
     int lo[3], hi[3];
     for (int d = 0; d < 3; d++) { lo[d] = ng; hi[d] = p->nx[d] + ng + 1; }
     hi[e] = p->nx[e] + ng;
     for (int k = lo[2]; k < hi[2]; k++) for (int j = lo[1]; j < hi[1]; j++) for (int i = lo[0]; i < hi[0]; i++) {
       const size_t c = cid(k, j, i), sa = str[a], sb = str[b];
       const double mean = 0.25 * ((Eaf(c - sb) + Eaf(c)) + (Ebf(c - sa) + Ebf(c)));
-      const double l2 = upwind(Fa[c - sb], Ebf(c - sa) - E0[c - sa - sb], Ebf(c) - E0[c - sb]);
-      const double r2 = upwind(Fa[c],      Ebf(c - sa) - E0[c - sa],      Ebf(c) - E0[c]);
-      const double l1 = upwind(Fb[c - sa], Eaf(c - sb) - E0[c - sa - sb], Eaf(c) - E0[c - sa]);
-      const double r1 = upwind(Fb[c],      Eaf(c - sb) - E0[c - sb],      Eaf(c) - E0[c]);
+      const double* rho = W.data();
+      const double l2 = upwind(ka, Fa[c - sb], rho[c - sb - sa], rho[c - sb], Ebf(c - sa) - E0[c - sa - sb], Ebf(c) - E0[c - sb]);
+      const double r2 = upwind(ka, Fa[c],      rho[c - sa],      rho[c],      Ebf(c - sa) - E0[c - sa],      Ebf(c) - E0[c]);
+      const double l1 = upwind(kb, Fb[c - sa], rho[c - sa - sb], rho[c - sa], Eaf(c - sb) - E0[c - sa - sb], Eaf(c) - E0[c - sa]);
+      const double r1 = upwind(kb, Fb[c],      rho[c - sb],      rho[c],      Eaf(c - sb) - E0[c - sb],      Eaf(c) - E0[c]);
       Ec[e * nc + c] = mean + 0.25 * ((l1 + r1) + (l2 + r2));
     }
   }

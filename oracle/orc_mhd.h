@@ -17,8 +17,8 @@
  * convergence to the exact Riemann solution; div B = 0 to round-off; conservation of mass, momentum, energy and mean field;
  * uniform state preserved bit-exactly; plane-parallel flow stays plane-parallel and direction-independent bit for bit; second-
  * order convergence of fast, Alfven and slow linear waves whose eigenvectors the test computes numerically.
- * PARITY UNPINNED beyond those properties: the HLLD wave-speed estimate and degenerate-case thresholds (Q34), the sharp
- * upwinding rule of the corner EMFs (Q36).
+ * PARITY UNPINNED beyond those properties: the HLLD wave-speed estimate and degenerate-case thresholds (Q34), the ramp
+ * width of the upwinding rule of the corner EMFs (Q36).
  */
 #ifndef ORC_MHD_H
 #define ORC_MHD_H

@@ -1,8 +1,9 @@
 // ak_mhd.cu -- MHD + constrained-transport stage over a MeshBlockPack (include/ak_mhd.h), first cut:
 // correct and device-resident, not yet fused.  Paper: Eq.(5) and the gamma-law energy, face-centred field with
 // CT and Gardiner-Stone upwinded EMFs, HLLD.  Readings DESIGN.md Q33-Q37.
-// Compiled with -fmad=false and IEEE division / sqrt: every expression rounds once per operation in the order written,
-// because the sign of a mass flux decides which side a corner EMF is upwinded from and a contracted product could flip it.
+// Compiled with -fmad=false: every expression rounds once per operation in the order written (fused multiply-adds only where
+// written out).  With akm_pack_set_exact the flux sweeps also use IEEE division / sqrt in the definition's order and the whole
+// path is bit-identical to the definition evaluated on the host; the default uses MUFU-seeded reciprocals and square roots.
 // Kernels, all one thread per cell with i fastest (coalesced), launched in this order per stage:
 //   prim_kernel      U -> W = (rho, v, u_g, B_cc)                                   work: W[8]
 //   flux_kernel<D>   PLM on W along D, HLLD at the lower D-face of every cell        work: F_D[7]
@@ -41,13 +42,38 @@ struct Dev {
   unsigned long long* cells;  // [0] min dt as ordered bits, [1] floor count, [2] non-finite count
 };
 
+// ---- division and square root in two flavours --------------------------------------------------------------------
+// X = true: IEEE division and sqrt in the definition's operation order -- the results are bit-identical to the definition
+// evaluated on the host, which is how this path is verified (akm_pack_set_exact).  X = false (default): MUFU seed + one
+// cubically convergent step (1-2 ulp), 3-4 FP64-pipe instructions instead of ~13, and quotients by a shared divisor formed
+// with one reciprocal: the sweeps are bound by the issue of exactly these instructions.  The fast flavour differs from the
+// exact one by rounding only (measured <= 1e-14 per stage in the parity metric); the upwind switch of the corner EMFs is
+// ramped (Q36), so a mass flux at round-off level does not turn that rounding into a different choice of side.
+__device__ __forceinline__ double rcp_fast(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  const double e = fma(-x, r, 1.0);
+  return fma(r, fma(e, e, e), r);
+}
+__device__ __forceinline__ double sqrt_fast(double x) {      // x > 0 (0 -> 0 handled by the caller where it can occur)
+  double r;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  const double e = fma(-(x * r), r, 1.0);
+  r = fma(r, e * fma(0.375, e, 0.5), r);
+  return x * r;
+}
+template <bool X> __device__ __forceinline__ double div_(double a, double b) { if constexpr (X) return a / b; else return a * rcp_fast(b); }
+template <bool X> __device__ __forceinline__ double rcp_(double b) { if constexpr (X) return 1.0 / b; else return rcp_fast(b); }
+template <bool X> __device__ __forceinline__ double sqrt_(double x) { if constexpr (X) return sqrt(x); else return x > 0.0 ? sqrt_fast(x) : 0.0; }
+
 // ---- HLLD (Miyoshi & Kusano 2005, restated; Q34): rotated states (rho, u, v, w, u_g, By, Bz), normal field bx ----
-// Written so that few values are live at a time (the sweeps are latency-bound and run at 64 registers): only the scalars of
-// both sides that the wave speeds need, the conserved vector and physical flux of the side the face lies on, and of the
-// other side's star state only what the double-star state takes from it.  Every value is formed by the same operations
-// in the same order as in the definition, so the result does not depend on this arrangement.
+// Written so that few values are live at a time (the sweeps run at 64 registers): only the scalars of both sides that the
+// wave speeds need, the conserved vector and physical flux of the side the face lies on, and of the other side's star state
+// only what the double-star state takes from it.  In the exact flavour every value is formed by the same operations in the
+// same order as in the definition, so the result does not depend on this arrangement.
 struct Side { double r, u, v, w, by, bz, pt, E, vb, cf; };
 
+template <bool X>
 __device__ __forceinline__ void side_init(double gamma, double bx, const double W[7], Side& s) {
   s.r = W[0]; s.u = W[1]; s.v = W[2]; s.w = W[3]; s.by = W[5]; s.bz = W[6];
   const double e = W[4], p = (gamma - 1.0) * e;
@@ -58,7 +84,7 @@ __device__ __forceinline__ void side_init(double gamma, double bx, const double 
   const double gp = gamma * p, sum = gp + b2;
   double disc = sum * sum - 4.0 * gp * (bx * bx);
   if (disc < 0.0) disc = 0.0;
-  s.cf = sqrt((sum + sqrt(disc)) / (2.0 * s.r));
+  s.cf = sqrt_<X>(div_<X>(sum + sqrt_<X>(disc), 2.0 * s.r));
 }
 __device__ __forceinline__ void cons_flux(double bx, const Side& s, double U[7], double F[7]) {
   U[0] = s.r; U[1] = s.r * s.u; U[2] = s.r * s.v; U[3] = s.r * s.w; U[4] = s.E; U[5] = s.by; U[6] = s.bz;
@@ -67,47 +93,61 @@ __device__ __forceinline__ void cons_flux(double bx, const Side& s, double U[7],
   F[6] = s.bz * s.u - bx * s.w;
 }
 
-// star state of side K behind the outer wave SK: density, transverse velocities and fields, v.B (and the energy if asked for)
-struct Star { double rs, vs, ws, bys, bzs, vbs; };
+// star state of side K behind the outer wave SK: density, transverse velocities and fields, v.B; isdm = 1 / (SK - SM)
+struct Star { double rs, vs, ws, bys, bzs, vbs, isdm; };
+template <bool X>
 __device__ __forceinline__ void star_state(double bx, const Side& s, double SK, double SM, double pts, Star& t) {
   const double sdu = SK - s.u, sdm = SK - SM;
-  t.rs = s.r * sdu / sdm;
+  if constexpr (X) { t.rs = s.r * sdu / sdm; t.isdm = 0.0; }
+  else { t.isdm = rcp_fast(sdm); t.rs = (s.r * sdu) * t.isdm; }
   const double den = s.r * sdu * sdm - bx * bx;
   if (fabs(den) < 1e-8 * pts) {
     t.vs = s.v; t.ws = s.w; t.bys = s.by; t.bzs = s.bz;
   } else {
-    const double f1 = bx * (SM - s.u) / den, f2 = (s.r * sdu * sdu - bx * bx) / den;
+    double f1, f2;
+    if constexpr (X) { f1 = bx * (SM - s.u) / den; f2 = (s.r * sdu * sdu - bx * bx) / den; }
+    else { const double id = rcp_fast(den); f1 = (bx * (SM - s.u)) * id; f2 = (s.r * sdu * sdu - bx * bx) * id; }
     t.vs = s.v - s.by * f1; t.ws = s.w - s.bz * f1;
     t.bys = s.by * f2; t.bzs = s.bz * f2;
   }
   t.vbs = SM * bx + (t.vs * t.bys + t.ws * t.bzs);
 }
+template <bool X>
 __device__ __forceinline__ double star_energy(double bx, const Side& s, double SK, double SM, double pts, const Star& t) {
-  return ((SK - s.u) * s.E - s.pt * s.u + pts * SM + bx * (s.vb - t.vbs)) / (SK - SM);
+  const double num = (SK - s.u) * s.E - s.pt * s.u + pts * SM + bx * (s.vb - t.vbs);
+  if constexpr (X) return num / (SK - SM); else return num * t.isdm;
 }
 
+template <bool X>
 __device__ void hlld(double gamma, double bn, const double WL[7], const double WR[7], double F[7]) {
   Side L, R;
-  side_init(gamma, bn, WL, L);
-  side_init(gamma, bn, WR, R);
+  side_init<X>(gamma, bn, WL, L);
+  side_init<X>(gamma, bn, WR, R);
   const double cfm = fmax(L.cf, R.cf);
   const double SL = fmin(L.u, R.u) - cfm, SR = fmax(L.u, R.u) + cfm;
   double UK[7];
   if (SL >= 0.0) { cons_flux(bn, L, UK, F); return; }
   if (SR <= 0.0) { cons_flux(bn, R, UK, F); return; }
   const double mL = L.r * (SL - L.u), mR = R.r * (SR - R.u);
-  const double SM = ((mR * R.u - mL * L.u) - (R.pt - L.pt)) / (mR - mL);
-  const double pts = ((mR * L.pt - mL * R.pt) + mL * mR * (R.u - L.u)) / (mR - mL);
+  double SM, pts;
+  if constexpr (X) {
+    SM = ((mR * R.u - mL * L.u) - (R.pt - L.pt)) / (mR - mL);
+    pts = ((mR * L.pt - mL * R.pt) + mL * mR * (R.u - L.u)) / (mR - mL);
+  } else {
+    const double im = rcp_fast(mR - mL);
+    SM = ((mR * R.u - mL * L.u) - (R.pt - L.pt)) * im;
+    pts = ((mR * L.pt - mL * R.pt) + mL * mR * (R.u - L.u)) * im;
+  }
   Star tL, tR;
-  star_state(bn, L, SL, SM, pts, tL);
-  star_state(bn, R, SR, SM, pts, tR);
-  const double sqL = sqrt(tL.rs), sqR = sqrt(tR.rs);
-  const double SsL = SM - fabs(bn) / sqL, SsR = SM + fabs(bn) / sqR;
+  star_state<X>(bn, L, SL, SM, pts, tL);
+  star_state<X>(bn, R, SR, SM, pts, tR);
+  const double sqL = sqrt_<X>(tL.rs), sqR = sqrt_<X>(tR.rs);
+  const double SsL = SM - div_<X>(fabs(bn), sqL), SsR = SM + div_<X>(fabs(bn), sqR);
   const bool left = (SM >= 0.0);
   const Side& K = left ? L : R;
   const Star& tK = left ? tL : tR;
   const double SK = left ? SL : SR, SsK = left ? SsL : SsR;
-  const double EsK = star_energy(bn, K, SK, SM, pts, tK);
+  const double EsK = star_energy<X>(bn, K, SK, SM, pts, tK);
   const double Us[7] = {tK.rs, tK.rs * SM, tK.rs * tK.vs, tK.rs * tK.ws, EsK, tK.bys, tK.bzs};
   double FK[7];
   cons_flux(bn, K, UK, FK);
@@ -116,9 +156,11 @@ __device__ void hlld(double gamma, double bn, const double WL[7], const double W
     for (int n = 0; n < 7; n++) F[n] = FK[n] + SK * (Us[n] - UK[n]);
     return;
   }
-  // double-star state; the star velocities go through the conserved momenta as in the definition (rs vs / rs)
-  const double sgn = (bn > 0.0) ? 1.0 : -1.0, isum = 1.0 / (sqL + sqR);
-  const double vsL = (tL.rs * tL.vs) / tL.rs, wsL = (tL.rs * tL.ws) / tL.rs, vsR = (tR.rs * tR.vs) / tR.rs, wsR = (tR.rs * tR.ws) / tR.rs;
+  // double-star state; in the exact flavour the star velocities go through the conserved momenta as in the definition
+  const double sgn = (bn > 0.0) ? 1.0 : -1.0, isum = rcp_<X>(sqL + sqR);
+  double vsL, wsL, vsR, wsR;
+  if constexpr (X) { vsL = (tL.rs * tL.vs) / tL.rs; wsL = (tL.rs * tL.ws) / tL.rs; vsR = (tR.rs * tR.vs) / tR.rs; wsR = (tR.rs * tR.ws) / tR.rs; }
+  else { vsL = tL.vs; wsL = tL.ws; vsR = tR.vs; wsR = tR.ws; }
   const double vss = (sqL * vsL + sqR * vsR + (tR.bys - tL.bys) * sgn) * isum;
   const double wss = (sqL * wsL + sqR * wsR + (tR.bzs - tL.bzs) * sgn) * isum;
   const double byss = (sqL * tR.bys + sqR * tL.bys + sqL * sqR * (vsR - vsL) * sgn) * isum;
@@ -131,9 +173,10 @@ __device__ void hlld(double gamma, double bn, const double WL[7], const double W
   for (int n = 0; n < 7; n++) F[n] = FK[n] + SsK * Uss[n] - (SsK - SK) * Us[n] - SK * UK[n];
 }
 
+template <bool X>
 __device__ __forceinline__ void plm(double qm1, double q0, double qp1, double& qm, double& qp) {
   const double dL = q0 - qm1, dR = qp1 - q0, prod = dL * dR;
-  const double h = (prod > 0.0) ? prod / (dL + dR) : 0.0;
+  const double h = (prod > 0.0) ? div_<X>(prod, dL + dR) : 0.0;
   qm = q0 - h; qp = q0 + h;
 }
 
@@ -167,8 +210,11 @@ __global__ void __launch_bounds__(256) prim_kernel(Dev P, const double* __restri
 }
 
 // ---- S2 + S3: PLM + HLLD at the lower D-face of every cell whose stencil exists ----
-template <int D>
-__global__ void __launch_bounds__(128, 8) flux_kernel(Dev P, const double* __restrict__ U) {
+// Occupancy (measured at 256^3): the exact flavour waits on its IEEE division chains and runs best with 32 warps per SM (64
+// registers, 240 B spilled); the fast flavour is bound by the FP64 pipe and runs best without spills (96 registers, 20 warps:
+// 1.49 -> 1.67 G cell-updates/s against 8 CTAs per SM).
+template <int D, bool X>
+__global__ void __launch_bounds__(128, X ? 8 : 5) flux_kernel(Dev P, const double* __restrict__ U) {
   constexpr int D1 = (D + 1) % 3, D2 = (D + 2) % 3;
   const int m = blockIdx.y;
   const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -184,20 +230,22 @@ __global__ void __launch_bounds__(128, 8) flux_kernel(Dev P, const double* __res
   for (int q = 0; q < 7; q++) {
     const double* w = Wb + var[q] * nc;
     double qm, qp;
-    plm(w[cm - st], w[cm], w[cm + st], qm, qp); WL[q] = qp;
-    plm(w[c - st], w[c], w[c + st], qm, qp);    WR[q] = qm;
+    plm<X>(w[cm - st], w[cm], w[cm + st], qm, qp); WL[q] = qp;
+    plm<X>(w[c - st], w[c], w[c + st], qm, qp);    WR[q] = qm;
   }
-  hlld(P.gamma, U[(long long)m * 8 * nc + (5 + D) * nc + c], WL, WR, F);
+  hlld<X>(P.gamma, U[(long long)m * 8 * nc + (5 + D) * nc + c], WL, WR, F);
   double* Fb = P.F[D] + (long long)m * 7 * nc;
   Fb[c] = F[0]; Fb[(1 + D) * nc + c] = F[1]; Fb[(1 + D1) * nc + c] = F[2]; Fb[(1 + D2) * nc + c] = F[3];
   Fb[4 * nc + c] = F[4]; Fb[5 * nc + c] = F[5]; Fb[6 * nc + c] = F[6];
 }
 
-// upwinded (face - centre) EMF difference: from the side the mass flux comes from; the mean where it vanishes (Q36)
-__device__ __forceinline__ double upwind(double mflux, double from_lower, double from_upper) {
-  if (mflux > 0.0) return from_lower;
-  if (mflux < 0.0) return from_upper;
-  return 0.5 * (from_lower + from_upper);
+// upwinded (face - centre) EMF difference (Q36): weight w of the lower side = 1/2 + nu clipped to [0, 1] with
+// nu = 1024 dt F_mass / (dx (rho_1 + rho_2)) -- pure upwind once the contact crosses 2^-10 of a cell per step, the mean at
+// rest, continuous in between (a mass flux at round-off level does not decide the result).  k = 1024 dt / dx.
+template <bool X>
+__device__ __forceinline__ double upwind(double k, double mflux, double rho1, double rho2, double from_lower, double from_upper) {
+  const double w = 0.5 + fmax(-0.5, fmin(0.5, div_<X>(k * mflux, rho1 + rho2)));
+  return w * from_lower + (1.0 - w) * from_upper;
 }
 __device__ __forceinline__ double ecc(const double* __restrict__ Wb, long long nc, long long c, int e) {
   const int a = (e + 1) % 3, b = (e + 2) % 3;          // E_e = -(v_a B_b - v_b B_a)
@@ -205,13 +253,15 @@ __device__ __forceinline__ double ecc(const double* __restrict__ Wb, long long n
 }
 
 // ---- CT: E_e on the edges along e at the lower-a, lower-b corner of each cell (Q35, Q36) ----
-__global__ void __launch_bounds__(128) emf_kernel(Dev P) {
+template <bool X>
+__global__ void __launch_bounds__(128) emf_kernel(Dev P, double k0, double k1, double k2) {
   const int m = blockIdx.y;
   const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= P.ncell) return;
   int idx[3]; kji(P, c, idx[2], idx[1], idx[0]);
   const long long nc = P.ncell, str[3] = {1, P.nt[0], (long long)P.nt[0] * P.nt[1]};
   const double* Wb = P.W + (long long)m * 8 * nc;
+  const double kd[3] = {k0, k1, k2};
   for (int e = 0; e < 3; e++) {
     const int a = (e + 1) % 3, b = (e + 2) % 3;
     bool in = true;
@@ -224,10 +274,11 @@ __global__ void __launch_bounds__(128) emf_kernel(Dev P) {
     const double Eaf0 = -Fa[5 * nc + c], Eaf1 = -Fa[5 * nc + c - sb], Ebf0 = Fb[6 * nc + c], Ebf1 = Fb[6 * nc + c - sa];
     const double mean = 0.25 * ((Eaf1 + Eaf0) + (Ebf1 + Ebf0));
     const double E00 = ecc(Wb, nc, c, e), E10 = ecc(Wb, nc, c - sa, e), E01 = ecc(Wb, nc, c - sb, e), E11 = ecc(Wb, nc, c - sa - sb, e);
-    const double l2 = upwind(Fa[c - sb], Ebf1 - E11, Ebf0 - E01);
-    const double r2 = upwind(Fa[c],      Ebf1 - E10, Ebf0 - E00);
-    const double l1 = upwind(Fb[c - sa], Eaf1 - E11, Eaf0 - E10);
-    const double r1 = upwind(Fb[c],      Eaf1 - E01, Eaf0 - E00);
+    const double r00 = Wb[c], r10 = Wb[c - sa], r01 = Wb[c - sb], r11 = Wb[c - sa - sb];
+    const double l2 = upwind<X>(kd[a], Fa[c - sb], r11, r01, Ebf1 - E11, Ebf0 - E01);
+    const double r2 = upwind<X>(kd[a], Fa[c],      r10, r00, Ebf1 - E10, Ebf0 - E00);
+    const double l1 = upwind<X>(kd[b], Fb[c - sa], r11, r10, Eaf1 - E11, Eaf0 - E10);
+    const double r1 = upwind<X>(kd[b], Fb[c],      r01, r00, Eaf1 - E01, Eaf0 - E00);
     P.Ec[(long long)m * 3 * nc + e * nc + c] = mean + 0.25 * ((l1 + r1) + (l2 + r2));
   }
 }
@@ -348,6 +399,7 @@ struct akm_pack {
   cudaStream_t stream = nullptr;
   int cur = 0, device = -1;
   bool bound = false, ghosts_ok = false;
+  bool exact = false;          // akm_pack_set_exact: IEEE division / sqrt in the definition's order (bit-identical, slower)
   long long launches = 0;
 };
 
@@ -443,6 +495,12 @@ extern "C" int akm_pack_bind(akm_pack* p, void* u_a, void* u_b, void* work, void
   return 0;
 }
 
+extern "C" int akm_pack_set_exact(akm_pack* p, int on) {
+  if (!p) return fail(-1, "null pack");
+  p->exact = on != 0;
+  return 0;
+}
+
 extern "C" int akm_fill_ghosts(akm_pack* p) {
   if (!p || !p->bound) return fail(-2, "pack not bound");
   Guard guard(p->device);
@@ -471,10 +529,18 @@ extern "C" int akm_stage(akm_pack* p, int stage, double dt) {
   const long long nact = (long long)d.nx[0] * d.nx[1] * d.nx[2];
   dim3 gact((unsigned)((nact + 127) / 128), (unsigned)d.nmb);
   prim_kernel<<<gall256, 256, 0, p->stream>>>(d, Uin);
-  flux_kernel<0><<<gall128, 128, 0, p->stream>>>(d, Uin);
-  flux_kernel<1><<<gall128, 128, 0, p->stream>>>(d, Uin);
-  flux_kernel<2><<<gall128, 128, 0, p->stream>>>(d, Uin);
-  emf_kernel<<<gall128, 128, 0, p->stream>>>(d);
+  if (p->exact) {
+    flux_kernel<0, true><<<gall128, 128, 0, p->stream>>>(d, Uin);
+    flux_kernel<1, true><<<gall128, 128, 0, p->stream>>>(d, Uin);
+    flux_kernel<2, true><<<gall128, 128, 0, p->stream>>>(d, Uin);
+  } else {
+    flux_kernel<0, false><<<gall128, 128, 0, p->stream>>>(d, Uin);
+    flux_kernel<1, false><<<gall128, 128, 0, p->stream>>>(d, Uin);
+    flux_kernel<2, false><<<gall128, 128, 0, p->stream>>>(d, Uin);
+  }
+  const double k0 = 1024.0 * dt / d.dx[0], k1 = 1024.0 * dt / d.dx[1], k2 = 1024.0 * dt / d.dx[2];
+  if (p->exact) emf_kernel<true><<<gall128, 128, 0, p->stream>>>(d, k0, k1, k2);
+  else emf_kernel<false><<<gall128, 128, 0, p->stream>>>(d, k0, k1, k2);
   update_kernel<<<gact, 128, 0, p->stream>>>(d, Uin, p->u[0], Uout, g0, g1, beta * dt / d.dx[0], beta * dt / d.dx[1], beta * dt / d.dx[2]);
   AKM_CUDA(cudaGetLastError(), "akm_stage launch");
   p->launches += 6;

@@ -59,9 +59,9 @@ def turbulent_state(mesh, mach=0.5):
     return I.make_state_mhd(mesh, prim, A, (0.4, -0.3, 0.2))
 
 
-def lockstep(om, akm, mesh, U0, gamma, nsteps, cfl=0.3):
+def lockstep(om, akm, mesh, U0, gamma, nsteps, cfl=0.3, exact=False):
     po = om.OrcMhdPack(mesh, gamma, threads=P.NTHREADS)
-    pg = akm.MhdPack(mesh, gamma)
+    pg = akm.MhdPack(mesh, gamma, exact=exact)
     po.load(U0.numpy())
     pg.load(U0)
     a = act(mesh)
@@ -87,13 +87,18 @@ def lockstep(om, akm, mesh, U0, gamma, nsteps, cfl=0.3):
     return errs, po, pg
 
 
+@pytest.mark.parametrize("exact", [False, True])
 @pytest.mark.parametrize("nrb,nx", [((2, 2, 2), (16, 16, 16)), ((2, 1, 3), (24, 10, 6)), ((1, 1, 1), (4, 6, 8)), ((2, 2, 2), (32, 32, 32))])
-def test_turbulent_field_matches_the_oracle(om, akm, nrb, nx):
+def test_turbulent_field_matches_the_oracle(om, akm, nrb, nx, exact):
+    """Default arithmetic (MUFU-seeded reciprocals / square roots): within the hydro path's tolerances; verification mode
+    (akm_pack_set_exact: IEEE division / sqrt in the definition's order): bit-identical to the oracle."""
     mesh = I.uniform_mesh(nrb, nx, 3)
     U0 = turbulent_state(mesh)
-    errs, po, pg = lockstep(om, akm, mesh, U0, G53, 6 if nx[0] < 32 else 3)
-    P.report(f"[parity] MHD turbulent field nmb={mesh.nmb} nx={nx}: worst per step {max(errs):.3e} (bar {TOL_RUN:.0e}), first step {errs[0]:.3e}")
+    errs, po, pg = lockstep(om, akm, mesh, U0, G53, 6 if nx[0] < 32 else 3, exact=exact)
+    P.report(f"[parity] MHD turbulent field nmb={mesh.nmb} nx={nx} exact={exact}: worst per step {max(errs):.3e} (bar {TOL_RUN:.0e}), first step {errs[0]:.3e}")
     assert max(errs) <= TOL_RUN
+    if exact:
+        assert max(errs) == 0.0
     pg.fill_ghosts()
     ug = pg.current().cpu().numpy()
     assert np.abs(divb(mesh, ug)).max() <= 2e-13                          # div B on the GPU state
@@ -102,7 +107,7 @@ def test_turbulent_field_matches_the_oracle(om, akm, nrb, nx):
         scale = np.abs(U0.numpy()[a][:, n]).sum() + 1.0
         assert abs(ug[a][:, n].sum() - U0.numpy()[a][:, n].sum()) <= 1e-12 * scale, n
     # free-running: each side computes its own dt
-    p2 = akm.MhdPack(mesh, G53)
+    p2 = akm.MhdPack(mesh, G53, exact=exact)
     p2.load(U0)
     nst = 6 if nx[0] < 32 else 3
     for _ in range(nst):
@@ -111,12 +116,13 @@ def test_turbulent_field_matches_the_oracle(om, akm, nrb, nx):
     assert p2.launch_count() == nst * (2 + 2 * 7)                          # dt_init + dt + 2 x (fill + 6 stage kernels) per step
 
 
+@pytest.mark.parametrize("exact", [False, True])
 @pytest.mark.parametrize("d", [0, 1, 2])
-def test_brio_wu_on_the_gpu(om, akm, d):
+def test_brio_wu_on_the_gpu(om, akm, d, exact):
     mesh, U0 = brio_wu(64, d)
     U0 = torch.from_numpy(U0)
     po = om.OrcMhdPack(mesh, 2.0, threads=P.NTHREADS)
-    pg = akm.MhdPack(mesh, 2.0)
+    pg = akm.MhdPack(mesh, 2.0, exact=exact)
     po.load(U0.numpy()); pg.load(U0)
     t = 0.0
     while t < 0.05:
@@ -125,8 +131,8 @@ def test_brio_wu_on_the_gpu(om, akm, d):
         t += dt
     a = act(mesh)
     e = q_mhd(pg.current().cpu().numpy()[a], po.current()[a], 2.0)
-    P.report(f"[parity] MHD Brio-Wu along x{d + 1}, 64 cells: {e:.3e}")
-    assert e <= TOL_RUN and pg.floor_count() == 0
+    P.report(f"[parity] MHD Brio-Wu along x{d + 1}, 64 cells, exact={exact}: {e:.3e}")
+    assert e <= TOL_RUN and pg.floor_count() == 0 and (e == 0.0 or not exact)
 
 
 def test_uniform_state_dt_and_errors_on_the_gpu(om, akm):

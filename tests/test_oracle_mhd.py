@@ -202,6 +202,33 @@ def test_divb_conservation_and_mean_field_on_a_multiblock_mesh(om):
     assert np.abs(U[a] - U0[a]).max() > 1e-3                               # (something happened)
 
 
+def test_corner_emfs_are_continuous_where_a_mass_flux_changes_sign(om):
+    """Q36 (ramped upwind switch): a 3-D field whose x1 velocity vanishes on a plane.  Shifting that velocity by +-1e-14 -- the
+    size of a rounding difference between two arithmetics -- must move the result of a step by a comparable amount; with a
+    sharp switch on the sign of the mass flux the two runs pick opposite sides there and differ by ~1e-4."""
+    mesh = I.uniform_mesh((1, 1, 1), (8, 6, 12), 3)
+    k = 2 * math.pi
+
+    def A(X1, X2, X3):
+        return (0.1 * torch.sin(k * X2) * torch.cos(2 * k * X3) + 0 * X1, 0.1 * torch.sin(k * X3 + 0.3) * torch.cos(k * X1) + 0 * X2,
+                0.1 * torch.cos(2 * k * X1 + 0.7) * torch.sin(k * X2) + 0 * X3)
+
+    outs = []
+    for eps in (1e-14, -1e-14, 1e-3):
+        prim = lambda X1, X2, X3: (1.0 + 0.3 * torch.sin(k * X1) * torch.cos(k * X2) + 0 * X3,
+                                   eps + 0 * X1 + 0 * X2 + 0 * X3,              # x1 mass fluxes at round-off level everywhere
+                                   -0.5 * torch.cos(k * X3) * torch.sin(2 * k * X1) + 0 * X2,
+                                   0.5 * torch.sin(k * X1 + 1.0) * torch.sin(k * X2) + 0 * X3, 0.6 + 0 * X1 + 0 * X2 + 0 * X3)
+        U0 = I.make_state_mhd(mesh, prim, A, (0.4, -0.3, 0.2)).numpy()
+        p = om.OrcMhdPack(mesh, G53)
+        p.load(U0)
+        p.step(0.3, 2e-3)
+        outs.append(p.current()[act(mesh)].copy())
+        p.close()
+    assert np.abs(outs[0] - outs[1]).max() <= 1e-12                         # (measured 2.5e-14; a sharp switch gives ~1e-4)
+    assert np.abs(outs[0] - outs[2]).max() > 1e-6                           # (the velocity does matter once it is not round-off)
+
+
 def test_uniform_magnetised_state_is_preserved_bit_exactly(om):
     mesh = I.uniform_mesh((2, 1, 2), (6, 8, 4), 3)
     prim = lambda X1, X2, X3: (1.3 + 0 * X1 + 0 * X2 + 0 * X3, 0.4 + 0 * X1 + 0 * X2 + 0 * X3, -0.7 + 0 * X1 + 0 * X2 + 0 * X3,
