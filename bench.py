@@ -148,26 +148,6 @@ def run_reference(args):
     }))
 
 
-def mhd_workload(name):
-    """MHD workloads: a seeded turbulent field with a mean field on a uniform periodic pack, ng = 3."""
-    import math
-    import torch
-    from paper_2409_16053_b200 import inputs as I
-    nrb, nx = {"mhd_256": (2, 128), "mhd_128": (2, 64), "mhd_64": (2, 32)}[name]
-    mesh = I.uniform_mesh((nrb,) * 3, (nx,) * 3, 3)
-    rm = I.RandomModes.draw(0.5)
-    k = 2 * math.pi
-
-    def prim(X1, X2, X3):
-        v1, v2, v3 = (f(X1, X2, X3) for f in rm.v)
-        return (1.0 + rm.g(X1, X2, X3), v1, v2, v3, torch.ones_like(v1))
-
-    def A(X1, X2, X3):
-        return (0.05 * torch.sin(k * X2) * torch.cos(2 * k * X3) + 0 * X1, 0.05 * torch.sin(k * X3 + 0.3) * torch.cos(k * X1) + 0 * X2,
-                0.05 * torch.cos(2 * k * X1 + 0.7) * torch.sin(k * X2) + 0 * X3)
-    return mesh, prim, A, (0.4, 0.3, 0.2)
-
-
 def run_mhd(args):
     """The MHD + CT path (include/ak_mhd.h): same contract, metric and timing rules as the hydro line."""
     import torch
@@ -175,7 +155,7 @@ def run_mhd(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    mesh, prim, A, B0 = mhd_workload(args.workload)
+    mesh, prim, A, B0 = I.mhd_workload(args.workload)
     U0 = I.make_state_mhd(mesh, prim, A, B0, device=dev)
     pack = ak_mhd.MhdPack(mesh, I.GAMMA, device=dev)
     pack.load(U0)

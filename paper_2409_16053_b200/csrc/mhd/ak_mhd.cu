@@ -181,8 +181,14 @@ __device__ __forceinline__ void plm(double qm1, double q0, double qp1, double& q
 }
 
 // (k, j, i) of a flat cell index inside one block
+// (32-bit: a block has fewer than 2^31 cells, checked at create; the 64-bit form cost ~250 instructions per thread)
 __device__ __forceinline__ void kji(const Dev& P, long long c, int& k, int& j, int& i) {
-  i = (int)(c % P.nt[0]); j = (int)((c / P.nt[0]) % P.nt[1]); k = (int)(c / ((long long)P.nt[0] * P.nt[1]));
+  const unsigned cu = (unsigned)c, row = cu / (unsigned)P.nt[0], kk = row / (unsigned)P.nt[1];
+  i = (int)(cu - row * (unsigned)P.nt[0]); j = (int)(row - kk * (unsigned)P.nt[1]); k = (int)kk;
+}
+__device__ __forceinline__ void kji_active(const Dev& P, long long t, int& k, int& j, int& i) {
+  const unsigned tu = (unsigned)t, row = tu / (unsigned)P.nx[0], kk = row / (unsigned)P.nx[1];
+  i = (int)(tu - row * (unsigned)P.nx[0]) + P.ng; j = (int)(row - kk * (unsigned)P.nx[1]) + P.ng; k = (int)kk + P.ng;
 }
 
 // ---- S1: primitives with the cell-centred field = mean of the two faces (Q33); not for the outermost upper layer ----
@@ -290,7 +296,7 @@ __global__ void __launch_bounds__(128) update_kernel(Dev P, const double* __rest
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long nact = (long long)P.nx[0] * P.nx[1] * P.nx[2];
   if (t >= nact) return;
-  const int i = (int)(t % P.nx[0]) + P.ng, j = (int)((t / P.nx[0]) % P.nx[1]) + P.ng, k = (int)(t / ((long long)P.nx[0] * P.nx[1])) + P.ng;
+  int i, j, k; kji_active(P, t, k, j, i);
   const long long nc = P.ncell, str[3] = {1, P.nt[0], (long long)P.nt[0] * P.nt[1]};
   const long long c = k * str[2] + j * str[1] + i;
   const double cdt[3] = {c1, c2, c3};
@@ -322,16 +328,16 @@ __global__ void __launch_bounds__(256) fill_kernel(Dev P, double* __restrict__ U
   if (c >= P.ncell) return;
   int idx[3]; kji(P, c, idx[2], idx[1], idx[0]);
   bool ghost = false;
+  for (int d = 0; d < 3; d++) ghost = ghost || idx[d] < P.ng || idx[d] >= P.nx[d] + P.ng;
+  if (!ghost) return;
   int sl[3], s[3];
   for (int d = 0; d < 3; d++) {
     const int a = idx[d] - P.ng;
-    if (a < 0 || a >= P.nx[d]) ghost = true;
     const int N = P.nrb[d] * P.nx[d];
     int g = (P.lx[3 * m + d] * P.nx[d] + a) % N;
     if (g < 0) g += N;
     sl[d] = g / P.nx[d]; s[d] = g - sl[d] * P.nx[d] + P.ng;
   }
-  if (!ghost) return;
   const int src = P.leaf[(sl[2] * P.nrb[1] + sl[1]) * P.nrb[0] + sl[0]];
   const long long nc = P.ncell;
   const long long cs = ((long long)s[2] * P.nt[1] + s[1]) * P.nt[0] + s[0];
@@ -348,7 +354,7 @@ __global__ void __launch_bounds__(256) dt_kernel(Dev P, const double* __restrict
   double best = __longlong_as_double(0x7FF0000000000000ll);
   bool bad = false;
   if (t < nact) {
-    const int i = (int)(t % P.nx[0]) + P.ng, j = (int)((t / P.nx[0]) % P.nx[1]) + P.ng, k = (int)(t / ((long long)P.nx[0] * P.nx[1])) + P.ng;
+    int i, j, k; kji_active(P, t, k, j, i);
     const long long nc = P.ncell, str[3] = {1, P.nt[0], (long long)P.nt[0] * P.nt[1]};
     const long long c = (long long)m * 8 * nc + k * str[2] + j * str[1] + i;
     double rho = U[c];
@@ -446,6 +452,7 @@ extern "C" akm_pack* akm_pack_create(int nmb, int nx1, int nx2, int nx3, int ng,
     d.dx[e] = (xmax[e] - xmin[e]) / ((double)nrb[e] * nx[e]);
   }
   d.ncell = (long long)d.nt[0] * d.nt[1] * d.nt[2];
+  if (d.ncell >= (1ll << 31)) { fail(-3, "a MeshBlock with 2^31 or more cells (ghosts included) is not supported"); delete p; return nullptr; }
   p->lx.assign(lx, lx + 3 * (size_t)nmb);
   p->leaf.assign(nmb, -1);
   for (int m = 0; m < nmb; m++) {

@@ -354,3 +354,22 @@ def make_state_mhd(mesh: Mesh, prim_fn: PrimFn, A_fn, B0=(0.0, 0.0, 0.0), gamma:
         act[0] = rho; act[1] = rho * v1; act[2] = rho * v2; act[3] = rho * v3
         act[4] = P / (gamma - 1.0) + 0.5 * rho * (v1 * v1 + v2 * v2 + v3 * v3) + 0.5 * (bc1 * bc1 + bc2 * bc2 + bc3 * bc3)
     return U
+
+
+def mhd_workload(name: str):
+    """MHD workloads of bench.py and the full-size GPU test: the seeded Mach-0.5 random-mode velocity field and
+    5 % density modes of the hydro configs, P = 1, a tangled field from a vector potential plus a mean field, on a uniform periodic
+    pack of 8 MeshBlocks, ng = 3.  -> (mesh, prim_fn, A_fn, B0) for make_state_mhd."""
+    nrb, nx = {"mhd_256": (2, 128), "mhd_128": (2, 64), "mhd_64": (2, 32)}[name]
+    mesh = uniform_mesh((nrb,) * 3, (nx,) * 3, 3)
+    rm = RandomModes.draw(0.5)
+    k = 2 * math.pi
+
+    def prim(X1, X2, X3):
+        v1, v2, v3 = (f(X1, X2, X3) for f in rm.v)
+        return (1.0 + rm.g(X1, X2, X3), v1, v2, v3, torch.ones_like(v1))
+
+    def A(X1, X2, X3):
+        return (0.05 * torch.sin(k * X2) * torch.cos(2 * k * X3) + 0 * X1, 0.05 * torch.sin(k * X3 + 0.3) * torch.cos(k * X1) + 0 * X2,
+                0.05 * torch.cos(2 * k * X1 + 0.7) * torch.sin(k * X2) + 0 * X3)
+    return mesh, prim, A, (0.4, 0.3, 0.2)

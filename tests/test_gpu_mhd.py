@@ -161,3 +161,83 @@ def test_uniform_state_dt_and_errors_on_the_gpu(om, akm):
     assert "non-finite" in str(ei.value)
     with pytest.raises(akm.AkmError):
         akm.MhdPack(I.uniform_mesh((1, 1, 1), (8, 8, 8), 2), G53)        # ng < 3
+
+
+def _assemble8(mesh, U):
+    """Active cells of every block -> global (8, N3, N2, N1) on the device; a face field sits on the lower face of its cell, so the
+    periodic global array holds every face exactly once."""
+    g, nx = mesh.ng, mesh.nx
+    G = torch.empty((8, mesh.nrb[2] * nx[2], mesh.nrb[1] * nx[1], mesh.nrb[0] * nx[0]), dtype=U.dtype, device=U.device)
+    for m, (_, l1, l2, l3) in enumerate(mesh.blocks):
+        G[:, l3 * nx[2]:(l3 + 1) * nx[2], l2 * nx[1]:(l2 + 1) * nx[1], l1 * nx[0]:(l1 + 1) * nx[0]] = U[m][:, g:-g, g:-g, g:-g]
+    return G
+
+
+def _dt_reference_mhd(G, gamma, dx, cfl):
+    """cfl * min dx_d / (|v_d| + c_f,d) with torch ops on the assembled global state (not the library's kernels)."""
+    rho, mom, E = G[0], G[1:4], G[4]
+    B = torch.stack([0.5 * (G[5 + d] + torch.roll(G[5 + d], -1, dims=2 - d)) for d in range(3)])
+    b2 = (B ** 2).sum(0)
+    p = (gamma - 1.0) * (E - 0.5 * (mom ** 2).sum(0) / rho - 0.5 * b2)
+    gp = gamma * p
+    best = math.inf
+    for d in range(3):
+        disc = torch.clamp((gp + b2) ** 2 - 4.0 * gp * B[d] ** 2, min=0.0)
+        cf = torch.sqrt((gp + b2 + torch.sqrt(disc)) / (2.0 * rho))
+        best = min(best, float((dx[d] / (mom[d].abs() / rho + cf)).min()))
+    return cfl * best
+
+
+def test_mhd_256_full_size_sampled(om, akm):
+    """The workload bench.py times (`--workload mhd_256`: 8 MeshBlocks of 128^3, default arithmetic, the same launches): TWO steps on
+    the GPU, checked on sampled 64^3 sub-boxes that the oracle advances one by one as small periodic blocks with the same dx and dt
+    sequence.  One stage reaches at most 4 cells (PLM 2, cell-centred field 1, corner EMFs 1), two steps 16: the sub-box interior
+    >= 20 cells from its faces is exact (24^3 cells and faces compared per box; boxes on the corner where the 8 blocks meet, on the
+    periodic wrap, inside a block).  Plus what holds at any size: div B, totals, no floors, each dt against torch on the global state."""
+    mesh, prim, A, B0 = I.mhd_workload("mhd_256")
+    dev = torch.device("cuda", 0)
+    U0 = I.make_state_mhd(mesh, prim, A, B0, device=dev)
+    pg = akm.MhdPack(mesh, I.GAMMA, device=dev)
+    pg.load(U0)
+    G0 = _assemble8(mesh, U0)
+    del U0
+    nsteps, n, pad = 2, 64, 20
+    origins = [(96, 96, 96), (224, 224, 224), (30, 140, 200), (150, 10, 70)]
+    idx = lambda G, o: [(torch.arange(n, device=G.device) + o[d]) % G.shape[3 - d] for d in range(3)]
+    sub = lambda G, o: G.index_select(1, idx(G, o)[2]).index_select(2, idx(G, o)[1]).index_select(3, idx(G, o)[0]).cpu().numpy()
+    subs0 = [sub(G0, o) for o in origins]
+    tot0 = G0.sum(dim=(1, 2, 3)).cpu().numpy()
+    abs0 = G0.abs().sum(dim=(1, 2, 3)).cpu().numpy()
+    dx = mesh.dx(0)
+    dt_ref = _dt_reference_mhd(G0, I.GAMMA, dx, I.CFL)
+    del G0
+    dts = []
+    for step in range(nsteps):
+        dt = pg.new_dt(I.CFL)
+        assert abs(dt - dt_ref) <= 1e-13 * dt_ref, (step, dt, dt_ref)
+        pg.step(I.CFL, dt)
+        dts.append(dt)
+        G1 = _assemble8(mesh, pg.current())
+        dt_ref = _dt_reference_mhd(G1, I.GAMMA, dx, I.CFL)
+    assert pg.floor_count() == 0
+    tot1 = G1.sum(dim=(1, 2, 3)).cpu().numpy()
+    assert (np.abs(tot1 - tot0) / (abs0 + 1.0)).max() <= 1e-12                # mass, momentum, energy, mean field
+    div = sum((torch.roll(G1[5 + d], -1, dims=2 - d) - G1[5 + d]) / dx[d] for d in range(3))
+    assert float(div.abs().max()) <= 1e-11                                   # (|B| / dx ~ 250: a few ulp of that)
+    sub_mesh = I.Mesh((1, 1, 1), (n, n, n), 3, [(0, 0, 0, 0)], xmax=(n * dx[0], n * dx[1], n * dx[2]))
+    assert sub_mesh.dx(0) == dx
+    worst = 0.0
+    for o, s0 in zip(origins, subs0):
+        po = om.OrcMhdPack(sub_mesh, I.GAMMA, threads=P.NTHREADS)
+        u = np.zeros(sub_mesh.state_shape()[:1] + (8,) + sub_mesh.state_shape()[2:])
+        u[0][:, 3:-3, 3:-3, 3:-3] = s0
+        po.load(u)
+        for dt in dts:
+            po.step(I.CFL, dt)
+        ref = po.current()[0][:, 3 + pad:-3 - pad, 3 + pad:-3 - pad, 3 + pad:-3 - pad]
+        got = sub(G1, o)[:, pad:-pad, pad:-pad, pad:-pad]
+        e = q_mhd(got[None], ref[None], I.GAMMA)
+        worst = max(worst, e)
+        assert e <= 2 * nsteps * TOL_STAGE, (o, e)
+        po.close()
+    P.report(f"[parity] MHD mhd_256 full size (8 x 128^3, bench launch configuration): worst sampled difference after {nsteps} steps = {worst:.2e}")
