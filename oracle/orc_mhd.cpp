@@ -2,6 +2,7 @@
 // citations and pins).  Plain loops, fp64, compiled -O2 -ffp-contract=off -fno-fast-math.  P:NN = /root/reference/PAPER.md
 // line NN; Qnn = readings listed in DESIGN.md.
 #include "orc_mhd.h"
+#include "orc.h"       // orc_ppm4, orc_wenoz: the hydro oracle's reconstruction functions (same oracle, linked in)
 
 #include <cmath>
 #include <cstdio>
@@ -110,6 +111,8 @@ struct orcm_pack {
   std::vector<int> lx, leaf;             // lx[3m+d]; leaf[(l3*nrb2+l2)*nrb1+l1] -> m
   double* u[2] = { nullptr, nullptr };
   int cur = 0, nthreads = 1;
+  int recon = 0;                         // 0 PLM, 1 PPM4, 3 WENOZ (the hydro oracle's codes and functions: oracle/orc.h)
+  int nstages = 2;                       // 2: SSPRK(2,2), 3: SSPRK(3,3) (Q1)
   bool bound = false;
   long long floor_count = 0;
   size_t ncell() const { return (size_t)nt[0] * nt[1] * nt[2]; }
@@ -227,15 +230,23 @@ static long long block_stage(const orcm_pack* p, const double* Uin, const double
     const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
     const int var[7] = { 0, 1 + d, 1 + d1, 1 + d2, 4, 5 + d1, 5 + d2 };
     int lo[3] = { 0, 0, 0 }, hi[3] = { n1 - 1, n2 - 1, n3 - 1 };        // transverse: wherever W exists
-    lo[d] = 2; hi[d] = nt[d] - 2;                                       // along d: cells c-2 .. c+1 must hold W
+    const int R = (p->recon == 0) ? 2 : 3;                              // along d: cells c-R .. c+R-1 must hold W
+    lo[d] = R; hi[d] = nt[d] - R;
     for (int k = lo[2]; k < hi[2]; k++) for (int j = lo[1]; j < hi[1]; j++) for (int i = lo[0]; i < hi[0]; i++) {
       const size_t c = cid(k, j, i), cm = c - str[d];
       double WL[7], WR[7], F[7];
       for (int q = 0; q < 7; q++) {
         const double* w = &W[var[q] * nc];
         double qm, qp;
-        plm(w[cm - str[d]], w[cm], w[cm + str[d]], &qm, &qp); WL[q] = qp;
-        plm(w[c - str[d]], w[c], w[c + str[d]], &qm, &qp);    WR[q] = qm;
+        if (p->recon == 0) {
+          plm(w[cm - str[d]], w[cm], w[cm + str[d]], &qm, &qp); WL[q] = qp;
+          plm(w[c - str[d]], w[c], w[c + str[d]], &qm, &qp);    WR[q] = qm;
+        } else {                                                          // the hydro oracle's S2 / S2' on each primitive
+          const double sL[5] = { w[cm - 2 * str[d]], w[cm - str[d]], w[cm], w[cm + str[d]], w[cm + 2 * str[d]] };
+          const double sR[5] = { w[c - 2 * str[d]], w[c - str[d]], w[c], w[c + str[d]], w[c + 2 * str[d]] };
+          if (p->recon == 1) { orc_ppm4(sL, &qm, &qp); WL[q] = qp; orc_ppm4(sR, &qm, &qp); WR[q] = qm; }
+          else               { orc_wenoz(sL, &qm, &qp); WL[q] = qp; orc_wenoz(sR, &qm, &qp); WR[q] = qm; }
+        }
       }
       orcm_hlld(p->gamma, Ub[(5 + d) * nc + c], WL, WR, F);
       Fd[d][c] = F[0]; Fd[d][(1 + d) * nc + c] = F[1]; Fd[d][(1 + d1) * nc + c] = F[2]; Fd[d][(1 + d2) * nc + c] = F[3];
@@ -292,18 +303,42 @@ static long long block_stage(const orcm_pack* p, const double* Uin, const double
   return nfl;
 }
 
+// options: the reconstruction list of P:101 and the RK2 / RK3 integrators the paper's MHD tests and runs use (RK3 + PPMX /
+// WENOZ, PPM4, PLM on the linear waves; WENOZ + RK2 + HLLD for the turbulence run)
+extern "C" int orcm_pack_set_recon(orcm_pack* p, int recon) {
+  if (!p) return fail("null pack");
+  if (recon != 0 && recon != 1 && recon != 3) return fail("reconstruction: 0 PLM, 1 PPM4, 3 WENOZ");
+  if (recon != 0 && p->ng < 4) return fail("PPM4 / WENOZ with face-centred fields need ng >= 4");
+  p->recon = recon;
+  return 0;
+}
+extern "C" int orcm_pack_set_integrator(orcm_pack* p, int nstages) {
+  if (!p) return fail("null pack");
+  if (nstages != 2 && nstages != 3) return fail("integrator: 2 = SSPRK(2,2), 3 = SSPRK(3,3)");
+  if (p->cur != 0) return fail("the integrator can only change between steps");
+  p->nstages = nstages;
+  return 0;
+}
+
+// One stage: U_out = g0 U_in + g1 U^n - beta dt div F(U_in) for the cells, the same weights with the curl of the corner EMFs for
+// the faces.  SSPRK(2,2): A -> B, (B, A) -> A.  SSPRK(3,3) (Q1): A -> B; B <- 1/4 (B + dt L(B)) + 3/4 A (in place: every block
+// forms all its fluxes and EMFs from U_in before it writes); A <- 2/3 (B + dt L(B)) + 1/3 A.
 extern "C" int orcm_stage(orcm_pack* p, int stage, double dt) {
   if (!p || !p->bound) return fail("pack not bound");
-  if (stage < 1 || stage > 2 || p->cur != stage - 1) return fail("stages must be called in order, starting from U^n in buffer A");
+  const int ns = p->nstages;
+  if (stage < 1 || stage > ns || p->cur != (stage == 1 ? 0 : 1)) return fail("stages must be called in order, starting from U^n in buffer A");
   static const double C2[2][3] = { { 0.0, 1.0, 1.0 }, { 0.5, 0.5, 0.5 } };      // SSPRK(2,2), Q1
-  const double g0 = C2[stage - 1][0], g1 = C2[stage - 1][1], beta = C2[stage - 1][2];
+  static const double C3[3][3] = { { 0.0, 1.0, 1.0 }, { 0.25, 0.75, 0.25 }, { 2.0 / 3.0, 1.0 / 3.0, 2.0 / 3.0 } };
+  const double* cf = (ns == 2) ? C2[stage - 1] : C3[stage - 1];
+  const double g0 = cf[0], g1 = cf[1], beta = cf[2];
   const double* Uin = p->u[p->cur]; const double* U0 = p->u[0];
-  double* Uout = p->u[stage == 2 ? 0 : 1];
+  const int out = (stage == ns) ? 0 : 1;
+  double* Uout = p->u[out];
   long long nfl = 0;
 #pragma omp parallel for schedule(dynamic) num_threads(p->nthreads) reduction(+ : nfl) if (p->nthreads > 1)
   for (int m = 0; m < p->nmb; m++) nfl += block_stage(p, Uin, U0, Uout, m, g0, g1, beta, dt);
   p->floor_count += nfl;
-  p->cur = (stage == 2) ? 0 : 1;
+  p->cur = out;
   return 0;
 }
 

@@ -9,7 +9,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liborc_mhd.so")
-_SRC = [os.path.join(_HERE, "orc_mhd.cpp"), os.path.join(_HERE, "orc_mhd.h")]
+_SRC = [os.path.join(_HERE, f) for f in ("orc_mhd.cpp", "orc.cpp", "orc_mhd.h", "orc.h")]
 _lib = None
 
 
@@ -18,7 +18,7 @@ def build(force: bool = False) -> str:
             and all(os.path.getmtime(_SO) >= os.path.getmtime(s) for s in _SRC)):
         return _SO
     subprocess.run(["g++", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared", "-Wall",
-                    "-o", _SO, _SRC[0]], check=True, cwd=_HERE)
+                    "-o", _SO, _SRC[0], _SRC[1]], check=True, cwd=_HERE)
     return _SO
 
 
@@ -32,6 +32,8 @@ def lib():
     L.orcm_pack_create.argtypes = [C.c_int] * 5 + [C.c_double] + [C.c_int] * 3 + [ip, dp, dp]
     L.orcm_pack_bind.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     L.orcm_set_threads.argtypes = [C.c_void_p, C.c_int]
+    L.orcm_pack_set_recon.argtypes = [C.c_void_p, C.c_int]
+    L.orcm_pack_set_integrator.argtypes = [C.c_void_p, C.c_int]
     L.orcm_fill_ghosts.argtypes = [C.c_void_p]
     L.orcm_stage.argtypes = [C.c_void_p, C.c_int, C.c_double]
     L.orcm_new_dt.argtypes = [C.c_void_p, C.c_double, dp]
@@ -67,9 +69,10 @@ def hlld(gamma, bn, WL, WR):
 class OrcMhdPack:
     """Oracle MHD pack over a uniform Mesh (paper_2409_16053_b200.inputs.Mesh); owns two numpy state buffers of 8 variables."""
 
-    def __init__(self, mesh, gamma, threads=1):
+    def __init__(self, mesh, gamma, threads=1, recon=0, nstages=2):
         L = lib()
         self.mesh = mesh
+        self.nstages = nstages
         lx = [v for (_, l1, l2, l3) in mesh.blocks for v in (l1, l2, l3)]
         self._h = L.orcm_pack_create(mesh.nmb, *mesh.nx, mesh.ng, gamma, *mesh.nrb, (C.c_int * len(lx))(*lx),
                                      (C.c_double * 3)(*mesh.xmin), (C.c_double * 3)(*mesh.xmax))
@@ -81,6 +84,8 @@ class OrcMhdPack:
         _chk(L.orcm_pack_bind(self._h, self.ua.ctypes.data, self.ub.ctypes.data))
         if threads != 1:
             _chk(L.orcm_set_threads(self._h, threads))
+        _chk(L.orcm_pack_set_recon(self._h, recon))
+        _chk(L.orcm_pack_set_integrator(self._h, nstages))
 
     def load(self, U):
         self.ua[...] = np.asarray(U)
@@ -106,7 +111,7 @@ class OrcMhdPack:
     def step(self, cfl, dt=None):
         if dt is None:
             dt = self.new_dt(cfl)
-        for s in (1, 2):
+        for s in range(1, self.nstages + 1):
             self.fill_ghosts()
             self.stage(s, dt)
         return dt

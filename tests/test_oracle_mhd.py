@@ -104,8 +104,8 @@ def divb(mesh, U):
     return (b1[up1] - b1[s]) / dx[0] + (b2[up2] - b2[s]) / dx[1] + (b3[up3] - b3[s]) / dx[2]
 
 
-def run(om, mesh, U0, gamma=G53, cfl=0.3, nsteps=None, tend=None, threads=4):
-    p = om.OrcMhdPack(mesh, gamma, threads=threads)
+def run(om, mesh, U0, gamma=G53, cfl=0.3, nsteps=None, tend=None, threads=4, recon=0, nstages=2):
+    p = om.OrcMhdPack(mesh, gamma, threads=threads, recon=recon, nstages=nstages)
     p.load(U0)
     t, n = 0.0, 0
     while (nsteps is None or n < nsteps) and (tend is None or t < tend):
@@ -279,9 +279,9 @@ def mhd_eigenmode(family):
     return speed, v / np.abs(v).max(), (r, p, bx, by, bz)
 
 
-def wave_error(om, family, N, amp=1e-6):
+def wave_error(om, family, N, amp=1e-6, recon=0, nstages=2):
     speed, R, (r0, p0, bx, by0, bz0) = mhd_eigenmode(family)
-    mesh = I.uniform_mesh((1, 1, 1), (N, 4, 4), 3)
+    mesh = I.uniform_mesh((1, 1, 1), (N, 4, 4), 3 if recon == 0 else 4)
     k = 2 * math.pi
 
     def prim(X1, X2, X3):
@@ -293,9 +293,28 @@ def wave_error(om, family, N, amp=1e-6):
         return (0 * c, -amp * R[6] * c, amp * R[5] * c)
 
     U0 = I.make_state_mhd(mesh, prim, A, (bx, by0, bz0)).numpy()
-    U = run(om, mesh, U0, tend=1.0 / speed)
+    U = run(om, mesh, U0, tend=1.0 / speed, recon=recon, nstages=nstages)
     a = act(mesh)
     return math.sqrt(sum(np.abs(U[a][0, n] - U0[a][0, n]).mean() ** 2 for n in range(8)))
+
+
+def test_higher_order_options_reproduce_the_papers_convergence_orders(om):
+    """"While fourth-order convergence is observed for RK3+PPMX and RK3+WENOZ for slow and Alfven waves, the fast wave only
+    converges at second-order even in one-dimension.  For PPM4 and PLM reconstruction, all waves converge at second-order".
+    WENOZ + SSPRK(3,3): Alfven and slow errors fall by >= 2^3.5 per doubling, the fast wave's by 2^1.7 .. 2^3; PPM4 + RK2: second
+    order, below PLM's error at the same resolution.  (Measured rates: Alfven 4.8 / 4.4, slow 5.0, fast 2.5; PPM4 1.6-2.2.)"""
+    for family in ("alfven", "slow", "fast"):
+        e16, e32 = (wave_error(om, family, N, recon=3, nstages=3) for N in (16, 32))
+        rate = math.log2(e16 / e32)
+        if family == "fast":
+            assert 1.7 <= rate <= 3.0, (family, e16, e32)
+        else:
+            assert rate >= 3.5, (family, e16, e32)
+        p16, p32 = (wave_error(om, family, N, recon=1) for N in (16, 32))
+        l32 = wave_error(om, family, 32)
+        assert 1.4 <= math.log2(p16 / p32) <= 2.6 and p32 < l32 and e32 < 0.1 * p32, (family, p16, p32, l32, e32)
+    a32, a64 = (wave_error(om, "alfven", N, recon=3, nstages=3) for N in (32, 64))
+    assert math.log2(a32 / a64) >= 3.5, (a32, a64)
 
 
 @pytest.mark.parametrize("family", ["fast", "alfven", "slow"])
