@@ -155,9 +155,13 @@ def run_mhd(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    mesh, prim, A, B0 = I.mhd_workload(args.workload)
+    if args.recon == "ppmx":
+        raise SystemExit("the MHD path has PLM, PPM4 and WENOZ")
+    recon = {None: 0, "plm": 0, "ppm4": 1, "wenoz": 3}[args.recon]
+    nst = args.integrator
+    mesh, prim, A, B0 = I.mhd_workload(args.workload, ng=3 if recon == 0 else 4)
     U0 = I.make_state_mhd(mesh, prim, A, B0, device=dev)
-    pack = ak_mhd.MhdPack(mesh, I.GAMMA, device=dev)
+    pack = ak_mhd.MhdPack(mesh, I.GAMMA, device=dev, recon=recon, nstages=nst)
     pack.load(U0)
     ncell, state_bytes = mesh.ncells_active, U0.numel() * 8
     sampler = ClockSampler(local)
@@ -175,7 +179,7 @@ def run_mhd(args):
     e0.record(pack.stream)
     for _ in range(args.steps):
         dt = pack.new_dt(I.CFL)
-        for stage in (1, 2):
+        for stage in range(1, nst + 1):
             pack.fill_ghosts()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(pack.stream); pack.stage(stage, dt); b.record(pack.stream)
@@ -187,10 +191,10 @@ def run_mhd(args):
     floors = pack.floor_count()
     elapsed_ms = e0.elapsed_time(e1)
     value = ncell * args.steps / (elapsed_ms * 1e-3)
-    st_ms = {s_: statistics.mean(a.elapsed_time(b) for ss, a, b in stage_ev if ss == s_) for s_ in (1, 2)}
-    stage_ms = (st_ms[1] + st_ms[2]) / 2
+    st_ms = {s_: statistics.mean(a.elapsed_time(b) for ss, a, b in stage_ev if ss == s_) for s_ in range(1, nst + 1)}
+    stage_ms = sum(st_ms.values()) / nst
     peaks, which = measured_peaks()
-    alg = (128.0 + 192.0) / 2 * ncell           # stage 1 reads 8 and writes 8 variables, stage 2 reads 16 and writes 8
+    alg = (128.0 + 192.0 * (nst - 1)) / nst * ncell   # stage 1 reads 8 and writes 8 variables, the later stages read 16 and write 8
     ach = alg / (stage_ms * 1e-3) / 1e9
     host = torch.empty(U0.shape, dtype=torch.float64).pin_memory()
     host.copy_(U0)
@@ -205,12 +209,12 @@ def run_mhd(args):
         "metric": "3D MHD cell-updates/sec (fp64)", "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
-        "config": {"workload": f"{args.workload}: MHD + CT, PLM + HLLD, SSPRK2, {mesh.nmb} MeshBlocks of {mesh.nx[0]}^3, ng 3, Mach-0.5 modes + mean field",
+        "config": {"workload": f"{args.workload}: MHD + CT, {['PLM', 'PPM4', '', 'WENOZ'][recon]} + HLLD, SSPRK{nst}, {mesh.nmb} MeshBlocks of {mesh.nx[0]}^3, ng {mesh.ng}, Mach-0.5 modes + mean field",
                    "cells": ncell, "state_bytes": state_bytes, "l2_policy": "inputs larger than L2" if state_bytes > 4e8 else "state fits L2",
                    "parallelism": "single GPU"},
         "roofline": {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"], "traffic": None,
                      "peak_source": which + " (MEASURED_PEAKS.json hbm_gbs)", "kernel": "akm_stage (six kernels: prim, 3 x flux, emf, update)",
-                     "kernel_ms": stage_ms, "kernel_share_of_step": 2 * stage_ms * args.steps / elapsed_ms, "algorithmic_bytes_per_launch": alg},
+                     "kernel_ms": stage_ms, "kernel_share_of_step": nst * stage_ms * args.steps / elapsed_ms, "algorithmic_bytes_per_launch": alg},
         "cpu_baseline": None, "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "stage_ms": st_ms,
         "floor_activations": floors,
     }))

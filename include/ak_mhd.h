@@ -4,11 +4,12 @@
  * lines 146-150, cited as P:NN), on a MeshBlockPack resident in device memory.  "The magnetic field is discretized
  * as area-averages on cell-faces, and the constrained transport (CT) algorithm of Evans & Hawley (1988) is used to preserve the
  * divergence-free constraint with upwinded electric fields calculated using the method of Gardiner & Stone (2005, 2008)"
- * (P:116); HLLD Riemann solver.  Readings: DESIGN.md Q33-Q37.  Scope of this cut: uniform single-level periodic packs,
- * PLM (van Leer) reconstruction, HLLD, SSPRK(2,2); the kernels are not fused (face fluxes and corner EMFs pass through a
- * caller-owned work buffer in device memory).
+ * (P:116); HLLD Riemann solver.  Readings: DESIGN.md Q33-Q37.  Scope of this cut: uniform single-level periodic packs;
+ * PLM (van Leer), PPM4 or WENOZ reconstruction of the primitives; HLLD; SSPRK(2,2) or SSPRK(3,3) -- the options of the
+ * paper's MHD tests and runs; the kernels are not fused (face fluxes and corner EMFs pass through a caller-owned
+ * work buffer in device memory).
  *
- * One step:   akm_new_dt(p, cfl, &dt);  for stage in 1, 2: { akm_fill_ghosts(p); akm_stage(p, stage, dt); }
+ * One step:   akm_new_dt(p, cfl, &dt);  for stage in 1 .. nstages: { akm_fill_ghosts(p); akm_stage(p, stage, dt); }
  *
  * State layout: U[m][n][k][j][i], n = 0..7 = (rho, rho v1, rho v2, rho v3, E, b1, b2, b3), i fastest, fp64, ng >= 3 ghost
  * layers included; b_d of cell (k,j,i) is the field on the LOWER d-face of that cell.  Memory is caller-owned (device
@@ -40,17 +41,23 @@ int akm_pack_bind(akm_pack*, void* u_a, void* u_b, void* work, void* cuda_stream
  * differ by rounding only (<= 1e-14 per stage in the tests' metric); the upwind switch of the corner EMFs is ramped (DESIGN.md
  * Q36), so a face mass flux at round-off level does not decide a side. */
 int akm_pack_set_exact(akm_pack*, int on);
+/* Reconstruction: 0 PLM (default), 1 PPM4, 3 WENOZ (the codes of ak.h; Q29 for WENOZ); 1 and 3 need ng >= 4 (-1 otherwise);
+ * -3 for any other code. */
+int akm_pack_set_recon(akm_pack*, int recon);
+/* Integrator: 2 = SSPRK(2,2) (default), 3 = SSPRK(3,3); between steps only (-2 inside a step). */
+int akm_pack_set_integrator(akm_pack*, int nstages);
 
 /* Periodic copy of all 8 variables into the ghost cells of the current buffer; bit-exact.  Asynchronous. */
 int akm_fill_ghosts(akm_pack*);
-/* One SSPRK(2,2) stage (stage 1: A -> B; stage 2: B and A -> A): primitives, PLM + HLLD in x1, x2, x3, corner EMFs, flux
+/* One stage (SSPRK(2,2): 1: A -> B, 2: (B, A) -> A; SSPRK(3,3): 1: A -> B, 2: (B, A) -> B, 3: (B, A) -> A): primitives,
+ * reconstruction + HLLD in x1, x2, x3, corner EMFs, flux
  * divergence for the cells and curl of the EMFs for the faces (div B is preserved to round-off).  Needs akm_fill_ghosts
  * on the current buffer first (-2 otherwise).  Asynchronous. */
 int akm_stage(akm_pack*, int stage, double dt);
 /* cfl * min over active cells and d of dx_d / (|v_d| + c_fast,d) (Eq.(3), with the fast magnetosonic speed);
  * dt_out is a HOST pointer; synchronises the stream; -5 for a NaN / inf state. */
 int akm_new_dt(akm_pack*, double cfl, double* dt_out);
-/* akm_new_dt (unless dt_fixed > 0), then the two (fill, stage) pairs; dt_out (HOST, may be NULL) receives the step taken. */
+/* akm_new_dt (unless dt_fixed > 0), then the (fill, stage) pairs of the integrator; dt_out (HOST, may be NULL) receives the step taken. */
 int akm_step(akm_pack*, double cfl, double dt_fixed, double* dt_out);
 void* akm_pack_current(const akm_pack*);        /* device pointer of the buffer holding the latest state             */
 long long akm_pack_floor_count(akm_pack*);      /* floor activations since bind (synchronises); negative on error    */

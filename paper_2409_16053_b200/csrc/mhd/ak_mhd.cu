@@ -180,6 +180,63 @@ __device__ __forceinline__ void plm(double qm1, double q0, double qp1, double& q
   qm = q0 - h; qp = q0 + h;
 }
 
+// PPM4 (the hydro path's reading): fourth-order interface value clamped between its two cells, then Colella &
+// Woodward's (1984) Eq.(1.10) monotonicity constraint on the parabola of cell a with edge values (aL, aR).
+template <bool X>
+__device__ __forceinline__ double ppm4_iface(double qm1, double q0, double qp1, double qp2) {
+  const double n = 7.0 * (q0 + qp1) - (qm1 + qp2);
+  double v;
+  if constexpr (X) v = n / 12.0; else v = n * (1.0 / 12.0);
+  return fmax(fmin(q0, qp1), fmin(v, fmax(q0, qp1)));
+}
+template <bool X>
+__device__ __forceinline__ void ppm4_limit(double a, double aL, double aR, double& qm, double& qp) {
+  if ((aR - a) * (a - aL) <= 0.0) { aL = a; aR = a; }
+  else {
+    const double d = aR - aL, mu = a - 0.5 * (aL + aR), dmu = d * mu;
+    double d26;
+    if constexpr (X) d26 = d * d / 6.0; else d26 = (d * d) * (1.0 / 6.0);
+    if (dmu > d26) aL = 3.0 * a - 2.0 * aR;
+    else if (-d26 > dmu) aR = 3.0 * a - 2.0 * aL;
+  }
+  qm = aL; qp = aR;
+}
+// WENO-Z (Borges et al. 2008; Q29) value at the UPPER face of the middle cell of (a, b, c, d, e), in the differences
+// of neighbouring cells (constants reproduced exactly); the lower-face value is the same function of the mirrored stencil.
+template <bool X>
+__device__ __forceinline__ double wenoz_upper(double a, double b, double c, double d, double e) {
+  const double d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
+  const double P0 = 5.0 * d2 - 2.0 * d1, P1 = 2.0 * d3 + d2, P2 = 4.0 * d3 - d4;
+  const double s0 = d2 - d1, t0 = 3.0 * d2 - d1, s1 = d3 - d2, t1 = d2 + d3, s2 = d4 - d3, t2 = d4 - 3.0 * d3;
+  const double b0 = 13.0 / 12.0 * (s0 * s0) + 0.25 * (t0 * t0);
+  const double b1 = 13.0 / 12.0 * (s1 * s1) + 0.25 * (t1 * t1);
+  const double b2 = 13.0 / 12.0 * (s2 * s2) + 0.25 * (t2 * t2);
+  const double eps = 1e-40, tau = fabs(b0 - b2);
+  const double r0 = div_<X>(tau, b0 + eps), r1 = div_<X>(tau, b1 + eps), r2 = div_<X>(tau, b2 + eps);
+  const double a0 = 0.1 * (1.0 + r0 * r0), a1 = 0.6 * (1.0 + r1 * r1), a2 = 0.3 * (1.0 + r2 * r2);
+  return c + div_<X>(a0 * P0 + (a1 * P1 + a2 * P2), 6.0 * (a0 + (a1 + a2)));
+}
+// left and right state of one primitive at the face between cells cm = c - st and c (RECON: 0 PLM, 1 PPM4, 3 WENOZ)
+template <bool X, int RECON>
+__device__ __forceinline__ void face_states(const double* __restrict__ w, long long c, long long st, double& wl, double& wr) {
+  if constexpr (RECON == 0) {
+    double qm, qp;
+    plm<X>(w[c - 2 * st], w[c - st], w[c], qm, qp); wl = qp;
+    plm<X>(w[c - st], w[c], w[c + st], qm, qp);     wr = qm;
+  } else {
+    const double s0 = w[c - 3 * st], s1 = w[c - 2 * st], s2 = w[c - st], s3 = w[c], s4 = w[c + st], s5 = w[c + 2 * st];
+    if constexpr (RECON == 1) {
+      const double fL = ppm4_iface<X>(s0, s1, s2, s3), fM = ppm4_iface<X>(s1, s2, s3, s4), fR = ppm4_iface<X>(s2, s3, s4, s5);
+      double qm, qp;
+      ppm4_limit<X>(s2, fL, fM, qm, qp); wl = qp;
+      ppm4_limit<X>(s3, fM, fR, qm, qp); wr = qm;
+    } else {
+      wl = wenoz_upper<X>(s0, s1, s2, s3, s4);
+      wr = wenoz_upper<X>(s5, s4, s3, s2, s1);
+    }
+  }
+}
+
 // (k, j, i) of a flat cell index inside one block
 // (32-bit: a block has fewer than 2^31 cells, checked at create; the 64-bit form cost ~250 instructions per thread)
 __device__ __forceinline__ void kji(const Dev& P, long long c, int& k, int& j, int& i) {
@@ -219,26 +276,22 @@ __global__ void __launch_bounds__(256) prim_kernel(Dev P, const double* __restri
 // Occupancy (measured at 256^3): the exact flavour waits on its IEEE division chains and runs best with 32 warps per SM (64
 // registers, 240 B spilled); the fast flavour is bound by the FP64 pipe and runs best without spills (96 registers, 20 warps:
 // 1.49 -> 1.67 G cell-updates/s against 8 CTAs per SM).
-template <int D, bool X>
-__global__ void __launch_bounds__(128, X ? 8 : 5) flux_kernel(Dev P, const double* __restrict__ U) {
+template <int D, bool X, int RECON>
+__global__ void __launch_bounds__(128, X ? 8 : (RECON == 0 ? 5 : 4)) flux_kernel(Dev P, const double* __restrict__ U) {
   constexpr int D1 = (D + 1) % 3, D2 = (D + 2) % 3;
   const int m = blockIdx.y;
   const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= P.ncell) return;
   int idx[3]; kji(P, c, idx[2], idx[1], idx[0]);
-  if (idx[D] < 2 || idx[D] >= P.nt[D] - 2 || idx[D1] >= P.nt[D1] - 1 || idx[D2] >= P.nt[D2] - 1) return;
+  constexpr int R = (RECON == 0) ? 2 : 3;        // cells c-R .. c+R-1 along D must hold W
+  if (idx[D] < R || idx[D] >= P.nt[D] - R || idx[D1] >= P.nt[D1] - 1 || idx[D2] >= P.nt[D2] - 1) return;
   const long long nc = P.ncell, str[3] = {1, P.nt[0], (long long)P.nt[0] * P.nt[1]};
-  const long long st = str[D], cm = c - st;
+  const long long st = str[D];
   const double* Wb = P.W + (long long)m * 8 * nc;
   const int var[7] = {0, 1 + D, 1 + D1, 1 + D2, 4, 5 + D1, 5 + D2};
   double WL[7], WR[7], F[7];
 #pragma unroll
-  for (int q = 0; q < 7; q++) {
-    const double* w = Wb + var[q] * nc;
-    double qm, qp;
-    plm<X>(w[cm - st], w[cm], w[cm + st], qm, qp); WL[q] = qp;
-    plm<X>(w[c - st], w[c], w[c + st], qm, qp);    WR[q] = qm;
-  }
+  for (int q = 0; q < 7; q++) face_states<X, RECON>(Wb + var[q] * nc, c, st, WL[q], WR[q]);
   hlld<X>(P.gamma, U[(long long)m * 8 * nc + (5 + D) * nc + c], WL, WR, F);
   double* Fb = P.F[D] + (long long)m * 7 * nc;
   Fb[c] = F[0]; Fb[(1 + D) * nc + c] = F[1]; Fb[(1 + D1) * nc + c] = F[2]; Fb[(1 + D2) * nc + c] = F[3];
@@ -290,8 +343,9 @@ __global__ void __launch_bounds__(128) emf_kernel(Dev P, double k0, double k1, d
 }
 
 // ---- S4: cells by the flux divergence, faces by the curl of the corner EMFs, with the stage weights ----
-__global__ void __launch_bounds__(128) update_kernel(Dev P, const double* __restrict__ Uin, const double* __restrict__ U0,
-                                                     double* __restrict__ Uout, double g0, double g1, double c1, double c2, double c3) {
+// (U_out may be U_in (SSPRK(3,3) stage 2) or U^n (last stage): every thread reads its own cell before it writes it; no __restrict__)
+__global__ void __launch_bounds__(128) update_kernel(Dev P, const double* Uin, const double* U0, double* Uout,
+                                                     double g0, double g1, double c1, double c2, double c3) {
   const int m = blockIdx.y;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long nact = (long long)P.nx[0] * P.nx[1] * P.nx[2];
@@ -405,6 +459,7 @@ struct akm_pack {
   cudaStream_t stream = nullptr;
   int cur = 0, device = -1;
   bool bound = false, ghosts_ok = false;
+  int recon = 0, nstages = 2;  // akm_pack_set_recon (0 PLM, 1 PPM4, 3 WENOZ), akm_pack_set_integrator (2, 3)
   bool exact = false;          // akm_pack_set_exact: IEEE division / sqrt in the definition's order (bit-identical, slower)
   long long launches = 0;
 };
@@ -508,6 +563,36 @@ extern "C" int akm_pack_set_exact(akm_pack* p, int on) {
   return 0;
 }
 
+extern "C" int akm_pack_set_recon(akm_pack* p, int recon) {
+  if (!p) return fail(-1, "null pack");
+  if (recon != 0 && recon != 1 && recon != 3) return fail(-3, "reconstruction: 0 PLM, 1 PPM4, 3 WENOZ");
+  if (recon != 0 && p->d.ng < 4) return fail(-1, "PPM4 / WENOZ with face-centred fields need ng >= 4");
+  p->recon = recon;
+  return 0;
+}
+extern "C" int akm_pack_set_integrator(akm_pack* p, int nstages) {
+  if (!p) return fail(-1, "null pack");
+  if (nstages != 2 && nstages != 3) return fail(-3, "integrator: 2 = SSPRK(2,2), 3 = SSPRK(3,3)");
+  if (p->cur != 0) return fail(-2, "the integrator can only change between steps");
+  p->nstages = nstages;
+  return 0;
+}
+
+namespace {
+template <bool X, int RECON>
+void launch_sweeps(const akm_pack* p, dim3 grid, const double* Uin) {
+  flux_kernel<0, X, RECON><<<grid, 128, 0, p->stream>>>(p->d, Uin);
+  flux_kernel<1, X, RECON><<<grid, 128, 0, p->stream>>>(p->d, Uin);
+  flux_kernel<2, X, RECON><<<grid, 128, 0, p->stream>>>(p->d, Uin);
+}
+template <bool X>
+void launch_sweeps_recon(const akm_pack* p, dim3 grid, const double* Uin) {
+  if (p->recon == 1) launch_sweeps<X, 1>(p, grid, Uin);
+  else if (p->recon == 3) launch_sweeps<X, 3>(p, grid, Uin);
+  else launch_sweeps<X, 0>(p, grid, Uin);
+}
+}  // namespace
+
 extern "C" int akm_fill_ghosts(akm_pack* p) {
   if (!p || !p->bound) return fail(-2, "pack not bound");
   Guard guard(p->device);
@@ -522,36 +607,34 @@ extern "C" int akm_fill_ghosts(akm_pack* p) {
 
 extern "C" int akm_stage(akm_pack* p, int stage, double dt) {
   if (!p || !p->bound) return fail(-2, "pack not bound");
-  if (stage < 1 || stage > 2) return fail(-1, "stage must be 1 or 2");
+  const int ns = p->nstages;
+  if (stage < 1 || stage > ns) return fail(-1, "stage must be 1 .. number of stages of the integrator");
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(-1, "dt must be positive and finite");
-  if (p->cur != stage - 1) return fail(-2, "stages must be called in order, starting from U^n in buffer A");
+  if (p->cur != (stage == 1 ? 0 : 1)) return fail(-2, "stages must be called in order, starting from U^n in buffer A");
   if (!p->ghosts_ok) return fail(-2, "akm_fill_ghosts must precede akm_stage");
   Guard guard(p->device);
-  static const double C2[2][3] = {{0.0, 1.0, 1.0}, {0.5, 0.5, 0.5}};        // SSPRK(2,2), Q1
-  const double g0 = C2[stage - 1][0], g1 = C2[stage - 1][1], beta = C2[stage - 1][2];
+  // U_out = g0 U_in + g1 U^n - beta dt L(U_in).  SSPRK(2,2): A -> B, (B, A) -> A.  SSPRK(3,3): A -> B, (B, A) -> B in place
+  // (the update is pointwise once the fluxes and EMFs are in the work buffer), (B, A) -> A.  DESIGN.md Q1
+  static const double C2[2][3] = {{0.0, 1.0, 1.0}, {0.5, 0.5, 0.5}};
+  static const double C3[3][3] = {{0.0, 1.0, 1.0}, {0.25, 0.75, 0.25}, {2.0 / 3.0, 1.0 / 3.0, 2.0 / 3.0}};
+  const double* cf = (ns == 2) ? C2[stage - 1] : C3[stage - 1];
+  const double g0 = cf[0], g1 = cf[1], beta = cf[2];
+  const int out = (stage == ns) ? 0 : 1;
   const Dev& d = p->d;
   const double* Uin = p->u[p->cur];
-  double* Uout = p->u[stage == 2 ? 0 : 1];
+  double* Uout = p->u[out];
   dim3 gall256((unsigned)((d.ncell + 255) / 256), (unsigned)d.nmb), gall128((unsigned)((d.ncell + 127) / 128), (unsigned)d.nmb);
   const long long nact = (long long)d.nx[0] * d.nx[1] * d.nx[2];
   dim3 gact((unsigned)((nact + 127) / 128), (unsigned)d.nmb);
   prim_kernel<<<gall256, 256, 0, p->stream>>>(d, Uin);
-  if (p->exact) {
-    flux_kernel<0, true><<<gall128, 128, 0, p->stream>>>(d, Uin);
-    flux_kernel<1, true><<<gall128, 128, 0, p->stream>>>(d, Uin);
-    flux_kernel<2, true><<<gall128, 128, 0, p->stream>>>(d, Uin);
-  } else {
-    flux_kernel<0, false><<<gall128, 128, 0, p->stream>>>(d, Uin);
-    flux_kernel<1, false><<<gall128, 128, 0, p->stream>>>(d, Uin);
-    flux_kernel<2, false><<<gall128, 128, 0, p->stream>>>(d, Uin);
-  }
+  if (p->exact) launch_sweeps_recon<true>(p, gall128, Uin); else launch_sweeps_recon<false>(p, gall128, Uin);
   const double k0 = 1024.0 * dt / d.dx[0], k1 = 1024.0 * dt / d.dx[1], k2 = 1024.0 * dt / d.dx[2];
   if (p->exact) emf_kernel<true><<<gall128, 128, 0, p->stream>>>(d, k0, k1, k2);
   else emf_kernel<false><<<gall128, 128, 0, p->stream>>>(d, k0, k1, k2);
   update_kernel<<<gact, 128, 0, p->stream>>>(d, Uin, p->u[0], Uout, g0, g1, beta * dt / d.dx[0], beta * dt / d.dx[1], beta * dt / d.dx[2]);
   AKM_CUDA(cudaGetLastError(), "akm_stage launch");
   p->launches += 6;
-  p->cur = (stage == 2) ? 0 : 1;
+  p->cur = out;
   p->ghosts_ok = false;
   return 0;
 }
@@ -581,7 +664,7 @@ extern "C" int akm_new_dt(akm_pack* p, double cfl, double* dt_out) {
 extern "C" int akm_step(akm_pack* p, double cfl, double dt_fixed, double* dt_out) {
   double dt = dt_fixed;
   if (!(dt_fixed > 0.0)) { int rc = akm_new_dt(p, cfl, &dt); if (rc) return rc; }
-  for (int stage = 1; stage <= 2; stage++) {
+  for (int stage = 1; stage <= p->nstages; stage++) {
     int rc = akm_fill_ghosts(p); if (rc) return rc;
     rc = akm_stage(p, stage, dt); if (rc) return rc;
   }

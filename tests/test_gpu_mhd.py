@@ -59,9 +59,9 @@ def turbulent_state(mesh, mach=0.5):
     return I.make_state_mhd(mesh, prim, A, (0.4, -0.3, 0.2))
 
 
-def lockstep(om, akm, mesh, U0, gamma, nsteps, cfl=0.3, exact=False):
-    po = om.OrcMhdPack(mesh, gamma, threads=P.NTHREADS)
-    pg = akm.MhdPack(mesh, gamma, exact=exact)
+def lockstep(om, akm, mesh, U0, gamma, nsteps, cfl=0.3, exact=False, recon=0, nstages=2):
+    po = om.OrcMhdPack(mesh, gamma, threads=P.NTHREADS, recon=recon, nstages=nstages)
+    pg = akm.MhdPack(mesh, gamma, exact=exact, recon=recon, nstages=nstages)
     po.load(U0.numpy())
     pg.load(U0)
     a = act(mesh)
@@ -70,7 +70,7 @@ def lockstep(om, akm, mesh, U0, gamma, nsteps, cfl=0.3, exact=False):
         dt = po.new_dt(cfl)
         dtg = pg.new_dt(cfl)
         assert abs(dtg - dt) <= 1e-13 * dt, (step, dt, dtg)
-        for stage in (1, 2):
+        for stage in range(1, nstages + 1):
             po.fill_ghosts(); pg.fill_ghosts()
             if step == 0:
                 ug = pg.current().cpu().numpy()
@@ -114,6 +114,30 @@ def test_turbulent_field_matches_the_oracle(om, akm, nrb, nx, exact):
         p2.step(0.3)
     assert q_mhd(p2.current().cpu().numpy()[a], po.current()[a], G53) <= TOL_RUN
     assert p2.launch_count() == nst * (2 + 2 * 7)                          # dt_init + dt + 2 x (fill + 6 stage kernels) per step
+
+
+@pytest.mark.parametrize("exact", [False, True])
+@pytest.mark.parametrize("recon,nstages", [(1, 2), (3, 2), (3, 3), (0, 3)])
+@pytest.mark.parametrize("nrb,nx", [((2, 2, 2), (16, 16, 16)), ((2, 1, 3), (24, 10, 6))])
+def test_higher_order_options_match_the_oracle(om, akm, nrb, nx, recon, nstages, exact):
+    """PPM4 / WENOZ reconstruction and SSPRK(3,3) (the options of the paper's MHD tests and runs; ng = 4): same bars as
+    the PLM + RK2 path, bit-identical in the verification flavour."""
+    mesh = I.uniform_mesh(nrb, nx, 4)
+    U0 = turbulent_state(mesh)
+    errs, po, pg = lockstep(om, akm, mesh, U0, G53, 4, exact=exact, recon=recon, nstages=nstages)
+    name = f"{['PLM', 'PPM4', '', 'WENOZ'][recon]} + SSPRK{nstages}"
+    P.report(f"[parity] MHD {name} nmb={mesh.nmb} nx={nx} exact={exact}: worst per step {max(errs):.3e} (bar {TOL_RUN:.0e}), first step {errs[0]:.3e}")
+    assert max(errs) <= TOL_RUN and (max(errs) == 0.0 or not exact)
+    pg.fill_ghosts()
+    ug = pg.current().cpu().numpy()
+    assert np.abs(divb(mesh, ug)).max() <= 2e-13
+    a = act(mesh)
+    for n in range(8):
+        scale = np.abs(U0.numpy()[a][:, n]).sum() + 1.0
+        assert abs(ug[a][:, n].sum() - U0.numpy()[a][:, n].sum()) <= 1e-12 * scale, n
+    assert pg.launch_count() == 4 * (2 + nstages * 7) + 1                  # (+ the fill above)
+    with pytest.raises(akm.AkmError):
+        akm.MhdPack(I.uniform_mesh((1, 1, 1), (8, 8, 8), 3), G53, recon=recon or 1)   # ng < 4
 
 
 @pytest.mark.parametrize("exact", [False, True])
