@@ -2,7 +2,7 @@
 // citations and pins).  Plain loops, fp64, compiled -O2 -ffp-contract=off -fno-fast-math.  P:NN = /root/reference/PAPER.md
 // line NN; Qnn = readings listed in DESIGN.md.
 #include "orc_mhd.h"
-#include "orc.h"       // orc_ppm4, orc_wenoz: the hydro oracle's reconstruction functions (same oracle, linked in)
+#include "orc.h"       // orc_ppm4, orc_ppmx, orc_wenoz: the hydro oracle's reconstruction functions (same oracle, linked in)
 
 #include <cmath>
 #include <cstdio>
@@ -111,7 +111,7 @@ struct orcm_pack {
   std::vector<int> lx, leaf;             // lx[3m+d]; leaf[(l3*nrb2+l2)*nrb1+l1] -> m
   double* u[2] = { nullptr, nullptr };
   int cur = 0, nthreads = 1;
-  int recon = 0;                         // 0 PLM, 1 PPM4, 3 WENOZ (the hydro oracle's codes and functions: oracle/orc.h)
+  int recon = 0;                         // 0 PLM, 1 PPM4, 2 PPMX, 3 WENOZ (the hydro oracle's codes and functions: oracle/orc.h)
   int nstages = 2;                       // 2: SSPRK(2,2), 3: SSPRK(3,3) (Q1)
   bool bound = false;
   long long floor_count = 0;
@@ -245,6 +245,7 @@ static long long block_stage(const orcm_pack* p, const double* Uin, const double
           const double sL[5] = { w[cm - 2 * str[d]], w[cm - str[d]], w[cm], w[cm + str[d]], w[cm + 2 * str[d]] };
           const double sR[5] = { w[c - 2 * str[d]], w[c - str[d]], w[c], w[c + str[d]], w[c + 2 * str[d]] };
           if (p->recon == 1) { orc_ppm4(sL, &qm, &qp); WL[q] = qp; orc_ppm4(sR, &qm, &qp); WR[q] = qm; }
+          else if (p->recon == 2) { orc_ppmx(sL, &qm, &qp); WL[q] = qp; orc_ppmx(sR, &qm, &qp); WR[q] = qm; }
           else               { orc_wenoz(sL, &qm, &qp); WL[q] = qp; orc_wenoz(sR, &qm, &qp); WR[q] = qm; }
         }
       }
@@ -307,8 +308,8 @@ static long long block_stage(const orcm_pack* p, const double* Uin, const double
 // WENOZ, PPM4, PLM on the linear waves; WENOZ + RK2 + HLLD for the turbulence run)
 extern "C" int orcm_pack_set_recon(orcm_pack* p, int recon) {
   if (!p) return fail("null pack");
-  if (recon != 0 && recon != 1 && recon != 3) return fail("reconstruction: 0 PLM, 1 PPM4, 3 WENOZ");
-  if (recon != 0 && p->ng < 4) return fail("PPM4 / WENOZ with face-centred fields need ng >= 4");
+  if (recon < 0 || recon > 3) return fail("reconstruction: 0 PLM, 1 PPM4, 2 PPMX, 3 WENOZ");
+  if (recon != 0 && p->ng < 4) return fail("PPM4 / PPMX / WENOZ with face-centred fields need ng >= 4");
   p->recon = recon;
   return 0;
 }

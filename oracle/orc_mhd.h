@@ -7,7 +7,7 @@
  * the constrained transport (CT) algorithm of Evans & Hawley (1988) is used to preserve the divergence-free constraint with
  * upwinded electric fields calculated using the method of Gardiner & Stone (2005, 2008)"; HLLD is the solver of its
  * MHD run; all MHD waves converge at second order with PLM.  The formulas are deferred to those papers; the
- * readings taken are DESIGN.md Q33-Q37.  Scope: uniform single-level periodic packs; PLM (van Leer), PPM4 or WENOZ (the hydro
+ * readings taken are DESIGN.md Q33-Q37.  Scope: uniform single-level periodic packs; PLM (van Leer), PPM4, PPMX or WENOZ (the hydro
  * oracle's functions, orc.h) on the primitives (rho, v, u_g, B_t); HLLD; SSPRK(2,2) or SSPRK(3,3).
  *
  * Layout: U[m][n][k][j][i], n = 0..7 = (rho, rho v1, rho v2, rho v3, E, b1, b2, b3), i fastest, ghosts included, ng >= 3;
@@ -35,7 +35,7 @@ orcm_pack* orcm_pack_create(int nmb, int nx1, int nx2, int nx3, int ng, double g
                             const int* lx, const double xmin[3], const double xmax[3]);
 int orcm_pack_bind(orcm_pack*, double* u_a, double* u_b);   /* u_a holds U^n; both of nmb*8*nt1*nt2*nt3 doubles */
 int orcm_set_threads(orcm_pack*, int nthreads);
-int orcm_pack_set_recon(orcm_pack*, int recon);              /* 0 PLM (default), 1 PPM4, 3 WENOZ (orc.h's functions); ng >= 4 for 1, 3 */
+int orcm_pack_set_recon(orcm_pack*, int recon);              /* 0 PLM (default), 1 PPM4, 2 PPMX, 3 WENOZ (orc.h's functions); ng >= 4 for 1-3 */
 int orcm_pack_set_integrator(orcm_pack*, int nstages);      /* 2 = SSPRK(2,2) (default), 3 = SSPRK(3,3) */
 int orcm_fill_ghosts(orcm_pack*);                           /* periodic copy of all 8 variables into the ghost cells */
 int orcm_stage(orcm_pack*, int stage, double dt);           /* one stage: RK2 1: A -> B, 2: (B, A) -> A; RK3 2: (B, A) -> B, 3: (B, A) -> A */
