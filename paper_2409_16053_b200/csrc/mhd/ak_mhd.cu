@@ -201,6 +201,43 @@ __device__ __forceinline__ void ppm4_limit(double a, double aL, double aR, doubl
   }
   qm = aL; qp = aR;
 }
+// PPMX (Q30; Colella & Sekora 2008 / McCorquodale & Colella 2011, restated): fourth-order interface value, replaced
+// where it is not between its two cells by (q0 + q1)/2 - D/6 with D the second difference limited among the face-centred one
+// and C = 5/4 times the two cell-centred ones; ...
+template <bool X>
+__device__ __forceinline__ double ppmx_iface(double qm1, double q0, double q1, double q2) {
+  const double C = 1.25, n = 7.0 * (q0 + q1) - (qm1 + q2);
+  double v;
+  if constexpr (X) v = n / 12.0; else v = n * (1.0 / 12.0);
+  if ((v - q0) * (q1 - v) < 0.0) {
+    const double dc = 3.0 * ((q0 + q1) - 2.0 * v), dl = (qm1 + q1) - 2.0 * q0, dr = (q0 + q2) - 2.0 * q1;
+    double D = 0.0;
+    if (dc > 0.0 && dl > 0.0 && dr > 0.0) D = fmin(dc, C * fmin(dl, dr));
+    else if (dc < 0.0 && dl < 0.0 && dr < 0.0) D = -fmin(-dc, C * fmin(-dl, -dr));
+    if constexpr (X) v = 0.5 * (q0 + q1) - D / 6.0; else v = 0.5 * (q0 + q1) - D * (1.0 / 6.0);
+  }
+  return v;
+}
+// ... and the parabola of the cell q2 of (q0 .. q4) with edge values (aL, aR): at an extremum its second derivative is limited
+// among itself and C times the three cell-centred second differences and both edge increments are scaled by the ratio (kept when
+// the ratio >= 1 - 1e-12); elsewhere an edge increment is at most twice the other.
+template <bool X>
+__device__ __forceinline__ void ppmx_limit(double q0, double q1, double q2, double q3, double q4, double aL, double aR, double& qm, double& qp) {
+  const double C = 1.25, a = q2, dm = a - aL, dp = aR - a;
+  if (dm * dp <= 0.0 || (q3 - a) * (a - q1) <= 0.0) {
+    const double df = 6.0 * ((aL + aR) - 2.0 * a);
+    const double d1 = (q0 + q2) - 2.0 * q1, d2 = (q1 + q3) - 2.0 * q2, d3 = (q2 + q4) - 2.0 * q3;
+    double D = 0.0;
+    if (df > 0.0 && d1 > 0.0 && d2 > 0.0 && d3 > 0.0) D = fmin(df, C * fmin(d1, fmin(d2, d3)));
+    else if (df < 0.0 && d1 < 0.0 && d2 < 0.0 && d3 < 0.0) D = -fmin(-df, C * fmin(-d1, fmin(-d2, -d3)));
+    const double rho = (df != 0.0) ? div_<X>(D, df) : 0.0;
+    if (rho <= 1.0 - 1e-12) { aL = a - rho * dm; aR = a + rho * dp; }
+  } else {
+    if (fabs(dm) >= 2.0 * fabs(dp)) aL = a - 2.0 * dp;
+    if (fabs(dp) >= 2.0 * fabs(dm)) aR = a + 2.0 * dm;
+  }
+  qm = aL; qp = aR;
+}
 // WENO-Z (Borges et al. 2008; Q29) value at the UPPER face of the middle cell of (a, b, c, d, e), in the differences
 // of neighbouring cells (constants reproduced exactly); the lower-face value is the same function of the mirrored stencil.
 template <bool X>
@@ -216,7 +253,7 @@ __device__ __forceinline__ double wenoz_upper(double a, double b, double c, doub
   const double a0 = 0.1 * (1.0 + r0 * r0), a1 = 0.6 * (1.0 + r1 * r1), a2 = 0.3 * (1.0 + r2 * r2);
   return c + div_<X>(a0 * P0 + (a1 * P1 + a2 * P2), 6.0 * (a0 + (a1 + a2)));
 }
-// left and right state of one primitive at the face between cells cm = c - st and c (RECON: 0 PLM, 1 PPM4, 3 WENOZ)
+// left and right state of one primitive at the face between cells cm = c - st and c (RECON: 0 PLM, 1 PPM4, 2 PPMX, 3 WENOZ)
 template <bool X, int RECON>
 __device__ __forceinline__ void face_states(const double* __restrict__ w, long long c, long long st, double& wl, double& wr) {
   if constexpr (RECON == 0) {
@@ -230,6 +267,11 @@ __device__ __forceinline__ void face_states(const double* __restrict__ w, long l
       double qm, qp;
       ppm4_limit<X>(s2, fL, fM, qm, qp); wl = qp;
       ppm4_limit<X>(s3, fM, fR, qm, qp); wr = qm;
+    } else if constexpr (RECON == 2) {
+      const double fL = ppmx_iface<X>(s0, s1, s2, s3), fM = ppmx_iface<X>(s1, s2, s3, s4), fR = ppmx_iface<X>(s2, s3, s4, s5);
+      double qm, qp;
+      ppmx_limit<X>(s0, s1, s2, s3, s4, fL, fM, qm, qp); wl = qp;
+      ppmx_limit<X>(s1, s2, s3, s4, s5, fM, fR, qm, qp); wr = qm;
     } else {
       wl = wenoz_upper<X>(s0, s1, s2, s3, s4);
       wr = wenoz_upper<X>(s5, s4, s3, s2, s1);
@@ -473,7 +515,7 @@ struct akm_pack {
   cudaStream_t stream = nullptr;
   int cur = 0, device = -1;
   bool bound = false, ghosts_ok = false;
-  int recon = 0, nstages = 2;  // akm_pack_set_recon (0 PLM, 1 PPM4, 3 WENOZ), akm_pack_set_integrator (2, 3)
+  int recon = 0, nstages = 2;  // akm_pack_set_recon (0 PLM, 1 PPM4, 2 PPMX, 3 WENOZ), akm_pack_set_integrator (2, 3)
   bool exact = false;          // akm_pack_set_exact: IEEE division / sqrt in the definition's order (bit-identical, slower)
   long long launches = 0;
 };
@@ -579,8 +621,8 @@ extern "C" int akm_pack_set_exact(akm_pack* p, int on) {
 
 extern "C" int akm_pack_set_recon(akm_pack* p, int recon) {
   if (!p) return fail(-1, "null pack");
-  if (recon != 0 && recon != 1 && recon != 3) return fail(-3, "reconstruction: 0 PLM, 1 PPM4, 3 WENOZ");
-  if (recon != 0 && p->d.ng < 4) return fail(-1, "PPM4 / WENOZ with face-centred fields need ng >= 4");
+  if (recon < 0 || recon > 3) return fail(-3, "reconstruction: 0 PLM, 1 PPM4, 2 PPMX, 3 WENOZ");
+  if (recon != 0 && p->d.ng < 4) return fail(-1, "PPM4 / PPMX / WENOZ with face-centred fields need ng >= 4");
   p->recon = recon;
   return 0;
 }
@@ -602,6 +644,7 @@ void launch_sweeps(const akm_pack* p, dim3 grid, const double* Uin) {
 template <bool X>
 void launch_sweeps_recon(const akm_pack* p, dim3 grid, const double* Uin) {
   if (p->recon == 1) launch_sweeps<X, 1>(p, grid, Uin);
+  else if (p->recon == 2) launch_sweeps<X, 2>(p, grid, Uin);
   else if (p->recon == 3) launch_sweeps<X, 3>(p, grid, Uin);
   else launch_sweeps<X, 0>(p, grid, Uin);
 }

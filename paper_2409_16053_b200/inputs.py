@@ -359,7 +359,7 @@ def make_state_mhd(mesh: Mesh, prim_fn: PrimFn, A_fn, B0=(0.0, 0.0, 0.0), gamma:
 def mhd_workload(name: str, ng: int = 3):
     """MHD workloads of bench.py and the full-size GPU test: the seeded Mach-0.5 random-mode velocity field and
     5 % density modes of the hydro configs, P = 1, a tangled field from a vector potential plus a mean field, on a uniform periodic
-    pack of 8 MeshBlocks, ng = 3 (4 for PPM4 / WENOZ).  -> (mesh, prim_fn, A_fn, B0) for make_state_mhd."""
+    pack of 8 MeshBlocks, ng = 3 (4 for PPM4 / PPMX / WENOZ).  -> (mesh, prim_fn, A_fn, B0) for make_state_mhd."""
     nrb, nx = {"mhd_256": (2, 128), "mhd_128": (2, 64), "mhd_64": (2, 32)}[name]
     mesh = uniform_mesh((nrb,) * 3, (nx,) * 3, ng)
     rm = RandomModes.draw(0.5)

@@ -45,17 +45,22 @@ def q_mhd(Ug, Uo, gamma):
     return float(e.max())
 
 
-def turbulent_state(mesh, mach=0.5):
+def turbulent_state(mesh, mach=0.5, shift=(0.0, 0.0, 0.0)):
+    """Smooth 3-D field with a tangled magnetic field.  Unshifted it has planes of exact symmetry on the grid (a velocity that vanishes
+    on a plane of cell centres: the case the ramped upwind switch of Q36 exists for); `shift` moves the pattern off the grid."""
     k = 2 * math.pi
 
     def A(X1, X2, X3):
+        X1, X2, X3 = X1 + shift[0], X2 + shift[1], X3 + shift[2]
         return (0.1 * torch.sin(k * X2) * torch.cos(2 * k * X3) + 0 * X1, 0.1 * torch.sin(k * X3 + 0.3) * torch.cos(k * X1) + 0 * X2,
                 0.1 * torch.cos(2 * k * X1 + 0.7) * torch.sin(k * X2) + 0 * X3)
 
-    prim = lambda X1, X2, X3: (1.0 + 0.3 * torch.sin(k * X1) * torch.cos(k * X2) + 0 * X3,
-                               mach * torch.sin(k * X2 + 0.2) * torch.cos(k * X3) + 0 * X1,
-                               -mach * torch.cos(k * X3) * torch.sin(2 * k * X1) + 0 * X2,
-                               mach * torch.sin(k * X1 + 1.0) * torch.sin(k * X2) + 0 * X3, 0.6 + 0 * X1 + 0 * X2 + 0 * X3)
+    def prim(X1, X2, X3):
+        X1, X2, X3 = X1 + shift[0], X2 + shift[1], X3 + shift[2]
+        return (1.0 + 0.3 * torch.sin(k * X1) * torch.cos(k * X2) + 0 * X3,
+                mach * torch.sin(k * X2 + 0.2) * torch.cos(k * X3) + 0 * X1,
+                -mach * torch.cos(k * X3) * torch.sin(2 * k * X1) + 0 * X2,
+                mach * torch.sin(k * X1 + 1.0) * torch.sin(k * X2) + 0 * X3, 0.6 + 0 * X1 + 0 * X2 + 0 * X3)
     return I.make_state_mhd(mesh, prim, A, (0.4, -0.3, 0.2))
 
 
@@ -117,15 +122,19 @@ def test_turbulent_field_matches_the_oracle(om, akm, nrb, nx, exact):
 
 
 @pytest.mark.parametrize("exact", [False, True])
-@pytest.mark.parametrize("recon,nstages", [(1, 2), (3, 2), (3, 3), (0, 3)])
+@pytest.mark.parametrize("recon,nstages", [(1, 2), (2, 3), (3, 2), (3, 3), (0, 3)])
 @pytest.mark.parametrize("nrb,nx", [((2, 2, 2), (16, 16, 16)), ((2, 1, 3), (24, 10, 6))])
 def test_higher_order_options_match_the_oracle(om, akm, nrb, nx, recon, nstages, exact):
-    """PPM4 / WENOZ reconstruction and SSPRK(3,3) (the options of the paper's MHD tests and runs; ng = 4): same bars as
+    """PPM4 / PPMX / WENOZ reconstruction and SSPRK(3,3) (the options of the paper's MHD tests and runs; ng = 4): same bars as
     the PLM + RK2 path, bit-identical in the verification flavour."""
     mesh = I.uniform_mesh(nrb, nx, 4)
-    U0 = turbulent_state(mesh)
+    # PPMX switches between its extremum and its monotone limiter where two neighbouring cells are equal: a discontinuous function of
+    # the data there (Q30), so a field with exact mirror symmetries on the grid lets 1 ulp decide O(1e-7) -- in the default flavour
+    # the pattern is moved off the grid for it; the verification flavour takes the symmetric field (bit-identical either way)
+    shift = (0.0137, 0.0291, 0.0173) if (recon == 2 and not exact) else (0.0, 0.0, 0.0)
+    U0 = turbulent_state(mesh, shift=shift)
     errs, po, pg = lockstep(om, akm, mesh, U0, G53, 4, exact=exact, recon=recon, nstages=nstages)
-    name = f"{['PLM', 'PPM4', '', 'WENOZ'][recon]} + SSPRK{nstages}"
+    name = f"{['PLM', 'PPM4', 'PPMX', 'WENOZ'][recon]} + SSPRK{nstages}"
     P.report(f"[parity] MHD {name} nmb={mesh.nmb} nx={nx} exact={exact}: worst per step {max(errs):.3e} (bar {TOL_RUN:.0e}), first step {errs[0]:.3e}")
     assert max(errs) <= TOL_RUN and (max(errs) == 0.0 or not exact)
     pg.fill_ghosts()
@@ -182,7 +191,7 @@ def test_brio_wu_with_the_higher_order_options_on_the_gpu(om, akm, recon, nstage
             e40 = q_mhd(pg.current().cpu().numpy()[a], po.current()[a], 2.0)
     ug = pg.current().cpu().numpy()[a]
     e = q_mhd(ug, po.current()[a], 2.0)
-    P.report(f"[parity] MHD Brio-Wu 2 x 200 cells, {['PLM', 'PPM4', '', 'WENOZ'][recon]} + SSPRK{nstages}, exact={exact}: after 40 steps {e40:.3e} (bar {TOL_RUN:.0e}), after {n} steps {e:.3e}")
+    P.report(f"[parity] MHD Brio-Wu 2 x 200 cells, {['PLM', 'PPM4', 'PPMX', 'WENOZ'][recon]} + SSPRK{nstages}, exact={exact}: after 40 steps {e40:.3e} (bar {TOL_RUN:.0e}), after {n} steps {e:.3e}")
     assert n > 40 and e40 <= TOL_RUN and e <= 1e-6 and (e == 0.0 or not exact)
     assert pg.floor_count() == 0 and po.floor_count() == 0 and np.isfinite(ug).all()
     assert ug[0, 0].min() > 0.1 and ug[0, 0].max() <= 1.0 + 1e-12            # density stays within the initial bounds
