@@ -303,3 +303,48 @@ def test_mhd_256_full_size_sampled(om, akm):
         assert e <= 2 * nsteps * TOL_STAGE, (o, e)
         po.close()
     P.report(f"[parity] MHD mhd_256 full size (8 x 128^3, bench launch configuration): worst sampled difference after {nsteps} steps = {worst:.2e}")
+
+
+def _gpu_wave_error(akm, family, N, recon, nstages, amp=1e-6):
+    """L1 error of a 1-D linear MHD wave after one period on the CUDA path alone (the eigenvector comes from numpy, the reference is
+    the initial state): a property of the scheme that needs no oracle."""
+    from tests.test_oracle_mhd import mhd_eigenmode
+    speed, R, (r0, p0, bx, by0, bz0) = mhd_eigenmode(family)
+    mesh = I.uniform_mesh((1, 1, 1), (N, 4, 4), 4)
+    k = 2 * math.pi
+
+    def prim(X1, X2, X3):
+        s = torch.sin(k * X1) + 0 * X2 + 0 * X3
+        return (r0 + amp * R[0] * s, amp * R[1] * s, amp * R[2] * s, amp * R[3] * s, p0 + amp * R[4] * s)
+
+    def A(X1, X2, X3):
+        c = torch.cos(k * X1) / k + 0 * X2 + 0 * X3
+        return (0 * c, -amp * R[6] * c, amp * R[5] * c)
+
+    U0 = I.make_state_mhd(mesh, prim, A, (bx, by0, bz0))
+    pg = akm.MhdPack(mesh, G53, recon=recon, nstages=nstages)
+    pg.load(U0)
+    t, tend = 0.0, 1.0 / speed
+    while t < tend:
+        dt = min(pg.new_dt(0.3), tend - t)
+        pg.step(0.3, dt)
+        t += dt
+    a = act(mesh)
+    U = pg.current().cpu().numpy()
+    assert pg.floor_count() == 0
+    return math.sqrt(sum(np.abs(U[a][0, n] - U0.numpy()[a][0, n]).mean() ** 2 for n in range(8)))
+
+
+def test_the_papers_mhd_convergence_orders_on_the_gpu(akm):
+    """P:152 on the CUDA path itself (default arithmetic): RK3 + WENOZ and RK3 + PPMX converge at fourth order on the Alfven and slow
+    waves, the fast wave at second order; PLM + RK2 at second order."""
+    for family in ("alfven", "slow"):
+        for recon in (3, 2):
+            e16, e32 = (_gpu_wave_error(akm, family, N, recon, 3) for N in (16, 32))
+            assert math.log2(e16 / e32) >= 3.5, (family, recon, e16, e32)
+    f16, f32 = (_gpu_wave_error(akm, "fast", N, 3, 3) for N in (16, 32))
+    assert 1.7 <= math.log2(f16 / f32) <= 3.0, (f16, f32)
+    p32, p64 = (_gpu_wave_error(akm, "alfven", N, 0, 2) for N in (32, 64))
+    assert 1.6 <= math.log2(p32 / p64) <= 2.4, (p32, p64)
+    P.report(f"[property] MHD linear waves on the GPU: WENOZ + RK3 fast-wave rate {math.log2(f16 / f32):.2f}, PLM + RK2 Alfven rate {math.log2(p32 / p64):.2f}; "
+             f"Alfven / slow with WENOZ / PPMX + RK3 >= 3.5")
