@@ -215,6 +215,13 @@ def test_uniform_state_dt_and_errors_on_the_gpu(om, akm):
     pg.fill_ghosts()
     with pytest.raises(akm.AkmError):
         pg.stage(2, 1e-3)                                                # stage 2 before stage 1
+    pg.stage(1, 1e-3)
+    assert akm.lib().akm_pack_set_integrator(pg._h, 3) == -2             # the integrator cannot change inside a step
+    assert akm.lib().akm_pack_set_recon(pg._h, 7) == -3 and akm.lib().akm_pack_set_recon(pg._h, 3) == -1   # unknown code; ng = 3
+    pg.fill_ghosts(); pg.stage(2, 1e-3)
+    assert akm.lib().akm_pack_set_integrator(pg._h, 3) == 0
+    with pytest.raises(akm.AkmError):
+        pg.fill_ghosts(); pg.stage(1, 1e-3); pg.fill_ghosts(); pg.stage(2, 1e-3); pg.fill_ghosts(); pg.stage(3, 1e-3); pg.stage(1, 1e-3)   # ghosts not refilled
     bad = U0.clone()
     bad[0, 2, 4, 5, 6] = float("nan")
     pg.load(bad)
