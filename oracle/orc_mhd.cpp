@@ -113,6 +113,7 @@ struct orcm_pack {
   int cur = 0, nthreads = 1;
   int recon = 0;                         // 0 PLM, 1 PPM4, 2 PPMX, 3 WENOZ (the hydro oracle's codes and functions: oracle/orc.h)
   int nstages = 2;                       // 2: SSPRK(2,2), 3: SSPRK(3,3) (Q1)
+  int rsolver = 0;                       // 0 HLLD, 1 LLF, 2 HLLE
   bool bound = false;
   long long floor_count = 0;
   size_t ncell() const { return (size_t)nt[0] * nt[1] * nt[2]; }
@@ -178,6 +179,27 @@ extern "C" int orcm_fill_ghosts(orcm_pack* p) {
       for (int n = 0; n < 8; n++) U[p->idx(m, n, k, j, i)] = U[p->idx(src, n, s[2], s[1], s[0])];
     }
   return 0;
+}
+
+// LLF and HLLE for MHD ("the local Lax-Friedrichs (LLF) method, various versions of the Harten-Lax-van Leer method"), in
+// the same rotated variables.  LLF: F = (F_L + F_R)/2 - (lambda/2)(U_R - U_L), lambda = max(|u_L| + cf_L, |u_R| + cf_R).
+// HLLE: the single-state HLL flux between the outer speeds of HLLD (Eq. 67 above), b- = min(S_L, 0), b+ = max(S_R, 0),
+// F = [b+ F_L - b- F_R + b+ b- (U_R - U_L)] / (b+ - b-).
+extern "C" void orcm_llf(double gamma, double bn, const double WL[7], const double WR[7], double F[7]) {
+  Side L, R;
+  side_init(gamma, bn, WL, L);
+  side_init(gamma, bn, WR, R);
+  const double lam = std::fmax(std::fabs(L.u) + L.cf, std::fabs(R.u) + R.cf);
+  for (int n = 0; n < 7; n++) F[n] = 0.5 * (L.F[n] + R.F[n]) - 0.5 * lam * (R.U[n] - L.U[n]);
+}
+extern "C" void orcm_hlle(double gamma, double bn, const double WL[7], const double WR[7], double F[7]) {
+  Side L, R;
+  side_init(gamma, bn, WL, L);
+  side_init(gamma, bn, WR, R);
+  const double cfm = std::fmax(L.cf, R.cf);
+  const double SL = std::fmin(L.u, R.u) - cfm, SR = std::fmax(L.u, R.u) + cfm;
+  const double bm = std::fmin(SL, 0.0), bp = std::fmax(SR, 0.0);
+  for (int n = 0; n < 7; n++) F[n] = ((bp * L.F[n] - bm * R.F[n]) + bp * bm * (R.U[n] - L.U[n])) / (bp - bm);
 }
 
 // van Leer PLM (Q4, as in the hydro oracle)
@@ -249,7 +271,9 @@ static long long block_stage(const orcm_pack* p, const double* Uin, const double
           else               { orc_wenoz(sL, &qm, &qp); WL[q] = qp; orc_wenoz(sR, &qm, &qp); WR[q] = qm; }
         }
       }
-      orcm_hlld(p->gamma, Ub[(5 + d) * nc + c], WL, WR, F);
+      if (p->rsolver == 1) orcm_llf(p->gamma, Ub[(5 + d) * nc + c], WL, WR, F);
+      else if (p->rsolver == 2) orcm_hlle(p->gamma, Ub[(5 + d) * nc + c], WL, WR, F);
+      else orcm_hlld(p->gamma, Ub[(5 + d) * nc + c], WL, WR, F);
       Fd[d][c] = F[0]; Fd[d][(1 + d) * nc + c] = F[1]; Fd[d][(1 + d1) * nc + c] = F[2]; Fd[d][(1 + d2) * nc + c] = F[3];
       Fd[d][4 * nc + c] = F[4]; Fd[d][5 * nc + c] = F[5]; Fd[d][6 * nc + c] = F[6];
     }
@@ -311,6 +335,12 @@ extern "C" int orcm_pack_set_recon(orcm_pack* p, int recon) {
   if (recon < 0 || recon > 3) return fail("reconstruction: 0 PLM, 1 PPM4, 2 PPMX, 3 WENOZ");
   if (recon != 0 && p->ng < 4) return fail("PPM4 / PPMX / WENOZ with face-centred fields need ng >= 4");
   p->recon = recon;
+  return 0;
+}
+extern "C" int orcm_pack_set_rsolver(orcm_pack* p, int rsolver) {
+  if (!p) return fail("null pack");
+  if (rsolver < 0 || rsolver > 2) return fail("Riemann solver: 0 HLLD, 1 LLF, 2 HLLE");
+  p->rsolver = rsolver;
   return 0;
 }
 extern "C" int orcm_pack_set_integrator(orcm_pack* p, int nstages) {

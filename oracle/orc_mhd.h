@@ -36,6 +36,7 @@ orcm_pack* orcm_pack_create(int nmb, int nx1, int nx2, int nx3, int ng, double g
 int orcm_pack_bind(orcm_pack*, double* u_a, double* u_b);   /* u_a holds U^n; both of nmb*8*nt1*nt2*nt3 doubles */
 int orcm_set_threads(orcm_pack*, int nthreads);
 int orcm_pack_set_recon(orcm_pack*, int recon);              /* 0 PLM (default), 1 PPM4, 2 PPMX, 3 WENOZ (orc.h's functions); ng >= 4 for 1-3 */
+int orcm_pack_set_rsolver(orcm_pack*, int rsolver);          /* 0 HLLD (default), 1 LLF, 2 HLLE */
 int orcm_pack_set_integrator(orcm_pack*, int nstages);      /* 2 = SSPRK(2,2) (default), 3 = SSPRK(3,3) */
 int orcm_fill_ghosts(orcm_pack*);                           /* periodic copy of all 8 variables into the ghost cells */
 int orcm_stage(orcm_pack*, int stage, double dt);           /* one stage: RK2 1: A -> B, 2: (B, A) -> A; RK3 2: (B, A) -> B, 3: (B, A) -> A */
@@ -48,6 +49,8 @@ const char* orcm_last_error(void);
 /* HLLD flux of rotated states W = (rho, u_n, v_t1, v_t2, u_g, B_t1, B_t2) with the normal field bn;
  * F = (mass, normal momentum, transverse momenta, energy, flux of B_t1, flux of B_t2). */
 void orcm_hlld(double gamma, double bn, const double WL[7], const double WR[7], double F[7]);
+void orcm_llf(double gamma, double bn, const double WL[7], const double WR[7], double F[7]);    /* P:103, same variables */
+void orcm_hlle(double gamma, double bn, const double WL[7], const double WR[7], double F[7]);
 
 #ifdef __cplusplus
 }

@@ -43,8 +43,10 @@ def lib():
     L.orcm_pack_floor_count.argtypes = [C.c_void_p]
     L.orcm_pack_destroy.argtypes = [C.c_void_p]
     L.orcm_last_error.restype = C.c_char_p
-    L.orcm_hlld.argtypes = [C.c_double, C.c_double, dp, dp, dp]
-    L.orcm_hlld.restype = None
+    for f in (L.orcm_hlld, L.orcm_llf, L.orcm_hlle):
+        f.argtypes = [C.c_double, C.c_double, dp, dp, dp]
+        f.restype = None
+    L.orcm_pack_set_rsolver.argtypes = [C.c_void_p, C.c_int]
     _lib = L
     return L
 
@@ -58,18 +60,18 @@ def _chk(rc):
         raise OrcError(lib().orcm_last_error().decode())
 
 
-def hlld(gamma, bn, WL, WR):
+def hlld(gamma, bn, WL, WR, solver="hlld"):
     F = (C.c_double * 7)()
     a = (C.c_double * 7)(*[float(v) for v in WL])
     b = (C.c_double * 7)(*[float(v) for v in WR])
-    lib().orcm_hlld(gamma, bn, a, b, F)
+    getattr(lib(), "orcm_" + solver)(gamma, bn, a, b, F)
     return np.array(F[:])
 
 
 class OrcMhdPack:
     """Oracle MHD pack over a uniform Mesh (paper_2409_16053_b200.inputs.Mesh); owns two numpy state buffers of 8 variables."""
 
-    def __init__(self, mesh, gamma, threads=1, recon=0, nstages=2):
+    def __init__(self, mesh, gamma, threads=1, recon=0, nstages=2, rsolver=0):
         L = lib()
         self.mesh = mesh
         self.nstages = nstages
@@ -86,6 +88,7 @@ class OrcMhdPack:
             _chk(L.orcm_set_threads(self._h, threads))
         _chk(L.orcm_pack_set_recon(self._h, recon))
         _chk(L.orcm_pack_set_integrator(self._h, nstages))
+        _chk(L.orcm_pack_set_rsolver(self._h, rsolver))
 
     def load(self, U):
         self.ua[...] = np.asarray(U)

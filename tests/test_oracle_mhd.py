@@ -84,6 +84,49 @@ def test_hlld_keeps_a_stationary_contact_and_upwinds_supersonic_flow(om):
     np.testing.assert_allclose(om.hlld(G53, 0.7, WL, WR), phys_flux(G53, 0.7, WR), rtol=1e-14)
 
 
+def fast_speed(g, bx, W):
+    r, u, v, w, e, by, bz = W
+    gp, b2 = g * (g - 1) * e, bx * bx + by * by + bz * bz
+    return math.sqrt(0.5 * ((gp + b2) + math.sqrt((gp + b2) ** 2 - 4 * gp * bx * bx)) / r)
+
+
+@pytest.mark.parametrize("solver", ["llf", "hlle"])
+def test_llf_and_hlle_for_mhd(om, solver):
+    """P:103 names LLF and the HLL family; in MHD variables: consistency with Eq.(5), the mirror symmetry of Eq.(5), closed forms
+    of the dissipation on a stationary contact (LLF: -(lambda/2) dU with lambda = max(|u| + cf); HLLE between +-max cf: the same
+    value), HLLE upwinds supersonic flow exactly; in the scheme both carry linear waves at second order with more dissipation than
+    HLLD (error at N = 32 between 1 and 3 times HLLD's)."""
+    rng = np.random.default_rng(11)
+    sign = np.array([-1.0, 1.0, -1.0, -1.0, -1.0, -1.0, -1.0])
+    for _ in range(200):
+        W, bx = rand_state(rng), rng.normal() * rng.integers(0, 2)
+        F, Fx = om.hlld(G53, bx, W, W, solver), phys_flux(G53, bx, W)
+        assert np.abs(F - Fx).max() <= 1e-13 * (np.abs(Fx).max() + 1.0)
+        WL, WR = rand_state(rng), rand_state(rng)
+        F = om.hlld(G53, bx, WL, WR, solver)
+        ML, MR = list(WR), list(WL)
+        ML[1], MR[1] = -ML[1], -MR[1]
+        assert np.abs(om.hlld(G53, -bx, ML, MR, solver) - sign * F).max() <= 1e-12 * (np.abs(F).max() + 1.0)
+    bx, by, bz, ug = 0.8, -0.6, 0.3, 1.5
+    WL, WR = [1.0, 0, 0, 0, ug, by, bz], [0.1, 0, 0, 0, ug, by, bz]
+    lam = max(fast_speed(G53, bx, WL), fast_speed(G53, bx, WR))
+    pt = (G53 - 1) * ug + 0.5 * (bx * bx + by * by + bz * bz)
+    F = om.hlld(G53, bx, WL, WR, solver)                     # U_R - U_L = (-0.9, 0, 0, 0, 0, 0, 0): only the mass flux is smeared
+    np.testing.assert_allclose(F, [0.5 * lam * 0.9, pt - bx * bx, -bx * by, -bx * bz, 0.0, 0.0, 0.0], rtol=1e-14, atol=1e-15)
+    if solver == "hlle":
+        WL, WR = rand_state(rng), rand_state(rng)
+        WL[1], WR[1] = 30.0, 31.0
+        np.testing.assert_allclose(om.hlld(G53, 0.7, WL, WR, solver), phys_flux(G53, 0.7, WL), rtol=1e-14)
+        WL[1], WR[1] = -31.0, -30.0
+        np.testing.assert_allclose(om.hlld(G53, 0.7, WL, WR, solver), phys_flux(G53, 0.7, WR), rtol=1e-14)
+    # in the scheme: second-order convergence of a fast and a slow linear wave, with more dissipation than HLLD
+    rs = {"llf": 1, "hlle": 2}[solver]
+    for family in ("fast", "slow"):
+        e16, e32 = (wave_error(om, family, N, rsolver=rs) for N in (16, 32))
+        d32 = wave_error(om, family, 32)
+        assert 1.2 <= math.log2(e16 / e32) <= 2.4 and d32 <= e32 * (1 + 1e-9) and e32 < 3.0 * d32, (family, e16, e32, d32)
+
+
 # ---------------------------------------------------------------- helpers --------------------------
 ZERO_A = lambda X1, X2, X3: (0 * X1 + 0 * X2 + 0 * X3,) * 3
 
@@ -104,8 +147,8 @@ def divb(mesh, U):
     return (b1[up1] - b1[s]) / dx[0] + (b2[up2] - b2[s]) / dx[1] + (b3[up3] - b3[s]) / dx[2]
 
 
-def run(om, mesh, U0, gamma=G53, cfl=0.3, nsteps=None, tend=None, threads=4, recon=0, nstages=2):
-    p = om.OrcMhdPack(mesh, gamma, threads=threads, recon=recon, nstages=nstages)
+def run(om, mesh, U0, gamma=G53, cfl=0.3, nsteps=None, tend=None, threads=4, recon=0, nstages=2, rsolver=0):
+    p = om.OrcMhdPack(mesh, gamma, threads=threads, recon=recon, nstages=nstages, rsolver=rsolver)
     p.load(U0)
     t, n = 0.0, 0
     while (nsteps is None or n < nsteps) and (tend is None or t < tend):
@@ -279,7 +322,7 @@ def mhd_eigenmode(family):
     return speed, v / np.abs(v).max(), (r, p, bx, by, bz)
 
 
-def wave_error(om, family, N, amp=1e-6, recon=0, nstages=2):
+def wave_error(om, family, N, amp=1e-6, recon=0, nstages=2, rsolver=0):
     speed, R, (r0, p0, bx, by0, bz0) = mhd_eigenmode(family)
     mesh = I.uniform_mesh((1, 1, 1), (N, 4, 4), 3 if recon == 0 else 4)
     k = 2 * math.pi
@@ -293,7 +336,7 @@ def wave_error(om, family, N, amp=1e-6, recon=0, nstages=2):
         return (0 * c, -amp * R[6] * c, amp * R[5] * c)
 
     U0 = I.make_state_mhd(mesh, prim, A, (bx, by0, bz0)).numpy()
-    U = run(om, mesh, U0, tend=1.0 / speed, recon=recon, nstages=nstages)
+    U = run(om, mesh, U0, tend=1.0 / speed, recon=recon, nstages=nstages, rsolver=rsolver)
     a = act(mesh)
     return math.sqrt(sum(np.abs(U[a][0, n] - U0[a][0, n]).mean() ** 2 for n in range(8)))
 
