@@ -180,7 +180,10 @@ def run_mhd(args):
     nst = args.integrator
     mesh, prim, A, B0 = I.mhd_workload(args.workload, ng=3 if recon == 0 else 4)
     U0 = I.make_state_mhd(mesh, prim, A, B0, device=dev)
-    pack = ak_mhd.MhdPack(mesh, I.GAMMA, device=dev, recon=recon, nstages=nst)
+    rs = {"hllc": 0, "llf": 1, "hlle": 2}.get(args.rsolver)
+    if rs is None or (rs and recon):
+        raise SystemExit("MHD workloads: --rsolver llf | hlle (PLM only); the default is HLLD")
+    pack = ak_mhd.MhdPack(mesh, I.GAMMA, device=dev, recon=recon, nstages=nst, rsolver=rs)
     pack.load(U0)
     ncell, state_bytes = mesh.ncells_active, U0.numel() * 8
     sampler = ClockSampler(local)
@@ -228,7 +231,7 @@ def run_mhd(args):
         "metric": "3D MHD cell-updates/sec (fp64)", "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
-        "config": {"workload": f"{args.workload}: MHD + CT, {['PLM', 'PPM4', 'PPMX', 'WENOZ'][recon]} + HLLD, SSPRK{nst}, {mesh.nmb} MeshBlocks of {mesh.nx[0]}^3, ng {mesh.ng}, Mach-0.5 modes + mean field",
+        "config": {"workload": f"{args.workload}: MHD + CT, {['PLM', 'PPM4', 'PPMX', 'WENOZ'][recon]} + {['HLLD', 'LLF', 'HLLE'][rs]}, SSPRK{nst}, {mesh.nmb} MeshBlocks of {mesh.nx[0]}^3, ng {mesh.ng}, Mach-0.5 modes + mean field",
                    "cells": ncell, "state_bytes": state_bytes, "l2_policy": "inputs larger than L2" if state_bytes > 4e8 else "state fits L2",
                    "parallelism": "single GPU"},
         "roofline": {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"], "traffic": None,

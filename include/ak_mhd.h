@@ -5,7 +5,7 @@
  * as area-averages on cell-faces, and the constrained transport (CT) algorithm of Evans & Hawley (1988) is used to preserve the
  * divergence-free constraint with upwinded electric fields calculated using the method of Gardiner & Stone (2005, 2008)"
  * (P:116); HLLD Riemann solver.  Readings: DESIGN.md Q33-Q37.  Scope of this cut: uniform single-level periodic packs;
- * PLM (van Leer), PPM4, PPMX or WENOZ reconstruction of the primitives; HLLD; SSPRK(2,2) or SSPRK(3,3) -- the options of the
+ * PLM (van Leer), PPM4, PPMX or WENOZ reconstruction of the primitives; HLLD (LLF, HLLE with PLM); SSPRK(2,2) or SSPRK(3,3) -- the options of the
  * paper's MHD tests and runs; the kernels are not fused (face fluxes and corner EMFs pass through a caller-owned
  * work buffer in device memory).
  *
@@ -44,6 +44,8 @@ int akm_pack_set_exact(akm_pack*, int on);
 /* Reconstruction: 0 PLM (default), 1 PPM4, 2 PPMX, 3 WENOZ (the codes of ak.h; Q29, Q30); 1-3 need ng >= 4 (-1 otherwise);
  * -3 for any other code. */
 int akm_pack_set_recon(akm_pack*, int recon);
+/* Riemann solver: 0 HLLD (default), 1 LLF, 2 HLLE (in HLLD's variables and outer wave speeds); 1 and 2 with PLM only (-3). */
+int akm_pack_set_rsolver(akm_pack*, int rsolver);
 /* Integrator: 2 = SSPRK(2,2) (default), 3 = SSPRK(3,3); between steps only (-2 inside a step). */
 int akm_pack_set_integrator(akm_pack*, int nstages);
 

@@ -14,7 +14,7 @@ from . import ak as _ak
 SYMBOLS = [
     "akm_pack_create", "akm_pack_state_bytes", "akm_pack_work_bytes", "akm_pack_bind", "akm_fill_ghosts", "akm_stage",
     "akm_new_dt", "akm_step", "akm_pack_current", "akm_pack_floor_count", "akm_pack_launch_count", "akm_pack_destroy",
-    "akm_last_error", "akm_pack_set_exact", "akm_pack_set_recon", "akm_pack_set_integrator",
+    "akm_last_error", "akm_pack_set_exact", "akm_pack_set_recon", "akm_pack_set_integrator", "akm_pack_set_rsolver",
 ]
 _ready = False
 
@@ -38,7 +38,7 @@ def lib():
             "akm_new_dt": (i, [vp, d, dp]), "akm_step": (i, [vp, d, d, dp]),
             "akm_pack_current": (vp, [vp]), "akm_pack_floor_count": (ll, [vp]), "akm_pack_launch_count": (ll, [vp]),
             "akm_pack_destroy": (i, [vp]), "akm_last_error": (C.c_char_p, []), "akm_pack_set_exact": (i, [vp, i]),
-            "akm_pack_set_recon": (i, [vp, i]), "akm_pack_set_integrator": (i, [vp, i]),
+            "akm_pack_set_recon": (i, [vp, i]), "akm_pack_set_integrator": (i, [vp, i]), "akm_pack_set_rsolver": (i, [vp, i]),
         }
         for name, (res, args) in sig.items():
             fn = getattr(L, name)
@@ -55,7 +55,7 @@ def _chk(rc):
 class MhdPack:
     """An MHD MeshBlockPack (uniform periodic mesh) bound to torch-owned device buffers; methods map 1:1 to akm_* calls."""
 
-    def __init__(self, mesh, gamma, device="cuda:0", stream=None, exact=False, recon=0, nstages=2):
+    def __init__(self, mesh, gamma, device="cuda:0", stream=None, exact=False, recon=0, nstages=2, rsolver=0):
         L = lib()
         if not torch.cuda.is_available():
             raise AkmError("no CUDA device: the MHD path has no CPU fallback")
@@ -80,6 +80,8 @@ class MhdPack:
             _chk(L.akm_pack_set_recon(self._h, recon))
         if nstages != 2:
             _chk(L.akm_pack_set_integrator(self._h, nstages))
+        if rsolver:
+            _chk(L.akm_pack_set_rsolver(self._h, rsolver))
         self.nstages = nstages
 
     def _bind(self):

@@ -173,6 +173,47 @@ __device__ void hlld(double gamma, double bn, const double WL[7], const double W
   for (int n = 0; n < 7; n++) F[n] = FK[n] + SsK * Uss[n] - (SsK - SK) * Us[n] - SK * UK[n];
 }
 
+// LLF and HLLE in the same variables: F = (F_L + F_R)/2 - (lambda/2)(U_R - U_L) with lambda = max(|u| + cf); the HLL
+// flux between HLLD's outer speeds, b- = min(S_L, 0), b+ = max(S_R, 0).
+template <bool X>
+__device__ void llf(double gamma, double bn, const double WL[7], const double WR[7], double F[7]) {
+  Side L, R;
+  side_init<X>(gamma, bn, WL, L);
+  side_init<X>(gamma, bn, WR, R);
+  const double lam = fmax(fabs(L.u) + L.cf, fabs(R.u) + R.cf);
+  double UL[7], FL[7], UR[7], FR[7];
+  cons_flux(bn, L, UL, FL);
+  cons_flux(bn, R, UR, FR);
+#pragma unroll
+  for (int n = 0; n < 7; n++) F[n] = 0.5 * (FL[n] + FR[n]) - 0.5 * lam * (UR[n] - UL[n]);
+}
+template <bool X>
+__device__ void hlle(double gamma, double bn, const double WL[7], const double WR[7], double F[7]) {
+  Side L, R;
+  side_init<X>(gamma, bn, WL, L);
+  side_init<X>(gamma, bn, WR, R);
+  const double cfm = fmax(L.cf, R.cf);
+  const double SL = fmin(L.u, R.u) - cfm, SR = fmax(L.u, R.u) + cfm;
+  const double bm = fmin(SL, 0.0), bp = fmax(SR, 0.0);
+  double UL[7], FL[7], UR[7], FR[7];
+  cons_flux(bn, L, UL, FL);
+  cons_flux(bn, R, UR, FR);
+  if constexpr (X) {
+#pragma unroll
+    for (int n = 0; n < 7; n++) F[n] = ((bp * FL[n] - bm * FR[n]) + bp * bm * (UR[n] - UL[n])) / (bp - bm);
+  } else {
+    const double inv = rcp_fast(bp - bm);
+#pragma unroll
+    for (int n = 0; n < 7; n++) F[n] = ((bp * FL[n] - bm * FR[n]) + bp * bm * (UR[n] - UL[n])) * inv;
+  }
+}
+template <bool X, int RS>
+__device__ __forceinline__ void riemann(double gamma, double bn, const double WL[7], const double WR[7], double F[7]) {
+  if constexpr (RS == 1) llf<X>(gamma, bn, WL, WR, F);
+  else if constexpr (RS == 2) hlle<X>(gamma, bn, WL, WR, F);
+  else hlld<X>(gamma, bn, WL, WR, F);
+}
+
 template <bool X>
 __device__ __forceinline__ void plm(double qm1, double q0, double qp1, double& qm, double& qp) {
   const double dL = q0 - qm1, dR = qp1 - q0, prod = dL * dR;
@@ -318,7 +359,7 @@ __global__ void __launch_bounds__(256) prim_kernel(Dev P, const double* __restri
 // Occupancy (measured at 256^3): the exact flavour waits on its IEEE division chains and runs best with 32 warps per SM (64
 // registers, 240 B spilled); the fast flavour is bound by the FP64 pipe and runs best without spills (96 registers, 20 warps:
 // 1.49 -> 1.67 G cell-updates/s against 8 CTAs per SM).
-template <int D, bool X, int RECON>
+template <int D, bool X, int RECON, int RS>
 __global__ void __launch_bounds__(128, X ? 8 : (RECON == 0 ? 5 : 4)) flux_kernel(Dev P, const double* __restrict__ U) {
   constexpr int D1 = (D + 1) % 3, D2 = (D + 2) % 3;
   const int m = blockIdx.y;
@@ -334,7 +375,7 @@ __global__ void __launch_bounds__(128, X ? 8 : (RECON == 0 ? 5 : 4)) flux_kernel
   double WL[7], WR[7], F[7];
 #pragma unroll
   for (int q = 0; q < 7; q++) face_states<X, RECON>(Wb + var[q] * nc, c, st, WL[q], WR[q]);
-  hlld<X>(P.gamma, U[(long long)m * 8 * nc + (5 + D) * nc + c], WL, WR, F);
+  riemann<X, RS>(P.gamma, U[(long long)m * 8 * nc + (5 + D) * nc + c], WL, WR, F);
   double* Fb = P.F[D] + (long long)m * 7 * nc;
   Fb[c] = F[0]; Fb[(1 + D) * nc + c] = F[1]; Fb[(1 + D1) * nc + c] = F[2]; Fb[(1 + D2) * nc + c] = F[3];
   Fb[4 * nc + c] = F[4]; Fb[5 * nc + c] = F[5]; Fb[6 * nc + c] = F[6];
@@ -515,7 +556,7 @@ struct akm_pack {
   cudaStream_t stream = nullptr;
   int cur = 0, device = -1;
   bool bound = false, ghosts_ok = false;
-  int recon = 0, nstages = 2;  // akm_pack_set_recon (0 PLM, 1 PPM4, 2 PPMX, 3 WENOZ), akm_pack_set_integrator (2, 3)
+  int recon = 0, nstages = 2, rsolver = 0;  // akm_pack_set_rsolver (0 HLLD, 1 LLF, 2 HLLE); akm_pack_set_recon (0 PLM, 1 PPM4, 2 PPMX, 3 WENOZ), akm_pack_set_integrator (2, 3)
   bool exact = false;          // akm_pack_set_exact: IEEE division / sqrt in the definition's order (bit-identical, slower)
   long long launches = 0;
 };
@@ -623,7 +664,15 @@ extern "C" int akm_pack_set_recon(akm_pack* p, int recon) {
   if (!p) return fail(-1, "null pack");
   if (recon < 0 || recon > 3) return fail(-3, "reconstruction: 0 PLM, 1 PPM4, 2 PPMX, 3 WENOZ");
   if (recon != 0 && p->d.ng < 4) return fail(-1, "PPM4 / PPMX / WENOZ with face-centred fields need ng >= 4");
+  if (recon != 0 && p->rsolver != 0) return fail(-3, "LLF / HLLE are built with PLM only");
   p->recon = recon;
+  return 0;
+}
+extern "C" int akm_pack_set_rsolver(akm_pack* p, int rsolver) {
+  if (!p) return fail(-1, "null pack");
+  if (rsolver < 0 || rsolver > 2) return fail(-3, "Riemann solver: 0 HLLD, 1 LLF, 2 HLLE");
+  if (rsolver != 0 && p->recon != 0) return fail(-3, "LLF / HLLE are built with PLM only");
+  p->rsolver = rsolver;
   return 0;
 }
 extern "C" int akm_pack_set_integrator(akm_pack* p, int nstages) {
@@ -635,18 +684,20 @@ extern "C" int akm_pack_set_integrator(akm_pack* p, int nstages) {
 }
 
 namespace {
-template <bool X, int RECON>
+template <bool X, int RECON, int RS>
 void launch_sweeps(const akm_pack* p, dim3 grid, const double* Uin) {
-  flux_kernel<0, X, RECON><<<grid, 128, 0, p->stream>>>(p->d, Uin);
-  flux_kernel<1, X, RECON><<<grid, 128, 0, p->stream>>>(p->d, Uin);
-  flux_kernel<2, X, RECON><<<grid, 128, 0, p->stream>>>(p->d, Uin);
+  flux_kernel<0, X, RECON, RS><<<grid, 128, 0, p->stream>>>(p->d, Uin);
+  flux_kernel<1, X, RECON, RS><<<grid, 128, 0, p->stream>>>(p->d, Uin);
+  flux_kernel<2, X, RECON, RS><<<grid, 128, 0, p->stream>>>(p->d, Uin);
 }
 template <bool X>
 void launch_sweeps_recon(const akm_pack* p, dim3 grid, const double* Uin) {
-  if (p->recon == 1) launch_sweeps<X, 1>(p, grid, Uin);
-  else if (p->recon == 2) launch_sweeps<X, 2>(p, grid, Uin);
-  else if (p->recon == 3) launch_sweeps<X, 3>(p, grid, Uin);
-  else launch_sweeps<X, 0>(p, grid, Uin);
+  if (p->rsolver == 1) launch_sweeps<X, 0, 1>(p, grid, Uin);            // LLF / HLLE: PLM only (akm_pack_set_rsolver)
+  else if (p->rsolver == 2) launch_sweeps<X, 0, 2>(p, grid, Uin);
+  else if (p->recon == 1) launch_sweeps<X, 1, 0>(p, grid, Uin);
+  else if (p->recon == 2) launch_sweeps<X, 2, 0>(p, grid, Uin);
+  else if (p->recon == 3) launch_sweeps<X, 3, 0>(p, grid, Uin);
+  else launch_sweeps<X, 0, 0>(p, grid, Uin);
 }
 }  // namespace
 

@@ -64,9 +64,9 @@ def turbulent_state(mesh, mach=0.5, shift=(0.0, 0.0, 0.0)):
     return I.make_state_mhd(mesh, prim, A, (0.4, -0.3, 0.2))
 
 
-def lockstep(om, akm, mesh, U0, gamma, nsteps, cfl=0.3, exact=False, recon=0, nstages=2):
-    po = om.OrcMhdPack(mesh, gamma, threads=P.NTHREADS, recon=recon, nstages=nstages)
-    pg = akm.MhdPack(mesh, gamma, exact=exact, recon=recon, nstages=nstages)
+def lockstep(om, akm, mesh, U0, gamma, nsteps, cfl=0.3, exact=False, recon=0, nstages=2, rsolver=0):
+    po = om.OrcMhdPack(mesh, gamma, threads=P.NTHREADS, recon=recon, nstages=nstages, rsolver=rsolver)
+    pg = akm.MhdPack(mesh, gamma, exact=exact, recon=recon, nstages=nstages, rsolver=rsolver)
     po.load(U0.numpy())
     pg.load(U0)
     a = act(mesh)
@@ -147,6 +147,32 @@ def test_higher_order_options_match_the_oracle(om, akm, nrb, nx, recon, nstages,
     assert pg.launch_count() == 4 * (2 + nstages * 7) + 1                  # (+ the fill above)
     with pytest.raises(akm.AkmError):
         akm.MhdPack(I.uniform_mesh((1, 1, 1), (8, 8, 8), 3), G53, recon=recon or 1)   # ng < 4
+
+
+@pytest.mark.parametrize("exact", [False, True])
+@pytest.mark.parametrize("rsolver", [1, 2])
+def test_llf_and_hlle_match_the_oracle(om, akm, rsolver, exact):
+    """LLF and HLLE for MHD (PLM, RK2) on the ragged 6-block pack and along a Brio-Wu tube: same bars as HLLD."""
+    mesh = I.uniform_mesh((2, 1, 3), (24, 10, 6), 3)
+    U0 = turbulent_state(mesh)
+    errs, po, pg = lockstep(om, akm, mesh, U0, G53, 5, exact=exact, rsolver=rsolver)
+    mesh1, B0 = brio_wu(64, 1)
+    p1 = om.OrcMhdPack(mesh1, 2.0, threads=P.NTHREADS, rsolver=rsolver)
+    g1 = akm.MhdPack(mesh1, 2.0, exact=exact, rsolver=rsolver)
+    p1.load(B0); g1.load(torch.from_numpy(B0))
+    t = 0.0
+    while t < 0.05:
+        dt = min(p1.new_dt(0.3), 0.05 - t)
+        p1.step(0.3, dt); g1.step(0.3, dt)
+        t += dt
+    a = act(mesh1)
+    e = q_mhd(g1.current().cpu().numpy()[a], p1.current()[a], 2.0)
+    P.report(f"[parity] MHD {['', 'LLF', 'HLLE'][rsolver]} exact={exact}: turbulent field worst per step {max(errs):.3e}, Brio-Wu {e:.3e} (bar {TOL_RUN:.0e})")
+    assert max(errs) <= TOL_RUN and e <= TOL_RUN and (not exact or (max(errs) == 0.0 and e == 0.0))
+    assert g1.floor_count() == 0 and pg.floor_count() == 0
+    with pytest.raises(akm.AkmError) as ei:                                # LLF / HLLE are built with PLM only
+        akm.MhdPack(I.uniform_mesh((1, 1, 1), (8, 8, 8), 4), G53, recon=1, rsolver=rsolver)
+    assert "PLM only" in str(ei.value)
 
 
 @pytest.mark.parametrize("exact", [False, True])
