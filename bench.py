@@ -113,13 +113,13 @@ def cpu_baseline(threads=1, target_s=12.0):
                       f"{el:.1f} s, single-threaded C++ oracle"}
 
 
-def cpu_baseline_mhd(recon, nst, target_s=10.0):
+def cpu_baseline_mhd(recon, nst, rsolver=0, target_s=10.0):
     """The MHD oracle as it stands on a bounded sample of the MHD recipe (mhd_64: 8 MeshBlocks of 32^3), one thread."""
     from paper_2409_16053_b200 import inputs as I
     from oracle import orc_mhd
     orc_mhd.build()
     mesh, prim, A, B0 = I.mhd_workload("mhd_64", ng=3 if recon == 0 else 4)
-    p = orc_mhd.OrcMhdPack(mesh, I.GAMMA, recon=recon, nstages=nst)
+    p = orc_mhd.OrcMhdPack(mesh, I.GAMMA, recon=recon, nstages=nst, rsolver=rsolver)
     p.load(I.make_state_mhd(mesh, prim, A, B0).numpy())
     p.step(I.CFL)
     t0, n = time.perf_counter(), 0
@@ -237,7 +237,7 @@ def run_mhd(args):
         "roofline": {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"], "traffic": None,
                      "peak_source": which + " (MEASURED_PEAKS.json hbm_gbs)", "kernel": "akm_stage (six kernels: prim, 3 x flux, emf, update)",
                      "kernel_ms": stage_ms, "kernel_share_of_step": nst * stage_ms * args.steps / elapsed_ms, "algorithmic_bytes_per_launch": alg},
-        "cpu_baseline": None if args.no_cpu else cpu_baseline_mhd(recon, nst), "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        "cpu_baseline": None if args.no_cpu else cpu_baseline_mhd(recon, nst, rs), "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
         "stage_ms": st_ms, "floor_activations": floors,
     }))
 
