@@ -381,3 +381,21 @@ def test_the_papers_mhd_convergence_orders_on_the_gpu(akm):
     assert 1.6 <= math.log2(p32 / p64) <= 2.4, (p32, p64)
     P.report(f"[property] MHD linear waves on the GPU: WENOZ + RK3 fast-wave rate {math.log2(f16 / f32):.2f}, PLM + RK2 Alfven rate {math.log2(p32 / p64):.2f}; "
              f"Alfven / slow with WENOZ / PPMX + RK3 >= 3.5")
+
+
+@pytest.mark.parametrize("recon,ng", [(0, 3), (3, 4)])
+def test_block_decomposition_does_not_change_the_result_on_the_gpu(akm, recon, ng):
+    """The same periodic problem cut into 1, 4 and 12 MeshBlocks gives bit-identical global states on the CUDA path (default
+    arithmetic): every face and corner is computed from the same numbers in the same order whichever block owns it."""
+    from tests.test_oracle_mhd import assemble
+    outs = []
+    for nrb, nx in (((1, 1, 1), (16, 12, 8)), ((2, 2, 1), (8, 6, 8)), ((2, 3, 2), (8, 4, 4))):
+        mesh = I.uniform_mesh(nrb, nx, ng)
+        U0 = turbulent_state(mesh, shift=(0.0137, 0.0291, 0.0173))
+        pg = akm.MhdPack(mesh, G53, recon=recon)
+        pg.load(U0)
+        for _ in range(3):
+            pg.step(0.3, 2e-3)
+        outs.append(assemble(mesh, pg.current().cpu().numpy()))
+        assert pg.floor_count() == 0
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])

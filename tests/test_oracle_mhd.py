@@ -272,6 +272,43 @@ def test_corner_emfs_are_continuous_where_a_mass_flux_changes_sign(om):
     assert np.abs(outs[0] - outs[2]).max() > 1e-6                           # (the velocity does matter once it is not round-off)
 
 
+def assemble(mesh, U):
+    """Active cells of every block -> one global (8, N3, N2, N1) array (a face field sits on the lower face of its cell)."""
+    g, nx = mesh.ng, mesh.nx
+    G = np.empty((8, mesh.nrb[2] * nx[2], mesh.nrb[1] * nx[1], mesh.nrb[0] * nx[0]))
+    for m, (_, l1, l2, l3) in enumerate(mesh.blocks):
+        G[:, l3 * nx[2]:(l3 + 1) * nx[2], l2 * nx[1]:(l2 + 1) * nx[1], l1 * nx[0]:(l1 + 1) * nx[0]] = U[m][:, g:-g, g:-g, g:-g]
+    return G
+
+
+@pytest.mark.parametrize("recon,ng", [(0, 3), (3, 4)])
+def test_block_decomposition_does_not_change_the_result(om, recon, ng):
+    """The same periodic problem cut into 1, 4 and 12 MeshBlocks (the pack is an implementation device, not part of the
+    scheme): bit-identical global states after three steps -- ghost fill, face ownership at block boundaries and the corner EMFs
+    computed independently by neighbouring blocks all have to agree for that."""
+    k = 2 * math.pi
+
+    def A(X1, X2, X3):
+        return (0.1 * torch.sin(k * X2) * torch.cos(k * X3) + 0 * X1, 0.1 * torch.sin(k * X3 + 0.3) * torch.cos(k * X1) + 0 * X2,
+                0.1 * torch.cos(k * X1 + 0.7) * torch.sin(k * X2) + 0 * X3)
+
+    prim = lambda X1, X2, X3: (1.0 + 0.2 * torch.sin(k * X1) * torch.cos(k * X2) + 0 * X3, 0.3 * torch.sin(k * X2 + 0.1) + 0 * X1 + 0 * X3,
+                               -0.2 * torch.cos(k * X3) + 0 * X1 + 0 * X2, 0.1 * torch.sin(k * X1 + 1.0) + 0 * X2 + 0 * X3,
+                               0.6 + 0 * X1 + 0 * X2 + 0 * X3)
+    outs = []
+    for nrb, nx in (((1, 1, 1), (16, 12, 8)), ((2, 2, 1), (8, 6, 8)), ((2, 3, 2), (8, 4, 4))):
+        mesh = I.uniform_mesh(nrb, nx, ng)
+        U0 = I.make_state_mhd(mesh, prim, A, (0.3, -0.2, 0.1)).numpy()
+        p = om.OrcMhdPack(mesh, G53, recon=recon)
+        p.load(U0)
+        for _ in range(3):
+            p.step(0.3, 2e-3)
+        outs.append(assemble(mesh, p.current()))
+        p.close()
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+    assert np.abs(outs[0][0] - 1.0).max() > 0.1                             # (a non-trivial state)
+
+
 def test_uniform_magnetised_state_is_preserved_bit_exactly(om):
     mesh = I.uniform_mesh((2, 1, 2), (6, 8, 4), 3)
     prim = lambda X1, X2, X3: (1.3 + 0 * X1 + 0 * X2 + 0 * X3, 0.4 + 0 * X1 + 0 * X2 + 0 * X3, -0.7 + 0 * X1 + 0 * X2 + 0 * X3,
