@@ -15,9 +15,13 @@
  * the lower face of the first ghost cell beyond it).  All pointers are HOST pointers owned by the caller.
  *
  * Pins (tests/test_oracle_mhd.py): HLLD consistency with Eq.(5), mirror symmetry, exact stationary contact and (B = 0) Sod
- * convergence to the exact Riemann solution; div B = 0 to round-off; conservation of mass, momentum, energy and mean field;
- * uniform state preserved bit-exactly; plane-parallel flow stays plane-parallel and direction-independent bit for bit; second-
- * order convergence of fast, Alfven and slow linear waves whose eigenvectors the test computes numerically.
+ * convergence to the exact Riemann solution; LLF / HLLE consistency, mirror symmetry, closed-form dissipation on a stationary contact,
+ * exact supersonic upwinding (HLLE); div B = 0 to round-off; conservation of mass, momentum, energy and mean field; uniform state
+ * preserved bit-exactly; plane-parallel flow stays plane-parallel and direction-independent bit for bit; results independent of
+ * the block decomposition bit for bit; the corner EMFs continuous where a mass flux changes sign (Q36); second-order convergence
+ * of fast, Alfven and slow linear waves, along x1 and obliquely, whose eigenvectors the test computes numerically, and
+ * the paper's statement about the higher-order options: RK3 + WENOZ / PPMX converge at fourth order on Alfven and slow
+ * waves, the fast wave at second order, PPM4 at second order.
  * PARITY UNPINNED beyond those properties: the HLLD wave-speed estimate and degenerate-case thresholds (Q34), the ramp
  * width of the upwinding rule of the corner EMFs (Q36).
  */
