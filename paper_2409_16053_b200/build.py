@@ -3,6 +3,7 @@
     python -m paper_2409_16053_b200.build [--force]
 
 nvcc cross-compiles without a GPU.  ak_exact.cu (ghost fill, dt) and ak_stage.cu (stage kernels, flux correction, FOFC)
+(and mhd/ak_mhd.cu; only mhd/ak_mhd_fast.cu, the MHD sweeps of the default arithmetic flavour, allows contraction)
 are compiled with -fmad=false: no contraction behind the source's back, every fused multiply-add of the stage kernel is
 written out, so the same face solved by two tiles gives the same bits.  -lineinfo maps ncu's source page to these files.
 """
@@ -23,6 +24,7 @@ UNITS = {                      # translation unit -> extra flags
     "ak_exact.cu": ["-fmad=false"],
     "ak_stage.cu": ["-fmad=false", "-Xptxas", "-v"],
     "mhd/ak_mhd.cu": ["-fmad=false", "-Xptxas", "-v"],        # MHD + CT (include/ak_mhd.h)
+    "mhd/ak_mhd_fast.cu": ["-I", os.path.join(CSRC, "mhd"), "-Xptxas", "-v"],   # its default-flavour sweeps, contraction allowed
 }
 
 

@@ -20,15 +20,7 @@
 #include <string>
 #include <vector>
 
-namespace {
-
-thread_local std::string g_err;
-int fail(int code, const std::string& msg) { g_err = msg; return code; }
-int cuda_fail(cudaError_t e, const char* where) { return fail(-4, std::string(where) + ": " + cudaGetErrorString(e)); }
-#define AKM_CUDA(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, where); } while (0)
-
-constexpr double RHO_FLOOR = 1e-20, P_FLOOR = 1e-20;
-
+namespace akm {
 // plain-data view of the pack for the kernels
 struct Dev {
   int nmb, nx[3], ng, nt[3], nrb[3];
@@ -41,6 +33,23 @@ struct Dev {
   double* Ec;                 // [nmb][3][ncell] corner EMFs
   unsigned long long* cells;  // [0] min dt as ordered bits, [1] floor count, [2] non-finite count
 };
+// The flux sweeps of the default arithmetic flavour live in a second translation unit (ak_mhd_fast.cu = this file with
+// AKM_FAST_TU defined) compiled WITHOUT -fmad=false: the compiler may contract a*b+c there (-17 % FP64-pipe instructions with
+// PLM, -20 % with WENOZ; the sweeps are bound by that pipe).  The verification flavour and every other kernel stay in the
+// -fmad=false unit, where each operation is the one written.
+void launch_sweeps_fast(const Dev& d, int recon, int rsolver, dim3 grid, cudaStream_t stream, const double* Uin);
+}  // namespace akm
+
+namespace {
+using akm::Dev;
+
+thread_local std::string g_err;
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+int cuda_fail(cudaError_t e, const char* where) { return fail(-4, std::string(where) + ": " + cudaGetErrorString(e)); }
+#define AKM_CUDA(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, where); } while (0)
+
+constexpr double RHO_FLOOR = 1e-20, P_FLOOR = 1e-20;
+
 
 // ---- division and square root in two flavours --------------------------------------------------------------------
 // X = true: IEEE division and sqrt in the definition's operation order -- the results are bit-identical to the definition
@@ -381,6 +390,7 @@ __global__ void __launch_bounds__(128, X ? 8 : (RECON == 0 ? 5 : 4)) flux_kernel
   Fb[4 * nc + c] = F[4]; Fb[5 * nc + c] = F[5]; Fb[6 * nc + c] = F[6];
 }
 
+#ifndef AKM_FAST_TU
 // upwinded (face - centre) EMF difference (Q36): weight w of the lower side = 1/2 + nu clipped to [0, 1] with
 // nu = 1024 dt F_mass / (dx (rho_1 + rho_2)) -- pure upwind once the contact crosses 2^-10 of a cell per step, the mean at
 // rest, continuous in between (a mass flux at round-off level does not decide the result).  k = 1024 dt / dx.
@@ -684,20 +694,20 @@ extern "C" int akm_pack_set_integrator(akm_pack* p, int nstages) {
 }
 
 namespace {
-template <bool X, int RECON, int RS>
-void launch_sweeps(const akm_pack* p, dim3 grid, const double* Uin) {
-  flux_kernel<0, X, RECON, RS><<<grid, 128, 0, p->stream>>>(p->d, Uin);
-  flux_kernel<1, X, RECON, RS><<<grid, 128, 0, p->stream>>>(p->d, Uin);
-  flux_kernel<2, X, RECON, RS><<<grid, 128, 0, p->stream>>>(p->d, Uin);
+template <int RECON, int RS>
+void launch_sweeps_exact(const akm_pack* p, dim3 grid, const double* Uin) {
+  flux_kernel<0, true, RECON, RS><<<grid, 128, 0, p->stream>>>(p->d, Uin);
+  flux_kernel<1, true, RECON, RS><<<grid, 128, 0, p->stream>>>(p->d, Uin);
+  flux_kernel<2, true, RECON, RS><<<grid, 128, 0, p->stream>>>(p->d, Uin);
 }
-template <bool X>
-void launch_sweeps_recon(const akm_pack* p, dim3 grid, const double* Uin) {
-  if (p->rsolver == 1) launch_sweeps<X, 0, 1>(p, grid, Uin);            // LLF / HLLE: PLM only (akm_pack_set_rsolver)
-  else if (p->rsolver == 2) launch_sweeps<X, 0, 2>(p, grid, Uin);
-  else if (p->recon == 1) launch_sweeps<X, 1, 0>(p, grid, Uin);
-  else if (p->recon == 2) launch_sweeps<X, 2, 0>(p, grid, Uin);
-  else if (p->recon == 3) launch_sweeps<X, 3, 0>(p, grid, Uin);
-  else launch_sweeps<X, 0, 0>(p, grid, Uin);
+void launch_sweeps(const akm_pack* p, dim3 grid, const double* Uin) {
+  if (!p->exact) { akm::launch_sweeps_fast(p->d, p->recon, p->rsolver, grid, p->stream, Uin); return; }
+  if (p->rsolver == 1) launch_sweeps_exact<0, 1>(p, grid, Uin);      // LLF / HLLE: PLM only (akm_pack_set_rsolver)
+  else if (p->rsolver == 2) launch_sweeps_exact<0, 2>(p, grid, Uin);
+  else if (p->recon == 1) launch_sweeps_exact<1, 0>(p, grid, Uin);
+  else if (p->recon == 2) launch_sweeps_exact<2, 0>(p, grid, Uin);
+  else if (p->recon == 3) launch_sweeps_exact<3, 0>(p, grid, Uin);
+  else launch_sweeps_exact<0, 0>(p, grid, Uin);
 }
 }  // namespace
 
@@ -736,7 +746,7 @@ extern "C" int akm_stage(akm_pack* p, int stage, double dt) {
   const long long nact = (long long)d.nx[0] * d.nx[1] * d.nx[2];
   dim3 gact((unsigned)((nact + 127) / 128), (unsigned)d.nmb);
   prim_kernel<<<gall256, 256, 0, p->stream>>>(d, Uin);
-  if (p->exact) launch_sweeps_recon<true>(p, gall128, Uin); else launch_sweeps_recon<false>(p, gall128, Uin);
+  launch_sweeps(p, gall128, Uin);
   const double k0 = 1024.0 * dt / d.dx[0], k1 = 1024.0 * dt / d.dx[1], k2 = 1024.0 * dt / d.dx[2];
   if (p->exact) emf_kernel<true><<<gall128, 128, 0, p->stream>>>(d, k0, k1, k2);
   else emf_kernel<false><<<gall128, 128, 0, p->stream>>>(d, k0, k1, k2);
@@ -792,3 +802,23 @@ extern "C" long long akm_pack_floor_count(akm_pack* p) {
   return (long long)n;
 }
 extern "C" int akm_pack_destroy(akm_pack* p) { delete p; return 0; }
+#else   // AKM_FAST_TU: only the sweeps of the default flavour
+}  // namespace
+
+namespace akm {
+template <int RECON, int RS>
+static void sweeps(const Dev& d, dim3 grid, cudaStream_t st, const double* Uin) {
+  flux_kernel<0, false, RECON, RS><<<grid, 128, 0, st>>>(d, Uin);
+  flux_kernel<1, false, RECON, RS><<<grid, 128, 0, st>>>(d, Uin);
+  flux_kernel<2, false, RECON, RS><<<grid, 128, 0, st>>>(d, Uin);
+}
+void launch_sweeps_fast(const Dev& d, int recon, int rsolver, dim3 grid, cudaStream_t st, const double* Uin) {
+  if (rsolver == 1) sweeps<0, 1>(d, grid, st, Uin);                  // LLF / HLLE: PLM only (akm_pack_set_rsolver)
+  else if (rsolver == 2) sweeps<0, 2>(d, grid, st, Uin);
+  else if (recon == 1) sweeps<1, 0>(d, grid, st, Uin);
+  else if (recon == 2) sweeps<2, 0>(d, grid, st, Uin);
+  else if (recon == 3) sweeps<3, 0>(d, grid, st, Uin);
+  else sweeps<0, 0>(d, grid, st, Uin);
+}
+}  // namespace akm
+#endif
